@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py -- GDN chunk-forward throughput on B200 (BASELINE.json's metric and workload).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2|3] [--mode token|frame]
+
+A "step" is one pass of the whole hot path (one gdn_forward_chunk call = one streaming chunk) over one
+batch of synthetic input; the state of step i is the state_in of step i+1 (a real stream).  Prints ONE
+JSON line (rank 0).  See DESIGN.md "Measurement" for what every field means.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "gdn_chunk_fwd_tokens_per_s"
+UNIT = "tokens/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+L2_BYTES = 126e6
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            d = json.loads(p.read_text())
+            return {k: float(d[k]) for k in FALLBACK_PEAKS}, "measured"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def workload(args):
+    from paper_2605_30409_b200 import inputs as gin
+    wl = gin.config(args.config, frame=(args.mode == "frame"), chunk=args.chunk)
+    return wl
+
+
+def flops_per_call(wl, chunk):
+    """Algorithmic flops: mode T 6d^2 + 10 C d per token-head; mode F 6 d^2 per token-head
+    + 2 d^3 per frame-head.  (Inverse and element-wise work excluded.)"""
+    d = wl.d_k
+    th = wl.B * wl.H * wl.T
+    if wl.group == 1:
+        C = chunk or 64
+        return th * (6 * d * d + 10 * C * d)
+    return th * 6 * d * d + wl.B * wl.H * (wl.T // wl.group) * 2 * d ** 3
+
+
+def bytes_per_call(wl):
+    """Algorithmic HBM bytes: q,k,v read once, out written once (2 B each), alpha/beta fp32, state in+out."""
+    th = wl.B * wl.H * wl.T
+    es = 4 if str(wl.dtype).endswith("float32") else 2
+    per_tok = (2 * wl.d_k + 2 * wl.d_v) * es + 4 + (4 if wl.group == 1 else 0)
+    return th * per_tok + 2 * wl.B * wl.H * wl.d_k * wl.d_v * 4 + (0 if wl.group == 1 else wl.B * wl.H * (wl.T // wl.group) * 4)
+
+
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU during the timed region (pynvml)."""
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        s = self.samples
+        return {"sm_mhz": statistics.median(s) if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, timed on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    from paper_2605_30409_b200 import inputs as gin
+    wl = workload(args)
+    inp = gin.make_inputs(wl)
+    cores = oracle.max_threads()
+    st = inp.state
+    for _ in range(args.warmup):
+        _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, st, group=wl.group)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, st, group=wl.group)
+    dt = time.perf_counter() - t0
+    tokens = wl.B * wl.T * args.steps
+    val = tokens / dt
+    sample = f"full {wl.name} workload ({wl.B}x{wl.T} tokens, {wl.H} heads, d={wl.d_k}) per step, {args.steps} steps"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(wl, None),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(wl, info, extra=None):
+    d = {"workload": f"BASELINE.json configs[{int(wl.name[3]) - 1}] ({wl.name}): B={wl.B} H={wl.H} T={wl.T} "
+                     f"d_k=d_v={wl.d_k} {str(wl.dtype).split('.')[-1]}, "
+                     + ("token-wise (G=1)" if wl.group == 1 else f"frame-wise (G={wl.group})"),
+         "B": wl.B, "H": wl.H, "T": wl.T, "d_k": wl.d_k, "d_v": wl.d_v, "group": wl.group,
+         "parallelism": "replicas only (no collective)"}
+    if info is not None:
+        d.update({"path": info[0], "chunk": info[1], "launches_per_call": info[2]})
+    if extra:
+        d.update(extra)
+    return d
+
+
+def cpu_baseline(wl, budget_s=12.0):
+    """The oracle, as it stands, on a bounded sample of the same workload (rank 0, N=1)."""
+    import oracle
+    from paper_2605_30409_b200 import inputs as gin
+    inp = gin.make_inputs(wl)
+    cores = oracle.max_threads()
+    t0 = time.perf_counter()
+    _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=wl.group)
+    one = time.perf_counter() - t0
+    reps = max(1, min(50, int(budget_s / max(one, 1e-3))))
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, st, group=wl.group)
+    dt = time.perf_counter() - t0
+    return {"value": wl.B * wl.T * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"full {wl.name} workload x {reps} carried-state repeats ({dt:.1f} s of CPU work)"}
+
+
+def run_ours(args):
+    import torch
+    import paper_2605_30409_b200 as gdn
+    from paper_2605_30409_b200 import inputs as gin
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = workload(args)
+    es = 2 if wl.dtype == torch.bfloat16 else 4
+    set_bytes = wl.B * wl.T * wl.H * (2 * wl.d_k + 2 * wl.d_v) * es
+    n_sets = max(2, int(L2_BYTES * 1.5 // set_bytes) + 1)         # rotate so the inputs of a step are cold in L2
+    n_sets = min(n_sets, 16)
+    sets = []
+    for i in range(n_sets):
+        inp = gin.make_inputs(wl, seed=wl.seed + 17 * i + 1000 * rank)
+        sets.append(dict(q=inp.q.to(dev), k=inp.k.to(dev), v=inp.v.to(dev), alpha=inp.alpha.to(dev),
+                         beta=inp.beta.to(dev), out=torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=wl.dtype, device=dev)))
+    state = gin.make_inputs(wl).state.to(dev)
+    plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, chunk=wl.chunk,
+                       io_dtype=gdn.GDN_BF16 if wl.dtype == torch.bfloat16 else gdn.GDN_FP32)
+    info = plan.info
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        s = sets[i % n_sets]
+        plan.forward(s["q"], s["k"], s["v"], s["alpha"], s["beta"], state, s["out"], state, stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(args.steps):
+        step(i)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    clocks = sampler.stop()
+    assert torch.isfinite(state).all(), "state diverged"
+    ms_per_step = ms / args.steps
+    tokens_per_s = world * wl.B * wl.T * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel durations (separate pass with CUDA events between the launches) ----------------
+    kernels = plan_kernel_times(plan, step, args.steps, barrier)
+
+    # ---- end to end through the host entry point (pinned host buffers, copies inside the timing) ----
+    e2e = None
+    if not args.no_e2e:
+        inp = gin.make_inputs(wl)
+        pin = lambda t: t.contiguous().pin_memory()
+        hq, hk, hv, ha, hb, hs = map(pin, (inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state))
+        hout = torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=wl.dtype).pin_memory()
+        k_e2e = max(3, min(args.steps, 50))
+        for _ in range(3):
+            plan.forward_host(hq, hk, hv, ha, hb, hs, hout, hs, stream)
+        barrier()
+        e0.record(stream)
+        for _ in range(k_e2e):
+            plan.forward_host(hq, hk, hv, ha, hb, hs, hout, hs, stream)
+        e1.record(stream)
+        barrier()
+        ms_e = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms_e], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        nbytes = lambda *ts: int(sum(t.numel() * t.element_size() for t in ts))
+        e2e = {"value": world * wl.B * wl.T * k_e2e / (ms_e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": nbytes(hq, hk, hv, ha, hb, hs), "d2h_bytes_per_step": nbytes(hout, hs),
+               "steps": k_e2e, "ms_per_step": ms_e / k_e2e}
+
+    pk, pk_src = peaks()
+    fl = flops_per_call(wl, info.chunk)
+    by = bytes_per_call(wl)
+    tflops = fl / (ms_per_step * 1e-3) / 1e12
+    roof = roofline(wl, info, kernels, ms_per_step, pk, pk_src, by)
+    line = {
+        "metric": METRIC, "value": tokens_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16" if wl.dtype == torch.bfloat16 else "f32", "data": "synthetic",
+        "config": config_dict(wl, (gdn.PATH_NAMES[info.path], info.chunk, info.launches_per_call),
+                              {"l2": f"rotating {n_sets} input sets ({n_sets * set_bytes / 1e6:.0f} MB > 126 MB L2), carried state"}),
+        "tflops": tflops, "pct_bf16_peak": 100 * tflops / pk["bf16_tflops"], "peaks": pk_src,
+        "hbm_gbs_algorithmic": by / (ms_per_step * 1e-3) / 1e9,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * info.launches_per_call,
+        "roofline": roof, "kernels": kernels,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu:
+        line["cpu_baseline"] = cpu_baseline(wl)
+    plan.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def plan_kernel_times(plan, step, steps, barrier):
+    """Average duration of every kernel of a call, from CUDA events the library records between its own
+    launches on the launching stream (gdn_plan_set_profiling; a separate pass, not the timed region)."""
+    import paper_2605_30409_b200 as gdn
+    if not hasattr(gdn, "gdn_plan_kernel_times"):
+        return None
+    n = min(steps, 200)
+    gdn.gdn_plan_set_profiling(plan.handle, 1)
+    for i in range(n):
+        step(i)
+    barrier()
+    names, ms = gdn.gdn_plan_kernel_times(plan.handle)
+    gdn.gdn_plan_set_profiling(plan.handle, 0)
+    return [{"name": nm, "avg_us": 1e3 * m} for nm, m in zip(names, ms)]
+
+
+def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
+    """Roofline of the dominant kernel. HBM-bound: achieved = algorithmic bytes / duration."""
+    dur_ms, name = ms_per_step, "whole step"
+    if kernels:
+        top = max(kernels, key=lambda k: k["avg_us"])
+        dur_ms, name = top["avg_us"] * 1e-3, top["name"]
+    achieved = by / (dur_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
+            "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_source": pk_src,
+            "algorithmic_bytes": by}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 5])
+    ap.add_argument("--mode", default="token", choices=["token", "frame"])
+    ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 5 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        run_reference(args)
+    else:
+        args.steps = 300 if args.steps is None else args.steps
+        args.warmup = max(3, 20 if args.warmup is None else args.warmup)
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,175 @@
+/*
+ * gdn.h -- C ABI of the B200-native Gated DeltaNet (GDN) chunk forward.
+ *
+ * One operator, the token-mixing forward of SANA-Streaming's GDN blocks (arxiv/paper_2605_30409,
+ * cited below as PAPER.md:L<line>), with the fp32 recurrent state carried from streaming chunk to
+ * streaming chunk.  Per (batch b, head h), with the T tokens of the call split into T/G consecutive
+ * groups of G tokens (G = tokens per latent frame in the paper; G = 1 is the token-wise gated delta
+ * rule S_t = a_t S_{t-1}(I - b_t k_t k_t^T) + b_t v_t k_t^T, o_t = S_t q_t):
+ *
+ *     S~    = alpha_g * S_{g-1}                                  PAPER.md Eq. 17  (L591)
+ *     u_n   = beta_n * (v_n - k_n S~)      for every n in g      PAPER.md Eq. 18  (L595)
+ *     S_g   = S~ + sum_n k_n^T u_n                               PAPER.md Eq. 18/19 (L595-L599)
+ *     o_n   = scale * q_n S_g              for every n in g      PAPER.md Eq. 22  (L622), numerator
+ *
+ * and, with GDN_FLAG_NORMALIZER, the normaliser state z (Eq. 20-21, un-rotated keys) and
+ * the normalised readout o_n / (q_raw_n . z_g + eps) (Eq. 22).  Row-token orientation of Alg. 1 /
+ * Eq. 5 (L118, L369): q,k in R^{T x d_k}; v,o in R^{T x d_v}; S in R^{d_k x d_v}; z in R^{d_k}.
+ * The state cache of App. G.6 (L630-L636) is `state_out` of call i fed as `state_in` of call i+1.
+ *
+ * Conventions for every entry point
+ *   - All tensor pointers are DEVICE pointers unless the name says host; the caller owns them.
+ *   - Layouts: q,k [B,T,H,d_k]; v,out [B,T,H,d_v] (element type io_dtype, feature dim contiguous,
+ *     token stride configurable so a packed qkv [B,T,3,H,d] tensor works);
+ *     alpha [B,H,T/G] fp32; beta [B,H,T] fp32; state [B,H,d_k,d_v] fp32 row-major; z [B,H,d_k] fp32.
+ *   - Calls enqueue work on `stream` and return without synchronising; errors are return codes and
+ *     nothing throws across the ABI.  A plan is bound to the device current at gdn_plan() time and
+ *     must not be used from two host threads at once.  Two calls on the same plan must be issued to
+ *     the same stream or be externally ordered (they share the plan's workspace).
+ *   - There is no CPU fallback: on a device that is not sm_100 every compute call returns GDN_ERR_ARCH.
+ */
+#ifndef GDN_B200_H_
+#define GDN_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gdn_plan gdn_plan_t;          /* opaque; owned by the library, freed by gdn_destroy */
+typedef void* gdn_stream_t;                  /* a cudaStream_t (0 = the legacy default stream)     */
+
+typedef enum {
+    GDN_OK = 0,
+    GDN_ERR_INVALID_ARG = 1,   /* NULL where a pointer is required, non-positive sizes, T % G != 0, ...  */
+    GDN_ERR_UNSUPPORTED = 2,   /* well-formed but not implemented (head dim, flag, dtype combination)   */
+    GDN_ERR_ALIGNMENT = 3,     /* pointer not 16-byte aligned / token stride not a multiple of 8 elems  */
+    GDN_ERR_NOMEM = 4,         /* workspace allocation failed                                           */
+    GDN_ERR_ARCH = 5,          /* device is not sm_100 (B200); there is no fallback path                */
+    GDN_ERR_CUDA = 6           /* a CUDA runtime/driver call failed; see gdn_last_error()               */
+} gdn_status_t;
+
+typedef enum { GDN_BF16 = 0, GDN_FP32 = 1 } gdn_dtype_t;     /* element type of q, k, v, out */
+
+enum {
+    GDN_FLAG_NORMALIZER = 1u,  /* also run the z path and divide (gdn_forward_chunk_norm only)          */
+    GDN_FLAG_BIDIR      = 2u,  /* in-chunk reverse scan (Alg. 1 l.14-22); NOT implemented -> UNSUPPORTED */
+    GDN_FLAG_LOG_ALPHA  = 4u,  /* `alpha` holds log(alpha) (<= 0) instead of alpha in (0,1]             */
+    GDN_FLAG_FORCE_SIMT = 8u   /* use the fp32 CUDA-core kernel even where a tensor-core path exists    */
+};
+
+typedef struct {
+    uint32_t struct_size;      /* = sizeof(gdn_config_t); ABI versioning                                 */
+    int32_t  B, H, T;          /* T = tokens per call (one streaming chunk); B,H,T >= 0                  */
+    int32_t  d_k, d_v;         /* head dims, each in {32, 64, 128}                                       */
+    int32_t  group;            /* G: 1 = token-wise; tokens-per-frame = frame-wise (paper). T % G == 0   */
+    int32_t  chunk;            /* token-wise compute tile C in {64, 128}; 0 = auto. Ignored when G > 1.
+                                  Results do not depend on C beyond rounding.                           */
+    int32_t  io_dtype;         /* gdn_dtype_t                                                            */
+    float    scale;            /* multiplies the numerator q S; the paper has no query scale: use 1.0f   */
+    float    eps;              /* 1e-6f; only used with GDN_FLAG_NORMALIZER              */
+    uint32_t flags;
+    int64_t  q_token_stride, k_token_stride, v_token_stride, o_token_stride;
+                               /* elements between consecutive tokens; 0 => H*d (dense). The batch
+                                  stride is T*token_stride, the head stride is d.                        */
+} gdn_config_t;
+
+/* Which kernels a plan resolved to (for logs, tests and the bench JSON). */
+typedef enum { GDN_PATH_SIMT_FP32 = 0, GDN_PATH_TC_TOKEN = 1, GDN_PATH_TC_FRAME = 2 } gdn_path_t;
+
+typedef struct {
+    int32_t  path;             /* gdn_path_t                                                             */
+    int32_t  chunk;            /* resolved compute tile C (token-wise tensor-core path), else 0          */
+    int32_t  launches_per_call;/* number of kernel launches one gdn_forward_chunk enqueues               */
+    int32_t  sm_count;         /* SMs of the plan's device (0 if no device was visible at plan time)     */
+    uint64_t workspace_bytes;  /* device workspace owned by the plan                                     */
+} gdn_plan_info_t;
+
+/*
+ * gdn_plan: validate `cfg`, choose the kernels, allocate the plan's device workspace.
+ *   Returns GDN_OK and a plan in *plan_out, or an error and *plan_out = NULL.
+ *   Shapes, dtype, G and flags are fixed per plan (the paper's first chunk has 5 frames, later chunks
+ *   3 -- PAPER.md L460 -- so a stream holds one plan per distinct T).  With B, H or T equal to 0 the
+ *   plan is valid and every forward call is a no-op (state_out = state_in).
+ *   Plans can be created without a visible GPU (validation only); compute calls then return ARCH/CUDA.
+ */
+gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out);
+
+/*
+ * gdn_forward_chunk: out, state_out = GDN(q, k, v, alpha, beta, state_in)  -- equations at the top.
+ *   q,k        [B,T,H,d_k] io_dtype, device            alpha  [B,H,T/G] fp32, device (alpha or log alpha)
+ *   v          [B,T,H,d_v] io_dtype, device            beta   [B,H,T]   fp32, device
+ *   state_in   [B,H,d_k,d_v] fp32, device, or NULL (= zeros: "cached state or zero", Alg. 1 l.9 L338)
+ *   out        [B,T,H,d_v] io_dtype, device; must not alias any input
+ *   state_out  [B,H,d_k,d_v] fp32, device; may be the same buffer as state_in (streaming use)
+ *   Pointers must be 16-byte aligned and token strides multiples of 8 elements, else ALIGNMENT.
+ *   Domain: the update is a contraction when beta_n |k_n|^2 <= 1 (G=1) resp. ||K^T B K||_2 <= 1 (G>1);
+ *   the library does not check it (reading 21).
+ */
+gdn_status_t gdn_forward_chunk(gdn_plan_t* plan,
+                               const void* q, const void* k, const void* v,
+                               const float* alpha, const float* beta,
+                               const float* state_in,
+                               void* out, float* state_out,
+                               gdn_stream_t stream);
+
+/*
+ * gdn_forward_chunk_norm: the paper's full readout (plan must carry GDN_FLAG_NORMALIZER):
+ *   matrix path with the rotated q_rot,k_rot (Eq. 18-19), vector path z with the un-rotated k_raw
+ *   (Eq. 20-21), out_n = scale * q_rot_n S_g / (q_raw_n . z_g + eps) (Eq. 22).
+ *   z_in [B,H,d_k] fp32 or NULL; z_out [B,H,d_k] fp32 (may alias z_in).  Other arguments as above.
+ */
+gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan,
+                                    const void* q_rot, const void* k_rot, const void* v,
+                                    const void* q_raw, const void* k_raw,
+                                    const float* alpha, const float* beta,
+                                    const float* S_in, const float* z_in,
+                                    void* out, float* S_out, float* z_out,
+                                    gdn_stream_t stream);
+
+/*
+ * gdn_forward_chunk_host: the same operator with HOST buffers (dense layouts, strides in the plan are
+ *   ignored; pinned memory recommended).  Copies the inputs to plan-owned device staging buffers on
+ *   `stream`, runs gdn_forward_chunk, copies out and state_out back, and returns without synchronising:
+ *   the caller synchronises `stream` before reading the results.  state_in_host may be NULL.
+ */
+gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan,
+                                    const void* q_host, const void* k_host, const void* v_host,
+                                    const float* alpha_host, const float* beta_host,
+                                    const float* state_in_host,
+                                    void* out_host, float* state_out_host,
+                                    gdn_stream_t stream);
+
+/* gdn_destroy: free the plan and its workspace. NULL is allowed. Does not synchronise the stream:
+ * the caller makes sure no call using the plan is still in flight. */
+gdn_status_t gdn_destroy(gdn_plan_t* plan);
+
+/* gdn_plan_get_info: fill *info. */
+gdn_status_t gdn_plan_get_info(const gdn_plan_t* plan, gdn_plan_info_t* info);
+
+/*
+ * gdn_plan_set_profiling / gdn_plan_kernel_times: per-kernel device timing for bench.py's roofline.
+ *   With profiling enabled every forward call records CUDA events on the launching stream before its
+ *   first kernel and after each kernel.  gdn_plan_kernel_times synchronises those events, writes up to
+ *   max_n kernel names (static strings) and the AVERAGE duration in milliseconds of each kernel over the
+ *   calls made since profiling was enabled, sets *n_out, and clears the accumulated events.
+ *   Not meant for the timed region itself (events between launches add a little latency).
+ */
+gdn_status_t gdn_plan_set_profiling(gdn_plan_t* plan, int enable);
+gdn_status_t gdn_plan_kernel_times(gdn_plan_t* plan, int max_n, const char** names, float* avg_ms, int* n_out);
+
+/* gdn_status_string: static name of a status code. */
+const char* gdn_status_string(gdn_status_t status);
+
+/* gdn_last_error: detail text of the last failure on this plan (e.g. the CUDA error string);
+ * with plan == NULL, of the last failing gdn_plan() call on this thread. Never NULL. */
+const char* gdn_last_error(const gdn_plan_t* plan);
+
+/* gdn_version: library version, e.g. "0.1.0". */
+const char* gdn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GDN_B200_H_ */

@@ -1,0 +1,338 @@
+// gdn_api.cu -- the C ABI of include/gdn.h: plan / forward / destroy.
+// Host logic only (validation, path choice, workspace, launches); every arithmetic step of the path
+// runs in the kernels of gdn_simt.cuh (fp32 CUDA cores) and gdn_tc_*.cuh (tcgen05 tensor cores).
+#include "../../include/gdn.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "gdn_profile.cuh"
+#include "gdn_simt.cuh"
+#include "gdn_tc.cuh"
+
+namespace {
+
+thread_local std::string g_plan_error;
+
+struct Staging {                 // device buffers for gdn_forward_chunk_host
+    void *q = nullptr, *k = nullptr, *v = nullptr, *out = nullptr;
+    float *alpha = nullptr, *beta = nullptr, *state = nullptr;
+    bool ready = false;
+};
+
+}  // namespace
+
+struct gdn_plan {
+    gdn_config_t cfg;
+    int device = -1;
+    int sm_count = 0;
+    int cc_major = 0, cc_minor = 0;
+    gdn_path_t path = GDN_PATH_SIMT_FP32;
+    int chunk = 0;
+    int launches = 1;
+    void* workspace = nullptr;
+    size_t workspace_bytes = 0;
+    float* z_stage = nullptr;     // copy of z_in when z_out aliases it
+    Staging host;
+    gdn::TcPlan tc;               // tensor-core path state (tensor maps, workspace carving)
+    gdn::Profiler prof;           // optional per-kernel CUDA events (bench roofline)
+    std::string err;
+};
+
+namespace {
+
+size_t esize(int dt) { return dt == GDN_FP32 ? 4 : 2; }
+
+bool head_dim_ok(int d) { return d == 32 || d == 64 || d == 128; }
+
+gdn_status_t fail(gdn_plan_t* p, gdn_status_t st, const std::string& msg) {
+    if (p) p->err = msg; else g_plan_error = msg;
+    return st;
+}
+
+gdn_status_t cuda_fail(gdn_plan_t* p, cudaError_t e, const char* what) {
+    return fail(p, GDN_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+long long tok_stride(long long s, int H, int d) { return s ? s : (long long)H * d; }
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <typename TIn>
+void launch_simt(const gdn::SimtParams& sp, int dk, cudaStream_t st) {
+    const int tiles = sp.dv / gdn::kSimtCols;
+    const long long warps = (long long)sp.B * sp.H * tiles;
+    const int blocks = (int)((warps + gdn::kSimtWarps - 1) / gdn::kSimtWarps);
+    const dim3 block(gdn::kSimtWarps * 32);
+    switch (dk) {
+        case 32:  gdn::gdn_simt_kernel<32, TIn><<<blocks, block, 0, st>>>(sp); break;
+        case 64:  gdn::gdn_simt_kernel<64, TIn><<<blocks, block, 0, st>>>(sp); break;
+        default:  gdn::gdn_simt_kernel<128, TIn><<<blocks, block, 0, st>>>(sp); break;
+    }
+}
+
+gdn_status_t check_device(gdn_plan_t* p) {
+    if (p->device < 0) return fail(p, GDN_ERR_CUDA, "no CUDA device was visible when the plan was created");
+    if (!(p->cc_major == 10 && p->cc_minor == 0))
+        return fail(p, GDN_ERR_ARCH, "device is sm_" + std::to_string(p->cc_major * 10 + p->cc_minor) +
+                                         ", this library only carries sm_100a code (no fallback)");
+    return GDN_OK;
+}
+
+gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const void* v,
+                          const void* q_raw, const void* k_raw,
+                          const float* alpha, const float* beta, const float* S_in, const float* z_in,
+                          void* out, float* S_out, float* z_out, cudaStream_t st, bool normalizer) {
+    const gdn_config_t& c = p->cfg;
+    const size_t state_elems = (size_t)c.B * c.H * c.d_k * c.d_v;
+    if (c.B == 0 || c.H == 0) return GDN_OK;
+    if (!S_out) return fail(p, GDN_ERR_INVALID_ARG, "state_out is NULL");
+    if (c.T == 0) {                                   // empty chunk: the state passes through
+        gdn_status_t ds = check_device(p);
+        if (ds != GDN_OK) return ds;
+        cudaError_t e = cudaSuccess;
+        if (S_in == nullptr) e = cudaMemsetAsync(S_out, 0, state_elems * 4, st);
+        else if (S_in != S_out) e = cudaMemcpyAsync(S_out, S_in, state_elems * 4, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess && normalizer && z_out) {
+            if (z_in == nullptr) e = cudaMemsetAsync(z_out, 0, (size_t)c.B * c.H * c.d_k * 4, st);
+            else if (z_in != z_out) e = cudaMemcpyAsync(z_out, z_in, (size_t)c.B * c.H * c.d_k * 4, cudaMemcpyDeviceToDevice, st);
+        }
+        return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "state pass-through");
+    }
+    if (!q || !k || !v || !alpha || !beta || !out)
+        return fail(p, GDN_ERR_INVALID_ARG, "a required tensor pointer is NULL");
+    if (normalizer && (!q_raw || !k_raw || !z_out))
+        return fail(p, GDN_ERR_INVALID_ARG, "normaliser call needs q_raw, k_raw and z_out");
+    const void* ptrs[] = {q, k, v, alpha, beta, S_in, out, S_out, q_raw, k_raw, z_in, z_out};
+    for (const void* ptr : ptrs)
+        if (ptr && !aligned16(ptr)) return fail(p, GDN_ERR_ALIGNMENT, "tensor pointers must be 16-byte aligned");
+    if (out == q || out == k || out == v) return fail(p, GDN_ERR_INVALID_ARG, "out must not alias an input");
+    gdn_status_t ds = check_device(p);
+    if (ds != GDN_OK) return ds;
+
+    if (p->path != GDN_PATH_SIMT_FP32 && !normalizer) {
+        std::string msg;
+        gdn_status_t ts = gdn::tc_forward(p->tc, c, q, k, v, alpha, beta, S_in, out, S_out, st, &p->prof, &msg);
+        if (ts != GDN_OK) return fail(p, ts, msg);
+        return GDN_OK;
+    }
+
+    if (normalizer && z_in && z_in == z_out) {        // every column tile reads z_in: stage a copy
+        cudaError_t e = cudaMemcpyAsync(p->z_stage, z_in, (size_t)c.B * c.H * c.d_k * 4, cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "z staging copy");
+        z_in = p->z_stage;
+    }
+    gdn::SimtParams sp{};
+    sp.q = q; sp.k = k; sp.v = v; sp.q_raw = q_raw; sp.k_raw = k_raw;
+    sp.alpha = alpha; sp.beta = beta; sp.S_in = S_in; sp.z_in = z_in;
+    sp.out = out; sp.S_out = S_out; sp.z_out = z_out;
+    sp.B = c.B; sp.H = c.H; sp.T = c.T; sp.G = c.group; sp.dv = c.d_v;
+    sp.q_ts = tok_stride(c.q_token_stride, c.H, c.d_k);
+    sp.k_ts = tok_stride(c.k_token_stride, c.H, c.d_k);
+    sp.v_ts = tok_stride(c.v_token_stride, c.H, c.d_v);
+    sp.o_ts = tok_stride(c.o_token_stride, c.H, c.d_v);
+    sp.scale = c.scale; sp.eps = c.eps;
+    sp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
+    sp.normalizer = normalizer ? 1 : 0;
+    p->prof.begin(st);
+    if (c.io_dtype == GDN_FP32) launch_simt<float>(sp, c.d_k, st);
+    else launch_simt<__nv_bfloat16>(sp, c.d_k, st);
+    p->prof.mark(st, "gdn_simt_kernel");
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e, "gdn_simt_kernel launch");
+    return GDN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
+    if (plan_out) *plan_out = nullptr;
+    if (!cfg || !plan_out) return fail(nullptr, GDN_ERR_INVALID_ARG, "cfg or plan_out is NULL");
+    if (cfg->struct_size != sizeof(gdn_config_t))
+        return fail(nullptr, GDN_ERR_INVALID_ARG, "struct_size does not match this library's gdn_config_t");
+    const gdn_config_t& c = *cfg;
+    if (c.B < 0 || c.H < 0 || c.T < 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "B, H, T must be >= 0");
+    if (c.d_k <= 0 || c.d_v <= 0 || c.group <= 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "d_k, d_v, group must be > 0");
+    if (c.T % c.group != 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "T must be a multiple of group");
+    if (c.io_dtype != GDN_BF16 && c.io_dtype != GDN_FP32) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown io_dtype");
+    if (!(c.chunk == 0 || c.chunk == 64 || c.chunk == 128)) return fail(nullptr, GDN_ERR_INVALID_ARG, "chunk must be 0, 64 or 128");
+    const uint32_t known = GDN_FLAG_NORMALIZER | GDN_FLAG_BIDIR | GDN_FLAG_LOG_ALPHA | GDN_FLAG_FORCE_SIMT;
+    if (c.flags & ~known) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown flag bits");
+    if (!head_dim_ok(c.d_k) || !head_dim_ok(c.d_v))
+        return fail(nullptr, GDN_ERR_UNSUPPORTED, "d_k and d_v must each be 32, 64 or 128 (112 via padding is not implemented)");
+    if (c.flags & GDN_FLAG_BIDIR) return fail(nullptr, GDN_ERR_UNSUPPORTED, "GDN_FLAG_BIDIR (in-chunk reverse scan) is not implemented");
+    const long long strides[4] = {c.q_token_stride, c.k_token_stride, c.v_token_stride, c.o_token_stride};
+    const int dims[4] = {c.d_k, c.d_k, c.d_v, c.d_v};
+    for (int i = 0; i < 4; ++i) {
+        if (strides[i] < 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "token strides must be >= 0");
+        if (strides[i] != 0 && strides[i] < (long long)c.H * dims[i])
+            return fail(nullptr, GDN_ERR_INVALID_ARG, "token stride smaller than H*d");
+        if (strides[i] % 8 != 0) return fail(nullptr, GDN_ERR_ALIGNMENT, "token strides must be multiples of 8 elements");
+    }
+
+    gdn_plan_t* p = new (std::nothrow) gdn_plan_t();
+    if (!p) return fail(nullptr, GDN_ERR_NOMEM, "host allocation failed");
+    p->cfg = c;
+    int dev = -1;
+    if (cudaGetDevice(&dev) == cudaSuccess) {
+        p->device = dev;
+        cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&p->cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+        cudaDeviceGetAttribute(&p->cc_minor, cudaDevAttrComputeCapabilityMinor, dev);
+    } else {
+        cudaGetLastError();          // clear "no device": validation-only plan
+    }
+
+    // ---- path choice -----------------------------------------------------------------------------
+    p->path = GDN_PATH_SIMT_FP32;
+    p->chunk = 0;
+    p->launches = 1;
+    const bool want_tc = c.io_dtype == GDN_BF16 && !(c.flags & (GDN_FLAG_FORCE_SIMT | GDN_FLAG_NORMALIZER)) &&
+                         c.B > 0 && c.H > 0 && c.T > 0;
+    if (want_tc) {
+        std::string msg;
+        gdn_path_t path;
+        int chunk = 0, launches = 1;
+        if (gdn::tc_supported(c, &path, &chunk, &launches)) {
+            if (p->device >= 0 && p->cc_major == 10 && p->cc_minor == 0) {
+                gdn_status_t ts = gdn::tc_plan_init(p->tc, c, p->sm_count, &msg);
+                if (ts != GDN_OK) { delete p; return fail(nullptr, ts, msg); }
+            }
+            p->path = path; p->chunk = chunk; p->launches = launches;
+            p->workspace_bytes = p->tc.workspace_bytes;
+        }
+    }
+    if ((c.flags & GDN_FLAG_NORMALIZER) && p->device >= 0 && c.B * c.H > 0) {
+        cudaError_t e = cudaMalloc(&p->z_stage, (size_t)c.B * c.H * c.d_k * 4);
+        if (e != cudaSuccess) { cudaGetLastError(); gdn::tc_plan_free(p->tc); delete p; return fail(nullptr, GDN_ERR_NOMEM, "z staging allocation failed"); }
+        p->workspace_bytes += (size_t)c.B * c.H * c.d_k * 4;
+    }
+    *plan_out = p;
+    return GDN_OK;
+}
+
+gdn_status_t gdn_forward_chunk(gdn_plan_t* plan, const void* q, const void* k, const void* v,
+                               const float* alpha, const float* beta, const float* state_in,
+                               void* out, float* state_out, gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    if (plan->cfg.flags & GDN_FLAG_NORMALIZER)
+        return fail(plan, GDN_ERR_INVALID_ARG, "plan carries GDN_FLAG_NORMALIZER: call gdn_forward_chunk_norm");
+    return forward_impl(plan, q, k, v, nullptr, nullptr, alpha, beta, state_in, nullptr, out, state_out, nullptr,
+                        static_cast<cudaStream_t>(stream), false);
+}
+
+gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan, const void* q_rot, const void* k_rot, const void* v,
+                                    const void* q_raw, const void* k_raw, const float* alpha, const float* beta,
+                                    const float* S_in, const float* z_in, void* out, float* S_out, float* z_out,
+                                    gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    if (!(plan->cfg.flags & GDN_FLAG_NORMALIZER))
+        return fail(plan, GDN_ERR_INVALID_ARG, "plan was not created with GDN_FLAG_NORMALIZER");
+    return forward_impl(plan, q_rot, k_rot, v, q_raw, k_raw, alpha, beta, S_in, z_in, out, S_out, z_out,
+                        static_cast<cudaStream_t>(stream), true);
+}
+
+gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const void* k_host, const void* v_host,
+                                    const float* alpha_host, const float* beta_host, const float* state_in_host,
+                                    void* out_host, float* state_out_host, gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    gdn_plan_t* p = plan;
+    const gdn_config_t& c = p->cfg;
+    if (c.flags & GDN_FLAG_NORMALIZER) return fail(p, GDN_ERR_UNSUPPORTED, "host entry point has no normaliser variant");
+    if (c.q_token_stride || c.k_token_stride || c.v_token_stride || c.o_token_stride)
+        return fail(p, GDN_ERR_UNSUPPORTED, "host entry point needs dense layouts (token strides 0)");
+    if (c.B == 0 || c.H == 0) return GDN_OK;
+    if (!state_out_host) return fail(p, GDN_ERR_INVALID_ARG, "state_out_host is NULL");
+    if (c.T > 0 && (!q_host || !k_host || !v_host || !alpha_host || !beta_host || !out_host))
+        return fail(p, GDN_ERR_INVALID_ARG, "a required host pointer is NULL");
+    gdn_status_t ds = check_device(p);
+    if (ds != GDN_OK) return ds;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t es = esize(c.io_dtype);
+    const size_t nq = (size_t)c.B * c.T * c.H * c.d_k * es, nv = (size_t)c.B * c.T * c.H * c.d_v * es;
+    const size_t na = (size_t)c.B * c.H * (c.T / c.group) * 4, nb = (size_t)c.B * c.H * c.T * 4;
+    const size_t ns = (size_t)c.B * c.H * c.d_k * c.d_v * 4;
+    Staging& h = p->host;
+    if (!h.ready) {
+        cudaError_t e = cudaSuccess;
+        auto alloc = [&](void** ptr, size_t n) { if (e == cudaSuccess) e = cudaMalloc(ptr, n ? n : 16); };
+        alloc(&h.q, nq); alloc(&h.k, nq); alloc(&h.v, nv); alloc(&h.out, nv);
+        alloc((void**)&h.alpha, na); alloc((void**)&h.beta, nb); alloc((void**)&h.state, ns);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(p, GDN_ERR_NOMEM, "host-path staging allocation failed"); }
+        h.ready = true;
+        p->workspace_bytes += 2 * nq + 2 * nv + na + nb + ns;
+    }
+    cudaError_t e = cudaSuccess;
+    auto h2d = [&](void* d, const void* s, size_t n) { if (e == cudaSuccess && n) e = cudaMemcpyAsync(d, s, n, cudaMemcpyHostToDevice, st); };
+    h2d(h.q, q_host, nq); h2d(h.k, k_host, nq); h2d(h.v, v_host, nv);
+    h2d(h.alpha, alpha_host, na); h2d(h.beta, beta_host, nb);
+    if (state_in_host) h2d(h.state, state_in_host, ns);
+    if (e != cudaSuccess) return cuda_fail(p, e, "host->device copy");
+    gdn_status_t fs = forward_impl(p, h.q, h.k, h.v, nullptr, nullptr, h.alpha, h.beta,
+                                   state_in_host ? h.state : nullptr, nullptr, h.out, h.state, nullptr, st, false);
+    if (fs != GDN_OK) return fs;
+    if (nv) e = cudaMemcpyAsync(out_host, h.out, nv, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(state_out_host, h.state, ns, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(p, e, "device->host copy");
+    return GDN_OK;
+}
+
+gdn_status_t gdn_destroy(gdn_plan_t* plan) {
+    if (!plan) return GDN_OK;
+    gdn::tc_plan_free(plan->tc);
+    plan->prof.set_enabled(false);
+    if (plan->z_stage) cudaFree(plan->z_stage);
+    Staging& h = plan->host;
+    void* bufs[] = {h.q, h.k, h.v, h.out, h.alpha, h.beta, h.state};
+    for (void* b : bufs) if (b) cudaFree(b);
+    delete plan;
+    return GDN_OK;
+}
+
+gdn_status_t gdn_plan_get_info(const gdn_plan_t* plan, gdn_plan_info_t* info) {
+    if (!plan || !info) return GDN_ERR_INVALID_ARG;
+    info->path = plan->path;
+    info->chunk = plan->chunk;
+    info->launches_per_call = plan->launches;
+    info->sm_count = plan->sm_count;
+    info->workspace_bytes = plan->workspace_bytes;
+    return GDN_OK;
+}
+
+gdn_status_t gdn_plan_set_profiling(gdn_plan_t* plan, int enable) {
+    if (!plan) return GDN_ERR_INVALID_ARG;
+    plan->prof.set_enabled(enable != 0);
+    return GDN_OK;
+}
+
+gdn_status_t gdn_plan_kernel_times(gdn_plan_t* plan, int max_n, const char** names, float* avg_ms, int* n_out) {
+    if (!plan || !names || !avg_ms || !n_out || max_n < 0) return GDN_ERR_INVALID_ARG;
+    *n_out = plan->prof.collect(max_n, names, avg_ms);
+    return GDN_OK;
+}
+
+const char* gdn_status_string(gdn_status_t s) {
+    switch (s) {
+        case GDN_OK: return "GDN_OK";
+        case GDN_ERR_INVALID_ARG: return "GDN_ERR_INVALID_ARG";
+        case GDN_ERR_UNSUPPORTED: return "GDN_ERR_UNSUPPORTED";
+        case GDN_ERR_ALIGNMENT: return "GDN_ERR_ALIGNMENT";
+        case GDN_ERR_NOMEM: return "GDN_ERR_NOMEM";
+        case GDN_ERR_ARCH: return "GDN_ERR_ARCH";
+        case GDN_ERR_CUDA: return "GDN_ERR_CUDA";
+    }
+    return "GDN_ERR_UNKNOWN";
+}
+
+const char* gdn_last_error(const gdn_plan_t* plan) { return plan ? plan->err.c_str() : g_plan_error.c_str(); }
+
+const char* gdn_version(void) { return "0.1.0"; }
+
+}  // extern "C"
