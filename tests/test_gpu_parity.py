@@ -178,3 +178,109 @@ def test_split_invariance_device(G):
     o1, s1, _ = part(0, T1, inp.state)
     o2, s2, _ = part(T1, 256, s1)
     assert torch.equal(torch.cat([o1, o2], dim=1), o_full) and torch.equal(s2, s_full)
+
+
+# =====================================================================================================
+# Tensor-core (tcgen05) token-wise path: BASELINE.json's configs, literal (G = 1)
+# =====================================================================================================
+def _assert_tc(info):
+    assert info[0] == 1, f"expected the tensor-core token path, plan resolved to {info}"
+
+
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("C", [64, 128])
+@pytest.mark.parametrize("T", [1, 64, 128, 129, 200, 704, 1000])
+def test_tc_token_small(d, C, T):
+    wl = gin.GdnWorkload("tc", 2, 3, T, d, d, seed=7 * d + C + T, chunk=C)
+    eo, es, info = check(gin.make_inputs(wl))
+    _assert_tc(info)
+    assert info[1] == C
+
+
+@pytest.mark.parametrize("C", [64, 128])
+def test_tc_token_zero_state_and_scale(C):
+    wl = gin.GdnWorkload("tc0", 1, 2, 512, 64, 64, seed=21, chunk=C)
+    inp = gin.make_inputs(wl)
+    check(inp, state_in=None, scale=0.125)
+
+
+def test_tc_token_matches_simt_kernel():
+    """Two independent CUDA implementations (tensor-core chunkwise vs fp32 token loop) agree."""
+    wl = gin.GdnWorkload("x", 1, 4, 1024, 128, 128, seed=22)
+    inp = gin.make_inputs(wl)
+    o1, s1, i1 = run_cuda(inp)
+    o2, s2, i2 = run_cuda(inp, flags=gdn.GDN_FLAG_FORCE_SIMT)
+    assert i1[0] == 1 and i2[0] == 0
+    assert rel_err(o1, o2.double().numpy()) <= TOL_BF16 and rel_err(s1, s2.double().numpy()) <= TOL_BF16
+
+
+@pytest.mark.parametrize("C", [64, 128])
+def test_config2(C):
+    eo, es, info = check(gin.make_inputs(gin.config(2, chunk=C)))
+    _assert_tc(info)
+
+
+@pytest.mark.parametrize("C", [64, 128])
+def test_config3(C):
+    eo, es, info = check(gin.make_inputs(gin.config(3, chunk=C)))
+    _assert_tc(info)
+
+
+def test_config4_stream_of_20_chunks():
+    """20-chunk stream: the CUDA path carries its own fp32 state, the oracle carries its own fp64 state;
+    the error is tracked per chunk (it may accumulate -- that is the point of the config)."""
+    import oracle
+    dev = torch.device("cuda:0")
+    wl = gin.config(4)
+    plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=1, chunk=wl.chunk)
+    inp0 = gin.make_inputs(wl)
+    S_gpu = inp0.state.to(dev)
+    S_ref = inp0.state.double().numpy()
+    out = torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=torch.bfloat16, device=dev)
+    errs = []
+    for i in range(20):
+        inp = gin.make_inputs(gin.config(4, chunk_index=i), with_state=False)
+        plan.forward(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), inp.alpha.to(dev), inp.beta.to(dev), S_gpu, out, S_gpu)
+        torch.cuda.synchronize()
+        o_ref, S_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, S_ref)
+        errs.append((rel_err(out.cpu(), o_ref), rel_err(S_gpu.cpu(), S_ref)))
+    plan.close()
+    print("config 4 per-chunk (err_o, err_S):", [(f"{a:.2e}", f"{b:.2e}") for a, b in errs])
+    assert max(e[0] for e in errs) <= TOL_BF16 and max(e[1] for e in errs) <= TOL_BF16
+
+
+@pytest.mark.parametrize("T", [3520, 10560])
+def test_config5_stress(T):
+    """Strong decay tail (alpha down to ~2e-3): both compute tiles against the oracle and against each other."""
+    res = {}
+    inp = gin.make_inputs(gin.config(5, T=T))
+    o_ref, S_ref = run_oracle(inp)
+    for C in (64, 128):
+        out, S, info = run_cuda(inp, chunk=C)
+        _assert_tc(info)
+        eo, es = rel_err(out, o_ref), rel_err(S, S_ref)
+        assert eo <= TOL_BF16 and es <= TOL_BF16, f"C={C}: err_o={eo:.3e} err_S={es:.3e}"
+        res[C] = (out, S)
+    assert rel_err(res[64][0], res[128][0].double().numpy()) <= TOL_BF16
+    assert rel_err(res[64][1], res[128][1].double().numpy()) <= TOL_BF16
+
+
+@pytest.mark.slow
+def test_config5_T65536_sampled_heads():
+    """Full size (B=2, H=32, T=65536, d=128): the oracle runs on sampled (b,h) streams, every stream is
+    checked for finiteness and C=64 vs C=128 agreement (a property that holds at any size)."""
+    inp = gin.make_inputs(gin.config(5, T=65536))
+    heads = [(0, 0), (1, 17)]
+    ref = run_oracle(inp, heads=heads)
+    outs = {}
+    for C in (128, 64):
+        out, S, info = run_cuda(inp, chunk=C)
+        _assert_tc(info)
+        assert torch.isfinite(out.float()).all() and torch.isfinite(S).all()
+        for (b, h) in heads:
+            o_ref, S_ref = ref[(b, h)]
+            eo, es = rel_err(out[b, :, h], o_ref), rel_err(S[b, h], S_ref)
+            assert eo <= TOL_BF16 and es <= TOL_BF16, f"C={C} stream {(b, h)}: err_o={eo:.3e} err_S={es:.3e}"
+        outs[C] = (out, S)
+    assert rel_err(outs[64][0], outs[128][0].double().numpy()) <= TOL_BF16
+    assert rel_err(outs[64][1], outs[128][1].double().numpy()) <= TOL_BF16
