@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cstdio>
 #include <string>
 
 #include "../../include/gdn.h"
@@ -104,7 +105,7 @@ template <int D, int C>
 inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
     using namespace tok;
     constexpr int NB = D / 64;
-    const size_t smem1 = 3 * NB * kBlk + 6 * kBlk + 2048 + 1024;
+    const size_t smem1 = 3 * NB * kBlk + 6 * kBlk + 4096 + 1024;   // + 18 KB static (sL)
     const size_t smem2 = ChainSmem<D>::TOTAL;
     const size_t smem3 = NB * kBlk + (C == 128 ? 1 : 2) * D * D * 2 + 256 + 1024;
     static bool attr_done = false;
@@ -116,7 +117,7 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
         attr_done = true;
     }
     if (prof) prof->begin(st);
-    gdn_tok_prepass<D, C><<<tp.BH * tp.NT, 128, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, p);
+    gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, p);
     if (prof) prof->mark(st, "gdn_tok_prepass");
     gdn_tok_chain<D><<<tp.BH * (D / 64), 128, smem2, st>>>(tp.tmG, tp.tmN, p);
     if (prof) prof->mark(st, "gdn_tok_chain");
@@ -144,10 +145,27 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
+    p.dbg = nullptr;
+#ifdef GDN_PHASE_TIMING
+    static long long* dbg_dev = nullptr;
+    if (!dbg_dev) { cudaMalloc(&dbg_dev, 64 * sizeof(long long)); cudaMemset(dbg_dev, 0, 64 * sizeof(long long)); }
+    p.dbg = dbg_dev;
+#endif
     cudaError_t e;
     if (tp.D == 64) e = (tp.C == 128) ? tc_launch_token<64, 128>(tp, p, st, prof) : tc_launch_token<64, 64>(tp, p, st, prof);
     else            e = (tp.C == 128) ? tc_launch_token<128, 128>(tp, p, st, prof) : tc_launch_token<128, 64>(tp, p, st, prof);
     if (e != cudaSuccess) { if (err) *err = std::string("token tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+#ifdef GDN_PHASE_TIMING
+    {
+        long long hst[64];
+        cudaStreamSynchronize(st);
+        cudaMemcpy(hst, p.dbg, sizeof(hst), cudaMemcpyDeviceToHost);
+        fprintf(stderr, "[gdn phase cycles]");
+        for (int i = 1; i < 16; ++i) fprintf(stderr, " %d:%lld", i, hst[i] - hst[i - 1]);
+        fprintf(stderr, " [5->19:%lld 19->20:%lld 20->21:%lld 21->16:%lld 16->18:%lld 18->17:%lld 17->6:%lld]", hst[19] - hst[5], hst[20] - hst[19], hst[21] - hst[20], hst[16] - hst[21], hst[18] - hst[16], hst[17] - hst[18], hst[6] - hst[17]);
+        fprintf(stderr, " total:%lld\n", hst[15] - hst[0]);
+    }
+#endif
     return GDN_OK;
 }
 

@@ -40,7 +40,14 @@ struct TokParams {
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
+    long long* dbg;              // developer builds (-DGDN_PHASE_TIMING): per-phase clock64 stamps of CTA 0
 };
+
+#ifdef GDN_PHASE_TIMING
+#define GDN_STAMP(i) do { if (p.dbg && blockIdx.x == 0 && threadIdx.x == 0) p.dbg[i] = clock64(); } while (0)
+#else
+#define GDN_STAMP(i) do { } while (0)
+#endif
 
 namespace tok {
 
@@ -53,12 +60,58 @@ __device__ __forceinline__ void st_global_v4(void* p, uint32_t a, uint32_t b, ui
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Kernel 1: prepass.  grid = BH * NT, block = 128.
+// Kernel 1: prepass.  grid = BH * NT, block = 128 * NH threads (NH warps per TMEM lane quadrant).
+//   Thread (row, hh): row = 32*(warp&3) + lane is the token row / TMEM lane; hh = warp>>2 picks which
+//   CW = 32/NH columns of every 32-column chunk the thread handles, so each scheduler has NH warps to
+//   interleave across the many short dependent phases.  Thread 0 issues TMA and tcgen05.mma.
 // ---------------------------------------------------------------------------------------------------
+constexpr int kPrepassNH = 4;
+constexpr int kPrepassThreads = 128 * kPrepassNH;
+
+// 32x32 unit-lower-triangular inverse, one warp, no shuffles: lane c owns COLUMN c of X = (I + L)^-1.
+// Lt holds L TRANSPOSED (Lt[j*kLsStride + r] = L[r][j]) so that "column j of L" is a broadcast LDS.128
+// row.  Right-looking forward substitution: once x_j is final every later row takes
+// x_r -= L[r][j] x_j (31-j independent FMAs): the serial depth is 31 FMAs, not 31 shuffle rounds.
+constexpr int kLsStride = 36;                     // floats per row: 16-byte aligned, conflict-free
+template <int J>
+__device__ __forceinline__ void inv32_load_row(const float* __restrict__ Lt, float4 (&l)[8]) {
+#pragma unroll
+    for (int r4 = (J + 1) / 4; r4 < 8; ++r4) l[r4] = *reinterpret_cast<const float4*>(Lt + J * kLsStride + 4 * r4);
+}
+template <int J>
+__device__ __forceinline__ void inv32_apply_row(const float4 (&l)[8], float (&x)[32]) {
+    const float xj = x[J];
+#pragma unroll
+    for (int r4 = (J + 1) / 4; r4 < 8; ++r4) {
+        if (4 * r4 + 0 > J) x[4 * r4 + 0] = fmaf(-l[r4].x, xj, x[4 * r4 + 0]);
+        if (4 * r4 + 1 > J) x[4 * r4 + 1] = fmaf(-l[r4].y, xj, x[4 * r4 + 1]);
+        if (4 * r4 + 2 > J) x[4 * r4 + 2] = fmaf(-l[r4].z, xj, x[4 * r4 + 2]);
+        if (4 * r4 + 3 > J) x[4 * r4 + 3] = fmaf(-l[r4].w, xj, x[4 * r4 + 3]);
+    }
+}
+template <int J>
+__device__ __forceinline__ void inv32_steps(const float* __restrict__ Lt, float4 (&cur)[8], float4 (&nxt)[8], float (&x)[32]) {
+    if constexpr (J < 31) {
+        if constexpr (J + 1 < 31) inv32_load_row<J + 1>(Lt, nxt);      // next row's loads fly during this row's FMAs
+        inv32_apply_row<J>(cur, x);
+        inv32_steps<J + 1>(Lt, nxt, cur, x);
+    }
+}
+__device__ __forceinline__ void inv32_columns(const float* __restrict__ Lt, int lane, float (&x)[32]) {
+#pragma unroll
+    for (int r = 0; r < 32; ++r) x[r] = (r == lane) ? 1.f : 0.f;
+    float4 la[8], lb[8];
+    inv32_load_row<0>(Lt, la);
+    inv32_steps<0>(Lt, la, lb, x);
+}
+
 template <int D, int C>
-__global__ void __launch_bounds__(128, 1)
+__global__ void __launch_bounds__(kPrepassThreads, 1)
 gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const TokParams p) {
+    constexpr int NH = kPrepassNH;
+    constexpr int CW = 32 / NH;                   // columns of each 32-column chunk handled per thread
+    constexpr int CH = CW / 8;                    // 16-byte bf16 chunks per thread per 32-column chunk
     constexpr int NB = D / 64;
     constexpr uint32_t TILE = NB * kBlk;
     constexpr int KS = 8;                         // K = 16 steps over the 128 tokens of a tile
@@ -69,34 +122,42 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint8_t* sQ = smem + TILE;
     uint8_t* sV = smem + 2 * TILE;
     uint8_t* sA = smem + 3 * TILE;                // L_off -> Tm diag(beta gamma) -> Ut
-    uint8_t* sB = sA + 2 * kBlk;                  // D (block-diagonal inverse) -> W
+    uint8_t* sB = sA + 2 * kBlk;                  // D (block-diagonal inverse) -> W      (sB directly follows sA)
     uint8_t* sC = sB + 2 * kBlk;                  // X -> Tm diag(beta) -> P
     float* sGam = reinterpret_cast<float*>(sC + 2 * kBlk);     // [128] Gam_i (segmented for C = 64)
     float* sBeta = sGam + 128;                                 // [128] beta_j
     float* sBG = sBeta + 128;                                  // [128] beta_j e^{Gam_j}
-    float* sWarp = sBG + 128;                                  // [4] per-warp sums of log alpha
+    float* sCF = sBG + 128;                                    // [128] e^{Gam_ref(j) - Gam_j}, ref = last row of j's 32-chunk
+    float* sWarp = sCF + 128;                                  // [4] per-warp sums of log alpha
     uint64_t* bars = reinterpret_cast<uint64_t*>(sWarp + 4);   // [3]
+    __shared__ __align__(16) float sL[4 * 32 * kLsStride];     // diagonal 32x32 blocks of L^T (fp32), then of the inverse
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int wq = warp & 3, hh = warp >> 2;
+    const int row = wq * 32 + lane;               // token row == TMEM lane
+    const int cb = hh * CW;                       // this thread's columns inside every 32-column chunk
+    const uint32_t lane_base = (uint32_t)(wq * 32);
     const int tile = blockIdx.x % p.NT, bh = blockIdx.x / p.NT;
     const int b = bh / p.H, h = bh % p.H;
     uint64_t* bar_kq = &bars[0];
     uint64_t* bar_v = &bars[1];
     uint64_t* bar_mma = &bars[2];
+    const uint32_t aA = smem_u32(sA), aB = smem_u32(sB), aC = smem_u32(sC), aK = smem_u32(sK), aQ = smem_u32(sQ), aV = smem_u32(sV);
 
+    GDN_STAMP(0);
+    // gates first: their global-load latency overlaps the barrier / TMEM / TMA set-up
+    const int t = tile * 128 + row;
+    float g = 0.f, beta_i = 0.f;
+    if (t < p.T) {
+        g = p.alpha[(long long)bh * p.T + t];
+        beta_i = p.beta[(long long)bh * p.T + t];
+    } else if (!p.log_alpha) {
+        g = 1.f;
+    }
     if (tid == 0) {
         mbar_init(bar_kq, 1); mbar_init(bar_v, 1); mbar_init(bar_mma, 1);
         mbar_fence_init();
-    }
-    if (warp == 0) tmem_alloc(tmem_slot, 512);
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = *tmem_slot;
-    const uint32_t c0 = tmem, c1 = tmem + 128, c2 = tmem + 256, c3 = tmem + 384;
-
-    if (tid == 0) {
         mbar_expect_tx(bar_kq, 2 * TILE);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
@@ -107,48 +168,70 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, &tmV, bar_v, nb * 64, h, tile * 128, 0, b);
     }
-
-    // ---- T0: gates, in-tile inclusive scan of log alpha ------------------------------------------
-    const int t = tile * 128 + tid;
-    const bool valid = t < p.T;
-    float g = 0.f, beta_i = 0.f;
-    if (valid) {
-        const float a = p.alpha[(long long)bh * p.T + t];
-        g = p.log_alpha ? a : logf(a);
-        beta_i = p.beta[(long long)bh * p.T + t];
+    if (warp == 0) tmem_alloc(tmem_slot, 512);
+    // zero this thread's columns of the three 128x128 operand buffers
+#pragma unroll
+    for (int cc = 0; cc < 4; ++cc) {
+#pragma unroll
+        for (int q2 = 0; q2 < CH; ++q2) {
+            const uint32_t off = swz_chunk_off(row, cc * 4 + hh * CH + q2, kBlk);
+            st_shared_v4(aA + off, 0, 0, 0, 0);
+            st_shared_v4(aB + off, 0, 0, 0, 0);
+            st_shared_v4(aC + off, 0, 0, 0, 0);
+        }
     }
+
+    GDN_STAMP(1);
+    // ---- T0: in-tile inclusive scan of log alpha (every warp of a quadrant computes it, hh == 0 publishes) ----
+    if (!p.log_alpha) g = logf(g);
     float x = g;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const float y = __shfl_up_sync(0xffffffffu, x, o);
         if (lane >= o) x += y;
     }
-    if (lane == 31) sWarp[warp] = x;
+    if (hh == 0 && lane == 31) sWarp[wq] = x;
+    tc_fence_before();
     __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t c0 = tmem, c1 = tmem + 128, c2 = tmem + 256, c3 = tmem + 384;
     float gam_i, gam_end;            // Gam_i and Gam at the end of this row's chunk
     {
         const float w0 = sWarp[0], w1 = sWarp[1], w2 = sWarp[2], w3 = sWarp[3];
         if (C == 128) {
-            gam_i = x + (warp > 0 ? w0 : 0.f) + (warp > 1 ? w1 : 0.f) + (warp > 2 ? w2 : 0.f);
+            gam_i = x + (wq > 0 ? w0 : 0.f) + (wq > 1 ? w1 : 0.f) + (wq > 2 ? w2 : 0.f);
             gam_end = w0 + w1 + w2 + w3;
         } else {
-            gam_i = x + ((warp & 1) ? (warp == 1 ? w0 : w2) : 0.f);
-            gam_end = warp < 2 ? (w0 + w1) : (w2 + w3);
+            gam_i = x + ((wq & 1) ? (wq == 1 ? w0 : w2) : 0.f);
+            gam_end = wq < 2 ? (w0 + w1) : (w2 + w3);
         }
     }
-    sGam[tid] = gam_i;
-    sBeta[tid] = beta_i;
-    sBG[tid] = beta_i * __expf(gam_i);
+    const float gam_ref = __shfl_sync(0xffffffffu, gam_i, 31);     // Gam at the last row of this 32-chunk
+    if (hh == 0) {
+        sGam[row] = gam_i;
+        sBeta[row] = beta_i;
+        sBG[row] = beta_i * fast_exp(gam_i);
+        sCF[row] = fast_exp(gam_ref - gam_i);
+    }
     __syncthreads();
-    const int half_lo = (C == 128) ? 0 : (warp >> 1) * 2;      // first 32-column chunk of this row's chunk
+    const int half_lo = (C == 128) ? 0 : (wq >> 1) * 2;      // first 32-column chunk of this row's chunk
+    // decay factors: e^{Gam_i - Gam_j} = rf[cc] * sCF[j] for j in an earlier 32-chunk cc (both factors <= 1)
+    float rf[3];
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) rf[cc] = (cc < wq && cc >= half_lo) ? fast_exp(gam_i - sGam[cc * 32 + 31]) : 0.f;
 
     uint32_t ph = 0;
+    auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
+    auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
+
+    GDN_STAMP(2);
     // ---- T1: K K^T -> c0, Q K^T -> c1 ------------------------------------------------------------
     mbar_wait(bar_kq, 0);
+    GDN_STAMP(3);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, 128, false, false);
-        const uint32_t aK = smem_u32(sK), aQ = smem_u32(sQ);
 #pragma unroll
         for (int s = 0; s < DS; ++s) {
             const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
@@ -161,145 +244,152 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         umma_commit(bar_mma);
     }
-    mbar_wait(bar_mma, ph); ph ^= 1;
-    tc_fence_after();
+    wait_mma();
 
-    // ---- T2: L (strictly lower, decay-masked), 32x32 diagonal-block inverse in registers ---------
-    float Ld[32];
+    GDN_STAMP(4);
+    // ---- T2: L (strictly lower, decay-masked) -> sA off-diagonal chunks; diagonal 32x32 block -> Ld ----
 #pragma unroll
-    for (int cc = 0; cc < 4; ++cc) {
-        float v[32];
-        if (cc > warp || cc < half_lo) {
+    for (int cc = 0; cc < 3; ++cc) {
+        if (cc < wq && cc >= half_lo) {
+            float v[CW], cf[CW];
+            tmem_ldw(tmem_addr(c0, lane_base, cc * 32 + cb), v);
+            ld_shared_fw(sCF + cc * 32 + cb, cf);
+            const float f = beta_i * rf[cc];
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = 0.f;
-        } else {
-            tmem_ld32(tmem_addr(c0, warp * 32, cc * 32), v);
-#pragma unroll
-            for (int jj = 0; jj < 32; ++jj) {
-                const int j = cc * 32 + jj;
-                v[jj] = (j < tid) ? beta_i * __expf(gam_i - sGam[j]) * v[jj] : 0.f;
-            }
-            if (cc == warp) {
-#pragma unroll
-                for (int jj = 0; jj < 32; ++jj) { Ld[jj] = v[jj]; v[jj] = 0.f; }
-            }
-        }
-        store_row32_bf16(smem_u32(sA), kBlk, tid, cc * 32, v);
-    }
-    float X[32];                                   // row `lane` of (I + Ld)^-1
-#pragma unroll
-    for (int c = 0; c < 32; ++c) X[c] = (c == lane) ? 1.f : 0.f;
-#pragma unroll
-    for (int j = 0; j < 31; ++j) {
-#pragma unroll
-        for (int c = 0; c <= j; ++c) {
-            const float xjc = __shfl_sync(0xffffffffu, X[c], j);
-            if (lane > j) X[c] = fmaf(-Ld[j], xjc, X[c]);
+            for (int e = 0; e < CW; ++e) v[e] *= f * cf[e];
+            store_roww_bf16(aA, kBlk, row, cc * 32 + cb, v);
         }
     }
+    GDN_STAMP(5);
+    float X[CW];                                   // this thread's columns of row `lane` of (I + Ld)^-1
+    {
+        // diagonal 32x32 block: ONE warp per quadrant reads it from TMEM (TMEM reads are the scarce
+        // resource), masks it, shares it through shared memory and inverts it column-wise.
+        float* Lq = sL + wq * 32 * kLsStride;
+        if (hh == 0) {
+            float v0[16], v1[16], g0[16], g1[16];
+            tmem_ld16x2(tmem_addr(c0, lane_base, wq * 32), tmem_addr(c0, lane_base, wq * 32 + 16), v0, v1);
+            GDN_STAMP(19);
+            ld_shared_f16(sGam + wq * 32, g0);
+            ld_shared_f16(sGam + wq * 32 + 16, g1);
+            GDN_STAMP(20);
 #pragma unroll
-    for (int cc = 0; cc < 4; ++cc) {
-        float v[32];
+            for (int e = 0; e < 16; ++e) {
+                // branch-free: clamp the exponent (rows above the diagonal would be > 0), then select
+                const float m0 = (e < lane) ? beta_i : 0.f, m1 = (16 + e < lane) ? beta_i : 0.f;
+                v0[e] *= m0 * fast_exp(fminf(gam_i - g0[e], 0.f));
+                v1[e] *= m1 * fast_exp(fminf(gam_i - g1[e], 0.f));
+            }
+            GDN_STAMP(21);
+            // L^T into the scratch: element (r = lane, j) -> Lq[j][r]
 #pragma unroll
-        for (int j = 0; j < 32; ++j) v[j] = (cc == warp) ? X[j] : 0.f;
-        store_row32_bf16(smem_u32(sB), kBlk, tid, cc * 32, v);
+            for (int e = 0; e < 16; ++e) { Lq[e * kLsStride + lane] = v0[e]; Lq[(16 + e) * kLsStride + lane] = v1[e]; }
+            __syncwarp();
+            GDN_STAMP(16);
+            float xc[32];                          // column `lane` of the inverse
+            inv32_columns(Lq, lane, xc);
+            GDN_STAMP(18);
+            __syncwarp();
+            GDN_STAMP(17);
+            // transpose through the same scratch: element (r, c = lane) -> Lq[r][c]
+#pragma unroll
+            for (int r = 0; r < 32; ++r) Lq[r * kLsStride + lane] = xc[r];
+        }
+        // all NH warps of the quadrant pick up their columns of row `lane`
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + wq), "r"(32 * NH) : "memory");
+        ld_shared_fw(Lq + lane * kLsStride + cb, X);
     }
-    fence_proxy_async();
-    tc_fence_before();
-    __syncthreads();
+    store_roww_bf16(aB, kBlk, row, wq * 32 + cb, X);
+    sync_then_issue();
 
-    // one doubling level: Y = D (L_off D); returns with Y in c0
+    GDN_STAMP(6);
+    // one doubling level: Y = D (L_off D) -> c0.  X1 = L_off D is non-zero only in chunks cc < wq.
     auto doubling_mmas = [&]() {
-        if (tid == 0) {           // X = L_off * D  (A = sA K-major, B = sB MN-major)
+        if (tid == 0) {           // X1 = L_off * D  (A = sA K-major, B = sB MN-major)
             tc_fence_after();
             const uint32_t id = umma_idesc(128, 128, false, true);
-            const uint32_t aA = smem_u32(sA), aB = smem_u32(sB);
 #pragma unroll
             for (int s = 0; s < KS; ++s)
                 umma_bf16(c0, desc_kmajor(aA + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aB + s * 2048, kBlk), id, s > 0);
             umma_commit(bar_mma);
         }
-        mbar_wait(bar_mma, ph); ph ^= 1;
-        tc_fence_after();
+        wait_mma();
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-            float v[32];
-            tmem_ld32(tmem_addr(c0, warp * 32, cc * 32), v);
-            store_row32_bf16(smem_u32(sC), kBlk, tid, cc * 32, v);
+        for (int cc = 0; cc < 3; ++cc) {
+            if (cc < wq && cc >= half_lo) {
+                float v[CW];
+                tmem_ldw(tmem_addr(c0, lane_base, cc * 32 + cb), v);
+                store_roww_bf16(aC, kBlk, row, cc * 32 + cb, v);
+            }
         }
-        fence_proxy_async();
-        tc_fence_before();
-        __syncthreads();
-        if (tid == 0) {           // Y = D * X  (A = sB K-major, B = sC MN-major)
+        sync_then_issue();
+        if (tid == 0) {           // Y = D * X1  (A = sB K-major, B = sC MN-major)
             tc_fence_after();
             const uint32_t id = umma_idesc(128, 128, false, true);
-            const uint32_t aB = smem_u32(sB), aC = smem_u32(sC);
 #pragma unroll
             for (int s = 0; s < KS; ++s)
                 umma_bf16(c0, desc_kmajor(aB + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aC + s * 2048, kBlk), id, s > 0);
             umma_commit(bar_mma);
         }
-        mbar_wait(bar_mma, ph); ph ^= 1;
-        tc_fence_after();
+        wait_mma();
     };
 
     // ---- T3/T4: 32 -> 64 blocks: D' = D - mask(D L_off D) ------------------------------------------
     doubling_mmas();
-    float Dlow[32];                                // block (warp, warp-1) of the 64x64 inverse, odd warps
+    GDN_STAMP(7);
+    float Dlow[CW];                                // block (wq, wq-1) of the 64x64 inverse, odd wq
 #pragma unroll
-    for (int j = 0; j < 32; ++j) Dlow[j] = 0.f;
-    if (warp & 1) {
-        float v[32];
-        tmem_ld32(tmem_addr(c0, warp * 32, (warp - 1) * 32), v);
+    for (int j = 0; j < CW; ++j) Dlow[j] = 0.f;
+    if (wq & 1) {
+        float v[CW];
+        tmem_ldw(tmem_addr(c0, lane_base, (wq - 1) * 32 + cb), v);
 #pragma unroll
-        for (int j = 0; j < 32; ++j) Dlow[j] = -v[j];
-        store_row32_bf16(smem_u32(sB), kBlk, tid, (warp - 1) * 32, Dlow);
+        for (int j = 0; j < CW; ++j) Dlow[j] = -v[j];
+        store_roww_bf16(aB, kBlk, row, (wq - 1) * 32 + cb, Dlow);
     }
-    float Tlow[64];                                // rows >= 64, columns 0..63 of the 128x128 inverse
+    float Tlow[2 * CW];                            // rows >= 64, this thread's columns of chunks 0 and 1
 #pragma unroll
-    for (int j = 0; j < 64; ++j) Tlow[j] = 0.f;
+    for (int j = 0; j < 2 * CW; ++j) Tlow[j] = 0.f;
     if (C == 128) {
-        fence_proxy_async();
-        tc_fence_before();
-        __syncthreads();
+        sync_then_issue();
         doubling_mmas();
-        if (warp >= 2) {
-            float v[32];
-            tmem_ld32(tmem_addr(c0, warp * 32, 0), v);
+        if (wq >= 2) {
+            float v0[CW], v1[CW];
+            tmem_ldw2(tmem_addr(c0, lane_base, cb), tmem_addr(c0, lane_base, 32 + cb), v0, v1);
 #pragma unroll
-            for (int j = 0; j < 32; ++j) Tlow[j] = -v[j];
-            tmem_ld32(tmem_addr(c0, warp * 32, 32), v);
-#pragma unroll
-            for (int j = 0; j < 32; ++j) Tlow[32 + j] = -v[j];
+            for (int j = 0; j < CW; ++j) { Tlow[j] = -v0[j]; Tlow[CW + j] = -v1[j]; }
         }
     }
+    GDN_STAMP(8);
     // ---- scaled copies of Tm: sA = Tm diag(beta gamma), sC = Tm diag(beta) -------------------------
 #pragma unroll
     for (int cc = 0; cc < 4; ++cc) {
-        float va[32], vc[32];
+        if (cc <= wq && cc >= half_lo) {
+            float tm[CW], sbg[CW], sbt[CW], va[CW], vc[CW];
 #pragma unroll
-        for (int jj = 0; jj < 32; ++jj) {
-            float tm;
-            if (cc == warp) tm = X[jj];
-            else if ((warp & 1) && cc == warp - 1) tm = Dlow[jj];
-            else if (C == 128 && warp >= 2 && cc < 2) tm = Tlow[cc * 32 + jj];
-            else tm = 0.f;
-            va[jj] = tm * sBG[cc * 32 + jj];
-            vc[jj] = tm * sBeta[cc * 32 + jj];
+            for (int e = 0; e < CW; ++e) {
+                if (cc == wq) tm[e] = X[e];
+                else if ((wq & 1) && cc == wq - 1) tm[e] = Dlow[e];
+                else if (C == 128 && wq >= 2 && cc < 2) tm[e] = Tlow[cc * CW + e];
+                else tm[e] = 0.f;
+            }
+            ld_shared_fw(sBG + cc * 32 + cb, sbg);
+            ld_shared_fw(sBeta + cc * 32 + cb, sbt);
+#pragma unroll
+            for (int e = 0; e < CW; ++e) { va[e] = tm[e] * sbg[e]; vc[e] = tm[e] * sbt[e]; }
+            store_roww_bf16(aA, kBlk, row, cc * 32 + cb, va);
+            store_roww_bf16(aC, kBlk, row, cc * 32 + cb, vc);
         }
-        store_row32_bf16(smem_u32(sA), kBlk, tid, cc * 32, va);
-        store_row32_bf16(smem_u32(sC), kBlk, tid, cc * 32, vc);
     }
-    fence_proxy_async();
-    tc_fence_before();
-    __syncthreads();
+    sync_then_issue();
 
+    GDN_STAMP(9);
     // ---- T7: W = Tm diag(beta gamma) K -> c2,  Ut = Tm diag(beta) V -> c3 ---------------------------
     mbar_wait(bar_v, 0);
+    GDN_STAMP(10);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, D, false, true);
-        const uint32_t aA = smem_u32(sA), aC = smem_u32(sC), aK = smem_u32(sK), aV = smem_u32(sV);
 #pragma unroll
         for (int s = 0; s < KS; ++s)
             umma_bf16(c2, desc_kmajor(aA + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aK + s * 2048, kBlk), id, s > 0);
@@ -308,133 +398,130 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             umma_bf16(c3, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aV + s * 2048, kBlk), id, s > 0);
         umma_commit(bar_mma);
     }
-    mbar_wait(bar_mma, ph); ph ^= 1;
-    tc_fence_after();
+    wait_mma();
 
+    GDN_STAMP(11);
     // ---- round trip 6: W -> sB, Ut -> sA, P -> sC, Kt in place -------------------------------------
 #pragma unroll
     for (int cc = 0; cc < D / 32; ++cc) {
-        float v[32];
-        tmem_ld32(tmem_addr(c2, warp * 32, cc * 32), v);
-        store_row32_bf16(smem_u32(sB), kBlk, tid, cc * 32, v);
-        tmem_ld32(tmem_addr(c3, warp * 32, cc * 32), v);
-        store_row32_bf16(smem_u32(sA), kBlk, tid, cc * 32, v);
+        float w[CW], u[CW];
+        tmem_ldw2(tmem_addr(c2, lane_base, cc * 32 + cb), tmem_addr(c3, lane_base, cc * 32 + cb), w, u);
+        store_roww_bf16(aB, kBlk, row, cc * 32 + cb, w);
+        store_roww_bf16(aA, kBlk, row, cc * 32 + cb, u);
     }
 #pragma unroll
     for (int cc = 0; cc < 4; ++cc) {
-        float v[32];
-        if (cc > warp || cc < half_lo) {
+        if (cc <= wq && cc >= half_lo) {
+            float v[CW], f[CW];
+            tmem_ldw(tmem_addr(c1, lane_base, cc * 32 + cb), v);
+            if (cc == wq) {                        // same 32-chunk: direct exponentials, diagonal included
+                float gj[CW];
+                ld_shared_fw(sGam + wq * 32 + cb, gj);
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = 0.f;
-        } else {
-            tmem_ld32(tmem_addr(c1, warp * 32, cc * 32), v);
+                for (int e = 0; e < CW; ++e) f[e] = ((cb + e <= lane) ? 1.f : 0.f) * fast_exp(fminf(gam_i - gj[e], 0.f));
+            } else {
+                ld_shared_fw(sCF + cc * 32 + cb, f);
+                const float r = (cc == 0) ? rf[0] : (cc == 1 ? rf[1] : rf[2]);
 #pragma unroll
-            for (int jj = 0; jj < 32; ++jj) {
-                const int j = cc * 32 + jj;
-                v[jj] = (j <= tid) ? __expf(gam_i - sGam[j]) * v[jj] : 0.f;
+                for (int e = 0; e < CW; ++e) f[e] *= r;
             }
+#pragma unroll
+            for (int e = 0; e < CW; ++e) v[e] *= f[e];
+            store_roww_bf16(aC, kBlk, row, cc * 32 + cb, v);
         }
-        store_row32_bf16(smem_u32(sC), kBlk, tid, cc * 32, v);
     }
     {
-        const float ks = __expf(gam_end - gam_i);
+        const float ks = fast_exp(gam_end - gam_i);
 #pragma unroll
-        for (int ch = 0; ch < D / 8; ++ch) {
-            const uint32_t addr = smem_u32(sK) + swz_chunk_off(tid, ch, kBlk);
+        for (int c2i = 0; c2i < D / (8 * NH); ++c2i) {
+            const int ch = c2i * NH + hh;
+            const uint32_t addr = aK + swz_chunk_off(row, ch, kBlk);
             float f[8];
             unpack8(ld_shared_v4(addr), f);
             st_shared_v4(addr, pack_bf16(f[0] * ks, f[1] * ks), pack_bf16(f[2] * ks, f[3] * ks),
                          pack_bf16(f[4] * ks, f[5] * ks), pack_bf16(f[6] * ks, f[7] * ks));
         }
     }
-    fence_proxy_async();
-    tc_fence_before();
-    __syncthreads();
+    sync_then_issue();
 
-    // ---- T8: G = Kt^T W -> c0, N = Kt^T Ut -> c1, P W -> c2, P Ut -> c3 -----------------------------
-    const float gamma_i = __expf(gam_i);
+    GDN_STAMP(12);
+    // ---- T8: [N | G] = Kt^T [Ut | W] -> c0.., [P Ut | P W] -> c2.. (B operand = sA then sB, N = 2D) ----
+    //      column layout of both results: [0, D) from Ut, [D, 2D) from W.  For D = 128 they take 256 columns
+    //      each: [N|G] -> c0,c1 and [PUt|PW] -> c2,c3.
+    const float gamma_i = fast_exp(gam_i);
     constexpr int NHALF = (C == 128) ? 1 : 2;
+    constexpr uint32_t LBO2 = (D == 128) ? kBlk : 2 * kBlk;     // distance between the 64-column blocks of [Ut | W]
 #pragma unroll
     for (int hf = 0; hf < NHALF; ++hf) {
         if (tid == 0) {
             tc_fence_after();
-            const uint32_t aA = smem_u32(sA), aB = smem_u32(sB), aC = smem_u32(sC), aK = smem_u32(sK);
-            const uint32_t idg = umma_idesc(D, D, true, true);
+            const uint32_t idg = umma_idesc(D, 2 * D, true, true);
             const int s_lo = (C == 128) ? 0 : hf * 4, s_hi = (C == 128) ? KS : hf * 4 + 4;
             for (int s = s_lo; s < s_hi; ++s)
-                umma_bf16(c0, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aB + s * 2048, kBlk), idg, s > s_lo);
-            for (int s = s_lo; s < s_hi; ++s)
-                umma_bf16(c1, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aA + s * 2048, kBlk), idg, s > s_lo);
+                umma_bf16(c0, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aA + s * 2048, LBO2), idg, s > s_lo);
             if (hf == 0) {
-                const uint32_t idp = umma_idesc(128, D, false, true);
+                const uint32_t idp = umma_idesc(128, 2 * D, false, true);
 #pragma unroll
                 for (int s = 0; s < KS; ++s)
-                    umma_bf16(c2, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aB + s * 2048, kBlk), idp, s > 0);
-#pragma unroll
-                for (int s = 0; s < KS; ++s)
-                    umma_bf16(c3, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aA + s * 2048, kBlk), idp, s > 0);
+                    umma_bf16(c2, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aA + s * 2048, LBO2), idp, s > 0);
             }
             umma_commit(bar_mma);
         }
-        mbar_wait(bar_mma, ph); ph ^= 1;
-        tc_fence_after();
+        wait_mma();
 
+        GDN_STAMP(13);
         // ---- round trip 7: write the summaries to the workspace ----------------------------------
         const int chunk = (C == 128) ? tile : 2 * tile + hf;
         const long long cidx = (long long)bh * p.NC + chunk;
-        const int m = (D == 128) ? tid : (16 * warp + lane);       // summary row held by this thread
+        const int m = (D == 128) ? row : (16 * wq + lane);          // summary row held by this thread
         const bool m_ok = (D == 128) || (lane < 16);
 #pragma unroll
         for (int cc = 0; cc < D / 32; ++cc) {
-            float v[32];
-            tmem_ld32(tmem_addr(c0, warp * 32, cc * 32), v);
+            float nv[CW], gv[CW];
+            tmem_ldw2(tmem_addr(c0, lane_base, cc * 32 + cb), tmem_addr(c0, lane_base, D + cc * 32 + cb), nv, gv);
             if (m_ok) {
-                __nv_bfloat16* dst = p.Gw + (cidx * D + m) * D + cc * 32;
+                __nv_bfloat16* dg = p.Gw + (cidx * D + m) * D + cc * 32 + cb;
 #pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4)
-                    st_global_v4(dst + q4 * 8, pack_bf16(v[8 * q4], v[8 * q4 + 1]), pack_bf16(v[8 * q4 + 2], v[8 * q4 + 3]),
-                                 pack_bf16(v[8 * q4 + 4], v[8 * q4 + 5]), pack_bf16(v[8 * q4 + 6], v[8 * q4 + 7]));
-            }
-            tmem_ld32(tmem_addr(c1, warp * 32, cc * 32), v);
-            if (m_ok) {
-                float* dst = p.Nw + (cidx * D + m) * D + cc * 32;
+                for (int q4 = 0; q4 < CH; ++q4)
+                    st_global_v4(dg + q4 * 8, pack_bf16(gv[8 * q4], gv[8 * q4 + 1]), pack_bf16(gv[8 * q4 + 2], gv[8 * q4 + 3]),
+                                 pack_bf16(gv[8 * q4 + 4], gv[8 * q4 + 5]), pack_bf16(gv[8 * q4 + 6], gv[8 * q4 + 7]));
+                float* dn = p.Nw + (cidx * D + m) * D + cc * 32 + cb;
 #pragma unroll
-                for (int q4 = 0; q4 < 8; ++q4)
-                    st_global_v4(dst + q4 * 4, __float_as_uint(v[4 * q4]), __float_as_uint(v[4 * q4 + 1]),
-                                 __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
+                for (int q4 = 0; q4 < CW / 4; ++q4)
+                    st_global_v4(dn + q4 * 4, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
+                                 __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
             }
         }
-        if (C == 128) { if (tid == 0) p.gam[cidx] = __expf(gam_end); }
-        else { if (tid == 64 * hf) p.gam[cidx] = __expf(gam_end); }
+        if (C == 128) { if (tid == 0) p.gam[cidx] = fast_exp(gam_end); }
+        else { if (tid == 64 * hf) p.gam[cidx] = fast_exp(gam_end); }
         if (hf == 0) {
-            const long long row = ((long long)bh * p.NT + tile) * 128 + tid;
+            const long long orow = ((long long)bh * p.NT + tile) * 128 + row;
 #pragma unroll
             for (int cc = 0; cc < D / 32; ++cc) {
-                float v[32];
-                tmem_ld32(tmem_addr(c2, warp * 32, cc * 32), v);        // (P W)_i
-                __nv_bfloat16* dq = p.Qt + row * D + cc * 32;
+                float pu[CW], pw[CW];
+                tmem_ldw2(tmem_addr(c2, lane_base, cc * 32 + cb), tmem_addr(c2, lane_base, D + cc * 32 + cb), pu, pw);
+                __nv_bfloat16* dq = p.Qt + orow * D + cc * 32 + cb;
+                __nv_bfloat16* dl = p.Ol + orow * D + cc * 32 + cb;
 #pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4) {
+                for (int q4 = 0; q4 < CH; ++q4) {
                     float f[8];
-                    unpack8(ld_shared_v4(smem_u32(sQ) + swz_chunk_off(tid, cc * 4 + q4, kBlk)), f);
+                    unpack8(ld_shared_v4(aQ + swz_chunk_off(row, cc * 4 + hh * CH + q4, kBlk)), f);
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - v[8 * q4 + e];
+                    for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - pw[8 * q4 + e];
                     st_global_v4(dq + q4 * 8, pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+                    st_global_v4(dl + q4 * 8, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
+                                 pack_bf16(pu[8 * q4 + 4], pu[8 * q4 + 5]), pack_bf16(pu[8 * q4 + 6], pu[8 * q4 + 7]));
                 }
-                tmem_ld32(tmem_addr(c3, warp * 32, cc * 32), v);        // (P Ut)_i
-                __nv_bfloat16* dl = p.Ol + row * D + cc * 32;
-#pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4)
-                    st_global_v4(dl + q4 * 8, pack_bf16(v[8 * q4], v[8 * q4 + 1]), pack_bf16(v[8 * q4 + 2], v[8 * q4 + 3]),
-                                 pack_bf16(v[8 * q4 + 4], v[8 * q4 + 5]), pack_bf16(v[8 * q4 + 6], v[8 * q4 + 7]));
             }
         }
         if (hf + 1 < NHALF) { tc_fence_before(); __syncthreads(); }
     }
 
+    GDN_STAMP(14);
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, 512);
+    GDN_STAMP(15);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -508,21 +595,27 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
 #pragma unroll
         for (int i = 0; i < 64; ++i) S[i] = 0.f;
     }
-    // publish S (bf16): shared operand buffer `buf` + global snapshot for chunk `c` (read by kernel 3)
-    auto publish = [&](int buf, int c) {
+    // publish S (bf16) as the next MMA's B operand (shared buffer `buf`)
+    auto publish_smem = [&](int buf) {
         if (m_ok) {
             const uint32_t sbase = smem_u32(sS + buf * L::S_BYTES);
-            __nv_bfloat16* g = p.Sc + (((long long)bh * p.NC + c) * D + m) * D + n0;
 #pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-                const uint32_t a = pack_bf16(S[8 * ch], S[8 * ch + 1]), b2 = pack_bf16(S[8 * ch + 2], S[8 * ch + 3]);
-                const uint32_t c2 = pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), d2 = pack_bf16(S[8 * ch + 6], S[8 * ch + 7]);
-                st_shared_v4(sbase + swz_chunk_off(m, ch, 0), a, b2, c2, d2);
-                if (c < p.NC) st_global_v4(g + ch * 8, a, b2, c2, d2);
-            }
+            for (int ch = 0; ch < 8; ++ch)
+                st_shared_v4(sbase + swz_chunk_off(m, ch, 0), pack_bf16(S[8 * ch], S[8 * ch + 1]), pack_bf16(S[8 * ch + 2], S[8 * ch + 3]),
+                             pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), pack_bf16(S[8 * ch + 6], S[8 * ch + 7]));
         }
     };
-    publish(0, 0);
+    // snapshot of the state at the start of chunk c for kernel 3 (off the critical path: issued after the MMA)
+    auto publish_global = [&](int c) {
+        if (m_ok && c < p.NC) {
+            __nv_bfloat16* g = p.Sc + (((long long)bh * p.NC + c) * D + m) * D + n0;
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch)
+                st_global_v4(g + ch * 8, pack_bf16(S[8 * ch], S[8 * ch + 1]), pack_bf16(S[8 * ch + 2], S[8 * ch + 3]),
+                             pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), pack_bf16(S[8 * ch + 6], S[8 * ch + 7]));
+        }
+    };
+    publish_smem(0);
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
@@ -543,6 +636,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
                 umma_bf16(tmem, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), id, s > 0);
             umma_commit(bar_mma);
         }
+        publish_global(c);                         // S still holds the state at the start of chunk c
         mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
         tc_fence_after();
         // S <- gamma_c S - G_c S + N_c
@@ -563,7 +657,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
                 }
             }
         }
-        publish((c + 1) & 1, c + 1);
+        publish_smem((c + 1) & 1);
         fence_proxy_async();
         tc_fence_before();
         __syncthreads();
