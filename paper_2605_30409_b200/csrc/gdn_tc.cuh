@@ -22,7 +22,7 @@ struct TcPlan {
     // token path workspace
     __nv_bfloat16 *Gw = nullptr, *Qt = nullptr, *Ol = nullptr, *Sc = nullptr;
     float *Nw = nullptr, *gam = nullptr;
-    CUtensorMap tmG, tmN, tmQt, tmSc;          // static (workspace) maps
+    CUtensorMap tmG, tmN, tmQt, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr;
     CUtensorMap tmQ, tmK, tmV;
@@ -75,6 +75,11 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         ok = ok && tc::make_tmap(&tp.tmG, tp.Gw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
         ok = ok && tc::make_tmap(&tp.tmSc, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
+    {   // S_c snapshots written by the chain: one column tile [D rows][64 cols] per TMA store
+        const uint64_t dims[3] = {D, D, BH * NC}, str[3] = {2, D * 2, D * D * 2};
+        const uint32_t box[3] = {64, (uint32_t)D, 1};
+        ok = ok && tc::make_tmap(&tp.tmScS, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+    }
     {   // N_c: fp32 (D, D, BH*NC), box {32, D, 1}
         const uint64_t dims[3] = {D, D, BH * NC}, str[3] = {4, D * 4, D * D * 4};
         const uint32_t box[3] = {32, (uint32_t)D, 1};
@@ -119,7 +124,7 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
     if (prof) prof->begin(st);
     gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, p);
     if (prof) prof->mark(st, "gdn_tok_prepass");
-    gdn_tok_chain<D><<<tp.BH * (D / 64), 128, smem2, st>>>(tp.tmG, tp.tmN, p);
+    gdn_tok_chain<D><<<tp.BH * (D / 64), kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, p);
     if (prof) prof->mark(st, "gdn_tok_chain");
     gdn_tok_output<D, C><<<tp.BH * tp.NT, 128, smem3, st>>>(tp.tmQt, tp.tmSc, p);
     if (prof) prof->mark(st, "gdn_tok_output");
@@ -164,6 +169,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         for (int i = 1; i < 16; ++i) fprintf(stderr, " %d:%lld", i, hst[i] - hst[i - 1]);
         fprintf(stderr, " [5->19:%lld 19->20:%lld 20->21:%lld 21->16:%lld 16->18:%lld 18->17:%lld 17->6:%lld]", hst[19] - hst[5], hst[20] - hst[19], hst[21] - hst[20], hst[16] - hst[21], hst[18] - hst[16], hst[17] - hst[18], hst[6] - hst[17]);
         fprintf(stderr, " total:%lld\n", hst[15] - hst[0]);
+        fprintf(stderr, "[gdn chain step cycles] snapshot:%lld premath:%lld wait_mma:%lld ld+sub:%lld publish:%lld fence+sync:%lld total:%lld\n",
+                hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36], hst[38] - hst[37], hst[38] - hst[32]);
     }
 #endif
     return GDN_OK;

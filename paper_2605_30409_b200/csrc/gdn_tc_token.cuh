@@ -540,9 +540,12 @@ struct ChainSmem {
     static constexpr uint32_t TOTAL = STAGES * STAGE + 2 * S_BYTES + 256 + 1024;
 };
 
+constexpr int kChainThreads = 192;     // warps 0-3: state rows (epilogue); warp 4: MMA issuer; warp 5: TMA producer
+
 template <int D>
-__global__ void __launch_bounds__(128, 1)
-gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN, const TokParams p) {
+__global__ void __launch_bounds__(kChainThreads, 1)
+gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN,
+              const __grid_constant__ CUtensorMap tmSc, const TokParams p) {
     using L = ChainSmem<D>;
     constexpr int NB = L::NB;
     constexpr int STAGES = L::STAGES;
@@ -557,8 +560,9 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
     constexpr int NT_COL = D / 64;
     const int ct = blockIdx.x % NT_COL, bh = blockIdx.x / NT_COL;
     const int n0 = ct * 64;
-    const int m = (D == 128) ? tid : (16 * warp + lane);
-    const bool m_ok = (D == 128) || (lane < 16);
+    const bool worker = warp < 4;
+    const int m = (D == 128) ? tid : (16 * warp + lane);              // state row of a worker thread
+    const bool m_ok = worker && ((D == 128) || (lane < 16));
     uint64_t* bar_mma = &bars[STAGES];
 
     if (tid == 0) {
@@ -582,7 +586,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
         tma_load_3d(base + L::G_BYTES, &tmN, &bars[st], n0, 0, z);
         tma_load_3d(base + L::G_BYTES + D * 128, &tmN, &bars[st], n0 + 32, 0, z);
     };
-    if (tid == 0)
+    if (warp == 5 && lane == 0)
         for (int c = 0; c < STAGES && c < p.NC; ++c) issue_loads(c);
 
     // state row m, columns n0..n0+63, fp32 master copy in registers
@@ -605,68 +609,97 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
                              pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), pack_bf16(S[8 * ch + 6], S[8 * ch + 7]));
         }
     };
-    // snapshot of the state at the start of chunk c for kernel 3 (off the critical path: issued after the MMA)
-    auto publish_global = [&](int c) {
-        if (m_ok && c < p.NC) {
-            __nv_bfloat16* g = p.Sc + (((long long)bh * p.NC + c) * D + m) * D + n0;
-#pragma unroll
-            for (int ch = 0; ch < 8; ++ch)
-                st_global_v4(g + ch * 8, pack_bf16(S[8 * ch], S[8 * ch + 1]), pack_bf16(S[8 * ch + 2], S[8 * ch + 3]),
-                             pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), pack_bf16(S[8 * ch + 6], S[8 * ch + 7]));
-        }
-    };
-    publish_smem(0);
+    if (worker) publish_smem(0);
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
 
-    uint32_t ph_mma = 0;
-    for (int c = 0; c < p.NC; ++c) {
-        const int st = c % STAGES;
-        const uint32_t ph_full = (uint32_t)(c / STAGES) & 1u;
-        const float gamma_c = p.gam[(long long)bh * p.NC + c];
-        uint8_t* base = sStage + st * L::STAGE;
-        mbar_wait(&bars[st], ph_full);
-        if (tid == 0) {
-            tc_fence_after();
-            const uint32_t id = umma_idesc(D, 64, false, true);
-            const uint32_t aG = smem_u32(base), aS = smem_u32(sS + (c & 1) * L::S_BYTES);
+    if (warp == 4) {
+        // ===== MMA issuer: D[tmem] = G_c (A, K-major) * S_c (B, MN-major), one commit per chunk =====
+        const uint32_t id = umma_idesc(D, 64, false, true);
+        for (int c = 0; c < p.NC; ++c) {
+            const int st = c % STAGES;
+            if (lane == 0) {
+                mbar_wait(&bars[st], (uint32_t)(c / STAGES) & 1u);
+                tc_fence_after();
+                const uint32_t aG = smem_u32(sStage + st * L::STAGE), aS = smem_u32(sS + (c & 1) * L::S_BYTES);
 #pragma unroll
-            for (int s = 0; s < D / 16; ++s)
-                umma_bf16(tmem, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), id, s > 0);
-            umma_commit(bar_mma);
+                for (int s = 0; s < D / 16; ++s)
+                    umma_bf16(tmem, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), id, s > 0);
+                umma_commit(bar_mma);
+            }
+            __syncwarp();
+            tc_fence_before();
+            __syncthreads();
         }
-        publish_global(c);                         // S still holds the state at the start of chunk c
-        mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
-        tc_fence_after();
-        // S <- gamma_c S - G_c S + N_c
-#pragma unroll
-        for (int cc = 0; cc < 2; ++cc) {
-            float v[32];
-            tmem_ld32(tmem_addr(tmem, warp * 32, cc * 32), v);
-            if (m_ok) {
-                const uint32_t nbase = smem_u32(base + L::G_BYTES + cc * (D * 128));
-#pragma unroll
-                for (int ch = 0; ch < 8; ++ch) {
-                    const uint4 u = ld_shared_v4(nbase + swz_chunk_off(m, ch, 0));
-                    const int i0 = cc * 32 + ch * 4;
-                    S[i0 + 0] = fmaf(gamma_c, S[i0 + 0], __uint_as_float(u.x) - v[ch * 4 + 0]);
-                    S[i0 + 1] = fmaf(gamma_c, S[i0 + 1], __uint_as_float(u.y) - v[ch * 4 + 1]);
-                    S[i0 + 2] = fmaf(gamma_c, S[i0 + 2], __uint_as_float(u.z) - v[ch * 4 + 2]);
-                    S[i0 + 3] = fmaf(gamma_c, S[i0 + 3], __uint_as_float(u.w) - v[ch * 4 + 3]);
-                }
+    } else if (warp == 5) {
+        // ===== TMA producer: refill a stage as soon as the step that used it has ended, and write the bf16
+        //       operand tile sS (= state at the start of chunk c) to the workspace for kernel 3 with one TMA
+        //       store straight from shared memory (no per-thread global stores on the chain) =====
+        auto store_snapshot = [&](int c) {           // sS[c & 1] holds the state at the start of chunk c
+            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NC + c);
+            tma_store_commit();
+        };
+        if (lane == 0) store_snapshot(0);
+        for (int c = 0; c < p.NC; ++c) {
+            if (lane == 0) tma_store_wait_read();    // snapshot c has left sS[c & 1] before step c+1 may overwrite it
+            __syncthreads();                          // end of step c: sS[(c+1) & 1] published, stage c % STAGES free
+            if (lane == 0) {
+                if (c + 1 < p.NC) store_snapshot(c + 1);
+                if (c + STAGES < p.NC) issue_loads(c + STAGES);
             }
         }
-        publish_smem((c + 1) & 1);
-        fence_proxy_async();
-        tc_fence_before();
-        __syncthreads();
-        if (tid == 0 && c + STAGES < p.NC) issue_loads(c + STAGES);
-    }
-    if (m_ok) {
-        float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + n0);
+        if (lane == 0) tma_store_wait_all();
+    } else {
+        // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
+        uint32_t ph_mma = 0;
+        float gamma_c = p.gam[(long long)bh * p.NC];
+        for (int c = 0; c < p.NC; ++c) {
+            const int st = c % STAGES;
+            uint8_t* base = sStage + st * L::STAGE;
+            const float gamma_next = (c + 1 < p.NC) ? p.gam[(long long)bh * p.NC + c + 1] : 0.f;
+            if (c == 10) GDN_STAMP(32);
+            if (c == 10) GDN_STAMP(33);
+            mbar_wait(&bars[st], (uint32_t)(c / STAGES) & 1u);
+            if (m_ok) {                                // state-independent part while the MMA runs
 #pragma unroll
-        for (int i = 0; i < 16; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+                for (int cc = 0; cc < 2; ++cc) {
+                    const uint32_t nbase = smem_u32(base + L::G_BYTES + cc * (D * 128));
+#pragma unroll
+                    for (int ch = 0; ch < 8; ++ch) {
+                        const uint4 u = ld_shared_v4(nbase + swz_chunk_off(m, ch, 0));
+                        const int i0 = cc * 32 + ch * 4;
+                        S[i0 + 0] = fmaf(gamma_c, S[i0 + 0], __uint_as_float(u.x));
+                        S[i0 + 1] = fmaf(gamma_c, S[i0 + 1], __uint_as_float(u.y));
+                        S[i0 + 2] = fmaf(gamma_c, S[i0 + 2], __uint_as_float(u.z));
+                        S[i0 + 3] = fmaf(gamma_c, S[i0 + 3], __uint_as_float(u.w));
+                    }
+                }
+            }
+            if (c == 10) GDN_STAMP(34);
+            mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
+            tc_fence_after();
+            if (c == 10) GDN_STAMP(35);
+            {
+                float v[64];
+                tmem_ld64(tmem_addr(tmem, warp * 32, 0), v);
+#pragma unroll
+                for (int i = 0; i < 64; ++i) S[i] -= v[i];
+            }
+            if (c == 10) GDN_STAMP(36);
+            publish_smem((c + 1) & 1);
+            if (c == 10) GDN_STAMP(37);
+            fence_proxy_async();
+            tc_fence_before();
+            __syncthreads();
+            if (c == 10) GDN_STAMP(38);
+            gamma_c = gamma_next;
+        }
+        if (m_ok) {
+            float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + n0);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+        }
     }
     tc_fence_before();
     __syncthreads();
