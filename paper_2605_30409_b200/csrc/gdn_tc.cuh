@@ -9,6 +9,7 @@
 #include "../../include/gdn.h"
 #include "gdn_profile.cuh"
 #include "gdn_tc_token.cuh"
+#include "gdn_tc_frame.cuh"
 #include "tc_tmap.cuh"
 
 namespace gdn {
@@ -16,12 +17,14 @@ namespace gdn {
 struct TcPlan {
     bool ready = false;
     int sm_count = 0;
+    int mode = 0;                              // GDN_PATH_TC_TOKEN or GDN_PATH_TC_FRAME
     int D = 0, C = 0, NT = 0, NC = 0, BH = 0;
+    int G = 1, F = 0, TPF = 0, NSPLIT = 1, NSc = 0;   // frame-wise: frames, 128-token tiles per frame, token splits
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
     // token path workspace
     __nv_bfloat16 *Gw = nullptr, *Qt = nullptr, *Ol = nullptr, *Sc = nullptr;
-    float *Nw = nullptr, *gam = nullptr;
+    float *Nw = nullptr, *gam = nullptr, *part = nullptr;
     CUtensorMap tmG, tmN, tmQt, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr;
@@ -34,7 +37,12 @@ inline int tc_default_chunk(const gdn_config_t& c) { return c.chunk ? c.chunk : 
 inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, int* launches) {
     if (c.io_dtype != GDN_BF16) return false;
     if (c.d_k != c.d_v || !(c.d_k == 64 || c.d_k == 128)) return false;
-    if (c.group != 1) return false;                                   // frame-wise tensor-core path: not yet
+    if (c.group != 1) {                                               // frame-wise (the paper's variant)
+        *path = GDN_PATH_TC_FRAME;
+        *chunk = 0;
+        *launches = 4;
+        return true;
+    }
     *path = GDN_PATH_TC_TOKEN;
     *chunk = tc_default_chunk(c);
     *launches = 3;
@@ -43,13 +51,73 @@ inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, in
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// token splits per frame for Phase A: minimise (waves x tiles per split), small penalty per extra partial
+inline int frame_splits(int units, int tpf, int sms) {
+    int best = 1;
+    double best_cost = 1e30;
+    for (int ns = 1; ns <= tpf; ++ns) {
+        const int per = (tpf + ns - 1) / ns;
+        if ((ns - 1) * per >= tpf) continue;                   // would leave an empty split
+        const long long ctas = (long long)units * ns;
+        const double cost = (double)((ctas + sms - 1) / sms) * per + 0.3 * ns;
+        if (cost < best_cost) { best_cost = cost; best = ns; }
+    }
+    return best;
+}
+
+inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm_count, std::string* err) {
+    tp.mode = GDN_PATH_TC_FRAME;
+    tp.sm_count = sm_count;
+    tp.D = c.d_k; tp.C = 0; tp.BH = c.B * c.H;
+    tp.G = c.group; tp.F = c.T / c.group; tp.TPF = (c.group + 127) / 128;
+    tp.NC = tp.F; tp.NSc = tp.F + 1; tp.NT = tp.F * tp.TPF;
+    tp.NSPLIT = frame_splits(tp.BH * tp.F, tp.TPF, sm_count > 0 ? sm_count : 148);
+    const size_t D = tp.D, BH = tp.BH, F = tp.F, NS = tp.NSPLIT;
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
+    const size_t oP = carve(BH * F * NS * D * 2 * D * 4), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
+    const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2);
+    if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
+        cudaGetLastError();
+        if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
+        return GDN_ERR_NOMEM;
+    }
+    tp.workspace_bytes = off;
+    uint8_t* w = static_cast<uint8_t*>(tp.workspace);
+    tp.part = reinterpret_cast<float*>(w + oP);
+    tp.Gw = reinterpret_cast<__nv_bfloat16*>(w + oG);
+    tp.Nw = reinterpret_cast<float*>(w + oN);
+    tp.gam = reinterpret_cast<float*>(w + oGam);
+    tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
+    bool ok = true;
+    {
+        const uint64_t dims[3] = {D, D, BH * F}, str[3] = {2, D * 2, D * D * 2};
+        const uint32_t box[3] = {64, (uint32_t)D, 1};
+        ok = ok && tc::make_tmap(&tp.tmG, tp.Gw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        const uint64_t dimsS[3] = {D, D, BH * (F + 1)};
+        ok = ok && tc::make_tmap(&tp.tmSc, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        ok = ok && tc::make_tmap(&tp.tmScS, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+    }
+    {
+        const uint64_t dims[3] = {D, D, BH * F}, str[3] = {4, D * 4, D * D * 4};
+        const uint32_t box[3] = {32, (uint32_t)D, 1};
+        ok = ok && tc::make_tmap(&tp.tmN, tp.Nw, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+    }
+    if (!ok) { cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
+    tp.ready = true;
+    return GDN_OK;
+}
+
 inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count, std::string* err) {
+    if (c.group != 1) return tc_plan_init_frame(tp, c, sm_count, err);
+    tp.mode = GDN_PATH_TC_TOKEN;
     tp.sm_count = sm_count;
     tp.D = c.d_k;
     tp.C = tc_default_chunk(c);
     tp.BH = c.B * c.H;
     tp.NT = (c.T + 127) / 128;
     tp.NC = tp.C == 128 ? tp.NT : 2 * tp.NT;
+    tp.NSc = tp.NC;
     const size_t D = tp.D, BH = tp.BH, NT = tp.NT, NC = tp.NC;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
@@ -131,22 +199,64 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
     return cudaGetLastError();
 }
 
+template <int D>
+inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof) {
+    using namespace frm;
+    constexpr int NB = D / 64;
+    const size_t smem1 = SumSmem<D>::TOTAL;
+    const size_t smem2 = tok::ChainSmem<D>::TOTAL;
+    const size_t smem3 = NB * tok::kBlk + D * D * 2 + 256 + 1024;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = set_smem(gdn_frm_summaries<D>, smem1);
+        if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain<D>, smem2);
+        if (e == cudaSuccess) e = set_smem(gdn_frm_readout<D>, smem3);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    if (prof) prof->begin(st);
+    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT, kSumThreads, smem1, st>>>(tp.tmK, tp.tmV, fp);
+    if (prof) prof->mark(st, "gdn_frm_summaries");
+    gdn_frm_reduce<D><<<dim3(tp.BH * tp.F, kReduceSlices), 256, 0, st>>>(fp);
+    if (prof) prof->mark(st, "gdn_frm_reduce");
+    tok::gdn_tok_chain<D><<<tp.BH * (D / 64), tok::kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, cp);
+    if (prof) prof->mark(st, "gdn_tok_chain");
+    gdn_frm_readout<D><<<tp.BH * tp.F * tp.TPF, 128, smem3, st>>>(tp.tmQ, tp.tmSc, fp);
+    if (prof) prof->mark(st, "gdn_frm_readout");
+    return cudaGetLastError();
+}
+
 inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q, const void* k, const void* v,
                                const float* alpha, const float* beta, const float* S_in, void* out, float* S_out,
                                cudaStream_t st, Profiler* prof, std::string* err) {
     if (!tp.ready) { if (err) *err = "tensor-core plan was not initialised (no sm_100 device at plan time)"; return GDN_ERR_ARCH; }
     auto ts = [&](long long s, int d) { return s ? s : (long long)c.H * d; };
     if (q != tp.cq || k != tp.ck || v != tp.cv) {
-        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, c.T, ts(c.q_token_stride, c.d_k), 128, err) &&
-                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, c.T, ts(c.k_token_stride, c.d_k), 128, err) &&
-                  tc::make_act_tmap(&tp.tmV, v, c.B, c.T, c.H, c.d_v, c.T, ts(c.v_token_stride, c.d_v), 128, err);
+        const int Gm = (tp.mode == GDN_PATH_TC_FRAME) ? c.group : c.T;      // token-wise: one "frame" of T tokens
+        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, Gm, ts(c.q_token_stride, c.d_k), 128, err) &&
+                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, Gm, ts(c.k_token_stride, c.d_k), 128, err) &&
+                  tc::make_act_tmap(&tp.tmV, v, c.B, c.T, c.H, c.d_v, Gm, ts(c.v_token_stride, c.d_v), 128, err);
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
+    }
+    if (tp.mode == GDN_PATH_TC_FRAME) {
+        FrmParams fp{};
+        fp.alpha = alpha; fp.beta = beta; fp.out = out; fp.part = tp.part; fp.Gw = tp.Gw; fp.Nw = tp.Nw; fp.gam = tp.gam;
+        fp.B = c.B; fp.H = c.H; fp.T = c.T; fp.G = tp.G; fp.F = tp.F; fp.NSPLIT = tp.NSPLIT; fp.TPF = tp.TPF; fp.NSc = tp.NSc;
+        fp.o_ts = ts(c.o_token_stride, c.d_v);
+        fp.scale = c.scale;
+        fp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
+        TokParams cp{};
+        cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
+        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
+        const cudaError_t e = (tp.D == 64) ? tc_launch_frame<64>(tp, fp, cp, st, prof) : tc_launch_frame<128>(tp, fp, cp, st, prof);
+        if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+        return GDN_OK;
     }
     TokParams p{};
     p.alpha = alpha; p.beta = beta; p.S_in = S_in; p.S_out = S_out; p.out = out;
     p.Gw = tp.Gw; p.Nw = tp.Nw; p.gam = tp.gam; p.Qt = tp.Qt; p.Ol = tp.Ol; p.Sc = tp.Sc;
-    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC;
+    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC; p.NSc = tp.NSc;
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;

@@ -37,6 +37,7 @@ struct TokParams {
     __nv_bfloat16* Ol;           // [BH][NT*128][D]    Ol rows
     __nv_bfloat16* Sc;           // [BH][NC][D][D]     state at chunk start (bf16 MMA operand)
     int B, H, T, NT, NC;
+    int NSc;                     // snapshot slots per (b,h) in Sc: NC (token-wise) or NC + 1 (frame-wise: also the final state)
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
@@ -637,7 +638,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
         //       operand tile sS (= state at the start of chunk c) to the workspace for kernel 3 with one TMA
         //       store straight from shared memory (no per-thread global stores on the chain) =====
         auto store_snapshot = [&](int c) {           // sS[c & 1] holds the state at the start of chunk c
-            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NC + c);
+            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + c);
             tma_store_commit();
         };
         if (lane == 0) store_snapshot(0);
@@ -645,7 +646,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
             if (lane == 0) tma_store_wait_read();    // snapshot c has left sS[c & 1] before step c+1 may overwrite it
             __syncthreads();                          // end of step c: sS[(c+1) & 1] published, stage c % STAGES free
             if (lane == 0) {
-                if (c + 1 < p.NC) store_snapshot(c + 1);
+                if (c + 1 < p.NSc) store_snapshot(c + 1);
                 if (c + STAGES < p.NC) issue_loads(c + STAGES);
             }
         }
@@ -743,7 +744,7 @@ gdn_tok_output(const __grid_constant__ CUtensorMap tmQt, const __grid_constant__
         for (int s = 0; s < NS; ++s)
 #pragma unroll
             for (int nb = 0; nb < NB; ++nb)
-                tma_load_3d(sS + s * S_BYTES + nb * (D * 128), &tmSc, &bars[0], nb * 64, 0, bh * p.NC + tile * NS + s);
+                tma_load_3d(sS + s * S_BYTES + nb * (D * 128), &tmSc, &bars[0], nb * 64, 0, bh * p.NSc + tile * NS + s);
     }
     // prefetch this row's Ol
     uint4 ol[D / 8];

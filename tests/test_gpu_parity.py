@@ -284,3 +284,93 @@ def test_config5_T65536_sampled_heads():
         outs[C] = (out, S)
     assert rel_err(outs[64][0], outs[128][0].double().numpy()) <= TOL_BF16
     assert rel_err(outs[64][1], outs[128][1].double().numpy()) <= TOL_BF16
+
+
+# =====================================================================================================
+# Tensor-core (tcgen05) frame-wise path: the paper's variant (G = tokens per frame), same shapes
+# =====================================================================================================
+def _assert_tc_frame(info):
+    assert info[0] == 2, f"expected the tensor-core frame path, plan resolved to {info}"
+
+
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("G,F", [(1 * 128, 1), (100, 3), (128, 4), (352, 2), (880, 3), (1000, 2)])
+def test_tc_frame_small(d, G, F):
+    wl = gin.GdnWorkload("tcF", 2, 3, G * F, d, d, group=G, seed=3 * d + G + F)
+    eo, es, info = check(gin.make_inputs(wl))
+    _assert_tc_frame(info)
+
+
+def test_tc_frame_zero_state_scale_and_log_alpha():
+    wl = gin.GdnWorkload("tcF0", 1, 2, 3 * 352, 64, 64, group=352, seed=31)
+    inp = gin.make_inputs(wl)
+    check(inp, state_in=None, scale=0.5)
+    o1, s1, _ = run_cuda(inp)
+    inp2 = gin.make_inputs(wl)
+    inp2.alpha = torch.log(inp.alpha)
+    o2, s2, _ = run_cuda(inp2, flags=gdn.GDN_FLAG_LOG_ALPHA)
+    assert rel_err(o2, o1.double().numpy()) < 1e-2 and rel_err(s2, s1.double().numpy()) < 1e-3
+
+
+def test_tc_frame_matches_simt_kernel():
+    wl = gin.GdnWorkload("xF", 1, 4, 2 * 880, 128, 128, group=880, seed=32)
+    inp = gin.make_inputs(wl)
+    o1, s1, i1 = run_cuda(inp)
+    o2, s2, i2 = run_cuda(inp, flags=gdn.GDN_FLAG_FORCE_SIMT)
+    assert i1[0] == 2 and i2[0] == 0
+    assert rel_err(o1, o2.double().numpy()) <= TOL_BF16 and rel_err(s1, s2.double().numpy()) <= TOL_BF16
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_config_frame_variants(cfg):
+    eo, es, info = check(gin.make_inputs(gin.config(cfg, frame=True)))
+    _assert_tc_frame(info)
+
+
+@pytest.mark.parametrize("frames", [3, 5])
+def test_paper_shape(frames):
+    """The paper's production chunk: 880 tokens per frame (22x40), 20 heads, d = 128; 5-frame first chunk, 3 after."""
+    eo, es, info = check(gin.make_inputs(gin.paper_shape(frames)))
+    _assert_tc_frame(info)
+
+
+def test_config4_frame_stream():
+    """Frame-wise 20-chunk stream with carried state (config 4, G = 3520)."""
+    import oracle
+    dev = torch.device("cuda:0")
+    wl = gin.config(4, frame=True)
+    plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group)
+    inp0 = gin.make_inputs(wl)
+    S_gpu = inp0.state.to(dev)
+    S_ref = inp0.state.double().numpy()
+    out = torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=torch.bfloat16, device=dev)
+    errs = []
+    for i in range(20):
+        inp = gin.make_inputs(gin.config(4, frame=True, chunk_index=i), with_state=False)
+        plan.forward(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), inp.alpha.to(dev), inp.beta.to(dev), S_gpu, out, S_gpu)
+        torch.cuda.synchronize()
+        o_ref, S_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, S_ref, group=wl.group)
+        errs.append((rel_err(out.cpu(), o_ref), rel_err(S_gpu.cpu(), S_ref)))
+    plan.close()
+    print("config 4 (frame-wise) per-chunk (err_o, err_S):", [(f"{a:.2e}", f"{b:.2e}") for a, b in errs])
+    assert max(e[0] for e in errs) <= TOL_BF16 and max(e[1] for e in errs) <= TOL_BF16
+
+
+@pytest.mark.parametrize("T", [3520, 10560])
+def test_config5_frame(T):
+    eo, es, info = check(gin.make_inputs(gin.config(5, T=T, frame=True)))
+    _assert_tc_frame(info)
+
+
+@pytest.mark.slow
+def test_config5_frame_T65536_sampled_heads():
+    inp = gin.make_inputs(gin.config(5, T=65536, frame=True))
+    heads = [(0, 3), (1, 30)]
+    ref = run_oracle(inp, heads=heads)
+    out, S, info = run_cuda(inp)
+    _assert_tc_frame(info)
+    assert torch.isfinite(out.float()).all() and torch.isfinite(S).all()
+    for (b, h) in heads:
+        o_ref, S_ref = ref[(b, h)]
+        eo, es = rel_err(out[b, :, h], o_ref), rel_err(S[b, h], S_ref)
+        assert eo <= TOL_BF16 and es <= TOL_BF16, f"stream {(b, h)}: err_o={eo:.3e} err_S={es:.3e}"
