@@ -25,7 +25,7 @@ struct TcPlan {
     // token path workspace
     __nv_bfloat16 *Gw = nullptr, *Qt = nullptr, *Ol = nullptr, *Sc = nullptr;
     float *Nw = nullptr, *gam = nullptr, *part = nullptr;
-    CUtensorMap tmG, tmN, tmQt, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
+    CUtensorMap tmG, tmN, tmQt, tmOl, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr;
     CUtensorMap tmQ, tmK, tmV;
@@ -157,6 +157,7 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         const uint64_t dims[2] = {D, BH * NT * 128}, str[2] = {2, D * 2};
         const uint32_t box[2] = {64, 128};
         ok = ok && tc::make_tmap(&tp.tmQt, tp.Qt, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        ok = ok && tc::make_tmap(&tp.tmOl, tp.Ol, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
     if (!ok) { cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
     tp.ready = true;
@@ -190,7 +191,7 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
         attr_done = true;
     }
     if (prof) prof->begin(st);
-    gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, p);
+    gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmOl, p);
     if (prof) prof->mark(st, "gdn_tok_prepass");
     gdn_tok_chain<D><<<tp.BH * (D / 64), kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, p);
     if (prof) prof->mark(st, "gdn_tok_chain");

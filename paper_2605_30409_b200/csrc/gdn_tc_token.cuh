@@ -109,7 +109,9 @@ __device__ __forceinline__ void inv32_columns(const float* __restrict__ Lt, int 
 template <int D, int C>
 __global__ void __launch_bounds__(kPrepassThreads, 1)
 gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                const __grid_constant__ CUtensorMap tmV, const TokParams p) {
+                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
+                const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmQt,
+                const __grid_constant__ CUtensorMap tmOl, const TokParams p) {
     constexpr int NH = kPrepassNH;
     constexpr int CW = 32 / NH;                   // columns of each 32-column chunk handled per thread
     constexpr int CH = CW / 8;                    // 16-byte bf16 chunks per thread per 32-column chunk
@@ -450,72 +452,119 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     //      column layout of both results: [0, D) from Ut, [D, 2D) from W.  For D = 128 they take 256 columns
     //      each: [N|G] -> c0,c1 and [PUt|PW] -> c2,c3.
     const float gamma_i = fast_exp(gam_i);
-    constexpr int NHALF = (C == 128) ? 1 : 2;
     constexpr uint32_t LBO2 = (D == 128) ? kBlk : 2 * kBlk;     // distance between the 64-column blocks of [Ut | W]
+    constexpr uint32_t SBLK = (uint32_t)D * 128;                 // one [D][64] bf16 or [D][32] fp32 summary block
+    const int m = (D == 128) ? row : (16 * wq + lane);           // summary row held by this thread
+    const bool m_ok = (D == 128) || (lane < 16);
+    auto issue_summary = [&](int hf) {                           // tid 0
+        tc_fence_after();
+        const uint32_t idg = umma_idesc(D, 2 * D, true, true);
+        const int s_lo = (C == 128) ? 0 : hf * 4, s_hi = (C == 128) ? KS : hf * 4 + 4;
+        const uint32_t acc = (hf == 0) ? c0 : c2;
+        for (int s = s_lo; s < s_hi; ++s)
+            umma_bf16(acc, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aA + s * 2048, LBO2), idg, s > s_lo);
+        if (hf == 0) {
+            const uint32_t idp = umma_idesc(128, 2 * D, false, true);
 #pragma unroll
-    for (int hf = 0; hf < NHALF; ++hf) {
-        if (tid == 0) {
-            tc_fence_after();
-            const uint32_t idg = umma_idesc(D, 2 * D, true, true);
-            const int s_lo = (C == 128) ? 0 : hf * 4, s_hi = (C == 128) ? KS : hf * 4 + 4;
-            for (int s = s_lo; s < s_hi; ++s)
-                umma_bf16(c0, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aA + s * 2048, LBO2), idg, s > s_lo);
-            if (hf == 0) {
-                const uint32_t idp = umma_idesc(128, 2 * D, false, true);
-#pragma unroll
-                for (int s = 0; s < KS; ++s)
-                    umma_bf16(c2, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aA + s * 2048, LBO2), idp, s > 0);
-            }
-            umma_commit(bar_mma);
+            for (int s = 0; s < KS; ++s)
+                umma_bf16(c2, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aA + s * 2048, LBO2), idp, s > 0);
         }
-        wait_mma();
-
-        GDN_STAMP(13);
-        // ---- round trip 7: write the summaries to the workspace ----------------------------------
-        const int chunk = (C == 128) ? tile : 2 * tile + hf;
-        const long long cidx = (long long)bh * p.NC + chunk;
-        const int m = (D == 128) ? row : (16 * wq + lane);          // summary row held by this thread
-        const bool m_ok = (D == 128) || (lane < 16);
+        umma_commit(bar_mma);
+    };
+    // The results leave through shared memory (the operand buffers, free once the MMAs have completed) and
+    // TMA stores: full-line writes issued by one thread instead of 32 half-used sectors per warp store.
+    //   [PUt | PW] at `acc` (lane = token row) -> Qt = gamma Q - P W in place in sQ, Ol = P Ut -> odst
+    auto stage_QO = [&](uint32_t acc, uint32_t odst) {
+#pragma unroll
+        for (int cc = 0; cc < D / 32; ++cc) {
+            float pu[CW], pw[CW];
+            tmem_ldw2(tmem_addr(acc, lane_base, cc * 32 + cb), tmem_addr(acc, lane_base, D + cc * 32 + cb), pu, pw);
+#pragma unroll
+            for (int q4 = 0; q4 < CH; ++q4) {
+                const uint32_t off = swz_chunk_off(row, cc * 4 + hh * CH + q4, kBlk);
+                float f[8];
+                unpack8(ld_shared_v4(aQ + off), f);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - pw[8 * q4 + e];
+                st_shared_v4(aQ + off, pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+                st_shared_v4(odst + off, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
+                             pack_bf16(pu[8 * q4 + 4], pu[8 * q4 + 5]), pack_bf16(pu[8 * q4 + 6], pu[8 * q4 + 7]));
+            }
+        }
+    };
+    //   [N | G] at `acc` (lane = summary row m) -> G bf16 as [D][64] blocks at gdst, N fp32 as [D][32] blocks at ndst
+    auto stage_NG = [&](uint32_t acc, uint32_t gdst, uint32_t ndst) {
 #pragma unroll
         for (int cc = 0; cc < D / 32; ++cc) {
             float nv[CW], gv[CW];
-            tmem_ldw2(tmem_addr(c0, lane_base, cc * 32 + cb), tmem_addr(c0, lane_base, D + cc * 32 + cb), nv, gv);
+            tmem_ldw2(tmem_addr(acc, lane_base, cc * 32 + cb), tmem_addr(acc, lane_base, D + cc * 32 + cb), nv, gv);
             if (m_ok) {
-                __nv_bfloat16* dg = p.Gw + (cidx * D + m) * D + cc * 32 + cb;
-#pragma unroll
-                for (int q4 = 0; q4 < CH; ++q4)
-                    st_global_v4(dg + q4 * 8, pack_bf16(gv[8 * q4], gv[8 * q4 + 1]), pack_bf16(gv[8 * q4 + 2], gv[8 * q4 + 3]),
-                                 pack_bf16(gv[8 * q4 + 4], gv[8 * q4 + 5]), pack_bf16(gv[8 * q4 + 6], gv[8 * q4 + 7]));
-                float* dn = p.Nw + (cidx * D + m) * D + cc * 32 + cb;
+                store_roww_bf16(gdst, SBLK, m, cc * 32 + cb, gv);
 #pragma unroll
                 for (int q4 = 0; q4 < CW / 4; ++q4)
-                    st_global_v4(dn + q4 * 4, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
-                                 __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
+                    st_shared_v4(ndst + cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4),
+                                 __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]), __float_as_uint(nv[4 * q4 + 2]),
+                                 __float_as_uint(nv[4 * q4 + 3]));
             }
         }
-        if (C == 128) { if (tid == 0) p.gam[cidx] = fast_exp(gam_end); }
-        else { if (tid == 64 * hf) p.gam[cidx] = fast_exp(gam_end); }
-        if (hf == 0) {
-            const long long orow = ((long long)bh * p.NT + tile) * 128 + row;
+    };
+    auto store_QO = [&](const uint8_t* odst) {                   // tid 0
+        const int r0 = (int)(((long long)bh * p.NT + tile) * 128);
 #pragma unroll
-            for (int cc = 0; cc < D / 32; ++cc) {
-                float pu[CW], pw[CW];
-                tmem_ldw2(tmem_addr(c2, lane_base, cc * 32 + cb), tmem_addr(c2, lane_base, D + cc * 32 + cb), pu, pw);
-                __nv_bfloat16* dq = p.Qt + orow * D + cc * 32 + cb;
-                __nv_bfloat16* dl = p.Ol + orow * D + cc * 32 + cb;
-#pragma unroll
-                for (int q4 = 0; q4 < CH; ++q4) {
-                    float f[8];
-                    unpack8(ld_shared_v4(aQ + swz_chunk_off(row, cc * 4 + hh * CH + q4, kBlk)), f);
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - pw[8 * q4 + e];
-                    st_global_v4(dq + q4 * 8, pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-                    st_global_v4(dl + q4 * 8, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
-                                 pack_bf16(pu[8 * q4 + 4], pu[8 * q4 + 5]), pack_bf16(pu[8 * q4 + 6], pu[8 * q4 + 7]));
-                }
-            }
+        for (int nb = 0; nb < NB; ++nb) {
+            tma_store_2d(&tmQt, sQ + nb * kBlk, nb * 64, r0);
+            tma_store_2d(&tmOl, odst + nb * kBlk, nb * 64, r0);
         }
-        if (hf + 1 < NHALF) { tc_fence_before(); __syncthreads(); }
+    };
+    auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
+        const int z = bh * p.NC + chunk;
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) tma_store_3d(&tmG, gsrc + nb * SBLK, nb * 64, 0, z);
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) tma_store_3d(&tmN, nsrc + j * SBLK, j * 32, 0, z);
+    };
+    auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
+
+    if (tid == 0) issue_summary(0);
+    wait_mma();
+    GDN_STAMP(13);
+    if (C == 128) {
+        // everything is free now: Qt in place, Ol -> sV, G -> sA, N -> sB (+ sC)
+        stage_QO(c2, aV);
+        stage_NG(c0, aA, aB);
+        if (tid == 0) p.gam[(long long)bh * p.NC + tile] = fast_exp(gam_end);
+        publish_staging();
+        if (tid == 0) {
+            store_QO(sV);
+            store_NG(sA, sB, tile);
+            tma_store_commit();
+            tma_store_wait_read();
+        }
+    } else {
+        // first half: drain [PUt | PW] (c2), send Qt / Ol off, then reuse c2 for the second chunk's [N | G]
+        stage_QO(c2, aV);
+        if (tid == 0 || tid == 64) p.gam[(long long)bh * p.NC + 2 * tile + (tid >> 6)] = fast_exp(gam_end);
+        publish_staging();
+        if (tid == 0) {
+            store_QO(sV);
+            tma_store_commit();
+            issue_summary(1);
+            if (D == 128) tma_store_wait_read();                 // sQ, sV are the staging of the second N below
+        }
+        wait_mma();
+        if (D == 128) __syncthreads();
+        // chunk 2t: G -> sC, N -> sA (+ sB);  chunk 2t+1: G -> sK, N -> sB (D = 64) or sQ + sV (D = 128)
+        const uint32_t aN1 = (D == 64) ? aB : aQ;
+        uint8_t* sN1 = (D == 64) ? sB : sQ;
+        stage_NG(c0, aC, aA);
+        stage_NG(c2, aK, aN1);
+        publish_staging();
+        if (tid == 0) {
+            store_NG(sC, sA, 2 * tile);
+            store_NG(sK, sN1, 2 * tile + 1);
+            tma_store_commit();
+            tma_store_wait_read();
+        }
     }
 
     GDN_STAMP(14);
