@@ -56,7 +56,9 @@ enum {
     GDN_FLAG_NORMALIZER = 1u,  /* also run the z path and divide (gdn_forward_chunk_norm only)          */
     GDN_FLAG_BIDIR      = 2u,  /* in-chunk reverse scan (Alg. 1 l.14-22); NOT implemented -> UNSUPPORTED */
     GDN_FLAG_LOG_ALPHA  = 4u,  /* `alpha` holds log(alpha) (<= 0) instead of alpha in (0,1]             */
-    GDN_FLAG_FORCE_SIMT = 8u   /* use the fp32 CUDA-core kernel even where a tensor-core path exists    */
+    GDN_FLAG_FORCE_SIMT = 8u,  /* use the fp32 CUDA-core kernel even where a tensor-core path exists    */
+    GDN_FLAG_UNFUSED    = 16u  /* token-wise tensor-core path as three kernels (prepass / chain / output)
+                                  instead of the single persistent kernel (C = 128 only; for A/B tests)  */
 };
 
 typedef struct {

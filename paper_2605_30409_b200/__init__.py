@@ -18,7 +18,7 @@ __all__ = [
     "GdnError", "GdnConfig", "GdnPlanInfo", "lib", "gdn_plan", "gdn_forward_chunk", "gdn_forward_chunk_norm",
     "gdn_forward_chunk_host", "gdn_destroy", "gdn_plan_get_info", "gdn_plan_set_profiling", "gdn_plan_kernel_times",
     "gdn_status_string", "gdn_last_error", "gdn_version", "GdnPlan", "GDN_BF16", "GDN_FP32", "GDN_FLAG_NORMALIZER", "GDN_FLAG_BIDIR",
-    "GDN_FLAG_LOG_ALPHA", "GDN_FLAG_FORCE_SIMT", "PATH_NAMES", "EXPORTED_SYMBOLS",
+    "GDN_FLAG_LOG_ALPHA", "GDN_FLAG_FORCE_SIMT", "GDN_FLAG_UNFUSED", "PATH_NAMES", "EXPORTED_SYMBOLS",
 ]
 
 _PKG = Path(__file__).resolve().parent
@@ -27,7 +27,7 @@ LIB_PATH = _PKG / "libgdn_b200.so"
 GDN_OK = 0
 GDN_ERR_INVALID_ARG, GDN_ERR_UNSUPPORTED, GDN_ERR_ALIGNMENT, GDN_ERR_NOMEM, GDN_ERR_ARCH, GDN_ERR_CUDA = 1, 2, 3, 4, 5, 6
 GDN_BF16, GDN_FP32 = 0, 1
-GDN_FLAG_NORMALIZER, GDN_FLAG_BIDIR, GDN_FLAG_LOG_ALPHA, GDN_FLAG_FORCE_SIMT = 1, 2, 4, 8
+GDN_FLAG_NORMALIZER, GDN_FLAG_BIDIR, GDN_FLAG_LOG_ALPHA, GDN_FLAG_FORCE_SIMT, GDN_FLAG_UNFUSED = 1, 2, 4, 8, 16
 PATH_NAMES = {0: "simt_fp32", 1: "tc_token", 2: "tc_frame"}
 EXPORTED_SYMBOLS = [
     "gdn_plan", "gdn_forward_chunk", "gdn_forward_chunk_norm", "gdn_forward_chunk_host", "gdn_destroy",

@@ -163,7 +163,7 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
     if (c.T % c.group != 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "T must be a multiple of group");
     if (c.io_dtype != GDN_BF16 && c.io_dtype != GDN_FP32) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown io_dtype");
     if (!(c.chunk == 0 || c.chunk == 64 || c.chunk == 128)) return fail(nullptr, GDN_ERR_INVALID_ARG, "chunk must be 0, 64 or 128");
-    const uint32_t known = GDN_FLAG_NORMALIZER | GDN_FLAG_BIDIR | GDN_FLAG_LOG_ALPHA | GDN_FLAG_FORCE_SIMT;
+    const uint32_t known = GDN_FLAG_NORMALIZER | GDN_FLAG_BIDIR | GDN_FLAG_LOG_ALPHA | GDN_FLAG_FORCE_SIMT | GDN_FLAG_UNFUSED;
     if (c.flags & ~known) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown flag bits");
     if (!head_dim_ok(c.d_k) || !head_dim_ok(c.d_v))
         return fail(nullptr, GDN_ERR_UNSUPPORTED, "d_k and d_v must each be 32, 64 or 128 (112 via padding is not implemented)");

@@ -4,12 +4,14 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <string>
 
 #include "../../include/gdn.h"
 #include "gdn_profile.cuh"
 #include "gdn_tc_token.cuh"
 #include "gdn_tc_frame.cuh"
+#include "gdn_tc_fused.cuh"
 #include "tc_tmap.cuh"
 
 namespace gdn {
@@ -27,8 +29,13 @@ struct TcPlan {
     float *Nw = nullptr, *gam = nullptr, *part = nullptr;
     CUtensorMap tmG, tmN, tmQt, tmOl, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
     // per-call activation maps, cached on the pointers they were built for
-    const void *cq = nullptr, *ck = nullptr, *cv = nullptr;
-    CUtensorMap tmQ, tmK, tmV;
+    const void *cq = nullptr, *ck = nullptr, *cv = nullptr, *co = nullptr;
+    CUtensorMap tmQ, tmK, tmV, tmO;
+    // fused single-kernel token path (C = 128): per-tile ready flags and the call epoch
+    bool fused = false;
+    unsigned int* flags = nullptr;
+    unsigned int epoch = 0;
+    int HPR = 0, NWC = 0, grid = 0;
 };
 
 inline int tc_default_chunk(const gdn_config_t& c) { return c.chunk ? c.chunk : 128; }
@@ -45,7 +52,7 @@ inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, in
     }
     *path = GDN_PATH_TC_TOKEN;
     *chunk = tc_default_chunk(c);
-    *launches = 3;
+    *launches = (*chunk == 128 && !(c.flags & GDN_FLAG_UNFUSED)) ? 1 : 3;
     return true;
 }
 
@@ -122,7 +129,26 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
     const size_t oG = carve(BH * NC * D * D * 2), oN = carve(BH * NC * D * D * 4), oGam = carve(BH * NC * 4);
-    const size_t oQt = carve(BH * NT * 128 * D * 2), oOl = carve(BH * NT * 128 * D * 2), oSc = carve(BH * NC * D * D * 2);
+    const size_t oQt = carve(BH * NT * 128 * D * 2), oOl = carve(BH * NT * 128 * D * 2);
+    tp.fused = tp.C == 128 && !(c.flags & GDN_FLAG_UNFUSED);
+    const size_t oSc = tp.fused ? 0 : carve(BH * NC * D * D * 2);
+    const size_t oFl = tp.fused ? carve(BH * NT * 4) : 0;
+    if (tp.fused) {
+        // role split: chain workers own (head, 64-column tile) units; heads are processed in groups of HPR
+        const int sms = sm_count > 0 ? sm_count : 148, nct = tp.D / 64;
+        int hpr = tp.BH;
+        if (tp.BH * nct > sms / 3) hpr = (sms / 5) / nct;
+        if (const char* e = getenv("GDN_FUSED_HPR")) { const int v = atoi(e); if (v > 0) hpr = v; }
+        if (hpr < 1) hpr = 1;
+        if (hpr > tp.BH) hpr = tp.BH;
+        if (hpr * nct > sms - 1) hpr = (sms - 1) / nct > 0 ? (sms - 1) / nct : 1;
+        tp.HPR = hpr;
+        tp.NWC = hpr * nct;
+        long long nwp = (long long)sms - tp.NWC;
+        if (nwp > (long long)BH * NT) nwp = (long long)BH * NT;
+        if (nwp < 1) nwp = 1;
+        tp.grid = tp.NWC + (int)nwp;
+    }
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -136,6 +162,14 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     tp.Qt = reinterpret_cast<__nv_bfloat16*>(w + oQt);
     tp.Ol = reinterpret_cast<__nv_bfloat16*>(w + oOl);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
+    if (tp.fused) {
+        tp.flags = reinterpret_cast<unsigned int*>(w + oFl);
+        if (cudaMemset(tp.flags, 0, BH * NT * 4) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
+            if (err) *err = "flag initialisation failed";
+            return GDN_ERR_CUDA;
+        }
+    }
     bool ok = true;
     {   // G_c: bf16 (D, D, BH*NC), box {64, D, 1}
         const uint64_t dims[3] = {D, D, BH * NC}, str[3] = {2, D * 2, D * D * 2};
@@ -179,7 +213,7 @@ template <int D, int C>
 inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
     using namespace tok;
     constexpr int NB = D / 64;
-    const size_t smem1 = 3 * NB * kBlk + 6 * kBlk + 4096 + 1024;   // + 18 KB static (sL)
+    const size_t smem1 = prepass_smem_bytes<D>() + 1024;
     const size_t smem2 = ChainSmem<D>::TOTAL;
     const size_t smem3 = NB * kBlk + (C == 128 ? 1 : 2) * D * D * 2 + 256 + 1024;
     static bool attr_done = false;
@@ -197,6 +231,26 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
     if (prof) prof->mark(st, "gdn_tok_chain");
     gdn_tok_output<D, C><<<tp.BH * tp.NT, 128, smem3, st>>>(tp.tmQt, tp.tmSc, p);
     if (prof) prof->mark(st, "gdn_tok_output");
+    return cudaGetLastError();
+}
+
+template <int D>
+inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
+    const size_t smem = fused::fused_smem_bytes<D>();
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = set_smem(fused::gdn_tok_fused<D>, smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    FusedParams fp{};
+    fp.t = p;
+    fp.flags = tp.flags;
+    fp.epoch = ++tp.epoch;
+    fp.NWC = tp.NWC; fp.HPR = tp.HPR; fp.total_tiles = tp.BH * tp.NT;
+    if (prof) prof->begin(st);
+    fused::gdn_tok_fused<D><<<tp.grid, fused::kThreads, smem, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmQt, tp.tmO, fp);
+    if (prof) prof->mark(st, "gdn_tok_fused");
     return cudaGetLastError();
 }
 
@@ -240,6 +294,10 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
     }
+    if (tp.fused && out != tp.co) {
+        if (!tc::make_act_tmap(&tp.tmO, out, c.B, c.T, c.H, c.d_v, c.T, ts(c.o_token_stride, c.d_v), 128, err)) { tp.co = nullptr; return GDN_ERR_CUDA; }
+        tp.co = out;
+    }
     if (tp.mode == GDN_PATH_TC_FRAME) {
         FrmParams fp{};
         fp.alpha = alpha; fp.beta = beta; fp.out = out; fp.part = tp.part; fp.Gw = tp.Gw; fp.Nw = tp.Nw; fp.gam = tp.gam;
@@ -268,7 +326,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.dbg = dbg_dev;
 #endif
     cudaError_t e;
-    if (tp.D == 64) e = (tp.C == 128) ? tc_launch_token<64, 128>(tp, p, st, prof) : tc_launch_token<64, 64>(tp, p, st, prof);
+    if (tp.fused) e = (tp.D == 64) ? tc_launch_fused<64>(tp, p, st, prof) : tc_launch_fused<128>(tp, p, st, prof);
+    else if (tp.D == 64) e = (tp.C == 128) ? tc_launch_token<64, 128>(tp, p, st, prof) : tc_launch_token<64, 64>(tp, p, st, prof);
     else            e = (tp.C == 128) ? tc_launch_token<128, 128>(tp, p, st, prof) : tc_launch_token<128, 64>(tp, p, st, prof);
     if (e != cudaSuccess) { if (err) *err = std::string("token tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
 #ifdef GDN_PHASE_TIMING

@@ -106,12 +106,48 @@ __device__ __forceinline__ void inv32_columns(const float* __restrict__ Lt, int 
     inv32_steps<0>(Lt, la, lb, x);
 }
 
-template <int D, int C>
-__global__ void __launch_bounds__(kPrepassThreads, 1)
-gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
-                const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmQt,
-                const __grid_constant__ CUtensorMap tmOl, const TokParams p) {
+// Shared-memory carve-up and barriers of one prepass CTA (set up once; a persistent CTA runs many tiles).
+struct PrepassCtx {
+    uint8_t *sK, *sQ, *sV, *sA, *sB, *sC;
+    float *sGam, *sBeta, *sBG, *sCF, *sWarp, *sL;
+    uint64_t *bar_kq, *bar_v, *bar_mma;
+    uint32_t tmem;                                // 512 TMEM columns
+};
+template <int D>
+constexpr uint32_t prepass_smem_bytes() { return 3u * (D / 64) * kBlk + 6u * kBlk + 4u * 32 * kLsStride * 4 + 4096u; }
+
+template <int D>
+__device__ __forceinline__ void prepass_carve(uint8_t* smem, PrepassCtx& cx, uint32_t** tmem_slot) {
+    constexpr uint32_t TILE = (D / 64) * kBlk;
+    cx.sK = smem;
+    cx.sQ = smem + TILE;
+    cx.sV = smem + 2 * TILE;
+    cx.sA = smem + 3 * TILE;                      // L_off -> Tm diag(beta gamma) -> Ut
+    cx.sB = cx.sA + 2 * kBlk;                     // D (block-diagonal inverse) -> W      (sB directly follows sA)
+    cx.sC = cx.sB + 2 * kBlk;                     // X -> Tm diag(beta) -> P
+    cx.sL = reinterpret_cast<float*>(cx.sC + 2 * kBlk);        // diagonal 32x32 blocks of L^T (fp32), then of the inverse
+    cx.sGam = cx.sL + 4 * 32 * kLsStride;         // [128] Gam_i (segmented for C = 64)
+    cx.sBeta = cx.sGam + 128;                     // [128] beta_j
+    cx.sBG = cx.sBeta + 128;                      // [128] beta_j e^{Gam_j}
+    cx.sCF = cx.sBG + 128;                        // [128] e^{Gam_ref(j) - Gam_j}, ref = last row of j's 32-chunk
+    cx.sWarp = cx.sCF + 128;                      // [4] per-warp sums of log alpha
+    uint64_t* bars = reinterpret_cast<uint64_t*>(cx.sWarp + 4);
+    cx.bar_kq = &bars[0]; cx.bar_v = &bars[1]; cx.bar_mma = &bars[2];
+    *tmem_slot = reinterpret_cast<uint32_t*>(bars + 3);
+}
+
+// One 128-token tile of one (b,h) stream.  `it` = how many tiles this CTA has run before (barrier parity),
+// `ph` = running parity of bar_mma.  FUSED = false: summaries in the layouts of the three-kernel path
+// (N row-major fp32 [D][D], Ol row-major [rows][D]), the call returns after the stores have read their
+// staging.  FUSED = true (gdn_tc_fused.cuh, C = 128): N and Ol leave in "chunk-major" layouts
+// ([16-byte chunk][row]) that the chain workers read with coalesced loads, and the caller publishes the
+// tile's ready flag once the stores have completed.
+template <int D, int C, bool FUSED>
+__device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtensorMap* tmQ, const CUtensorMap* tmK,
+                                             const CUtensorMap* tmV, const CUtensorMap* tmG, const CUtensorMap* tmN,
+                                             const CUtensorMap* tmQt, const CUtensorMap* tmOl, const TokParams& p,
+                                             int bh, int tile, uint32_t it, uint32_t& ph) {
+    static_assert(!FUSED || C == 128, "the fused path runs C = 128");
     constexpr int NH = kPrepassNH;
     constexpr int CW = 32 / NH;                   // columns of each 32-column chunk handled per thread
     constexpr int CH = CW / 8;                    // 16-byte bf16 chunks per thread per 32-column chunk
@@ -119,34 +155,18 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     constexpr uint32_t TILE = NB * kBlk;
     constexpr int KS = 8;                         // K = 16 steps over the 128 tokens of a tile
     constexpr int DS = D / 16;                    // K = 16 steps over the head dim
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint8_t* sK = smem;
-    uint8_t* sQ = smem + TILE;
-    uint8_t* sV = smem + 2 * TILE;
-    uint8_t* sA = smem + 3 * TILE;                // L_off -> Tm diag(beta gamma) -> Ut
-    uint8_t* sB = sA + 2 * kBlk;                  // D (block-diagonal inverse) -> W      (sB directly follows sA)
-    uint8_t* sC = sB + 2 * kBlk;                  // X -> Tm diag(beta) -> P
-    float* sGam = reinterpret_cast<float*>(sC + 2 * kBlk);     // [128] Gam_i (segmented for C = 64)
-    float* sBeta = sGam + 128;                                 // [128] beta_j
-    float* sBG = sBeta + 128;                                  // [128] beta_j e^{Gam_j}
-    float* sCF = sBG + 128;                                    // [128] e^{Gam_ref(j) - Gam_j}, ref = last row of j's 32-chunk
-    float* sWarp = sCF + 128;                                  // [4] per-warp sums of log alpha
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sWarp + 4);   // [3]
-    __shared__ __align__(16) float sL[4 * 32 * kLsStride];     // diagonal 32x32 blocks of L^T (fp32), then of the inverse
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3);
+    uint8_t *sK = cx.sK, *sQ = cx.sQ, *sV = cx.sV, *sA = cx.sA, *sB = cx.sB, *sC = cx.sC;
+    float *sGam = cx.sGam, *sBeta = cx.sBeta, *sBG = cx.sBG, *sCF = cx.sCF, *sWarp = cx.sWarp, *sL = cx.sL;
+    uint64_t *bar_kq = cx.bar_kq, *bar_v = cx.bar_v, *bar_mma = cx.bar_mma;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wq = warp & 3, hh = warp >> 2;
     const int row = wq * 32 + lane;               // token row == TMEM lane
     const int cb = hh * CW;                       // this thread's columns inside every 32-column chunk
     const uint32_t lane_base = (uint32_t)(wq * 32);
-    const int tile = blockIdx.x % p.NT, bh = blockIdx.x / p.NT;
     const int b = bh / p.H, h = bh % p.H;
-    uint64_t* bar_kq = &bars[0];
-    uint64_t* bar_v = &bars[1];
-    uint64_t* bar_mma = &bars[2];
     const uint32_t aA = smem_u32(sA), aB = smem_u32(sB), aC = smem_u32(sC), aK = smem_u32(sK), aQ = smem_u32(sQ), aV = smem_u32(sV);
+    const uint32_t par = it & 1u;
 
     GDN_STAMP(0);
     // gates first: their global-load latency overlaps the barrier / TMEM / TMA set-up
@@ -159,19 +179,16 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         g = 1.f;
     }
     if (tid == 0) {
-        mbar_init(bar_kq, 1); mbar_init(bar_v, 1); mbar_init(bar_mma, 1);
-        mbar_fence_init();
         mbar_expect_tx(bar_kq, 2 * TILE);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
-            tma_load_5d(sK + nb * kBlk, &tmK, bar_kq, nb * 64, h, tile * 128, 0, b);
-            tma_load_5d(sQ + nb * kBlk, &tmQ, bar_kq, nb * 64, h, tile * 128, 0, b);
+            tma_load_5d(sK + nb * kBlk, tmK, bar_kq, nb * 64, h, tile * 128, 0, b);
+            tma_load_5d(sQ + nb * kBlk, tmQ, bar_kq, nb * 64, h, tile * 128, 0, b);
         }
         mbar_expect_tx(bar_v, TILE);
 #pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, &tmV, bar_v, nb * 64, h, tile * 128, 0, b);
+        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, tmV, bar_v, nb * 64, h, tile * 128, 0, b);
     }
-    if (warp == 0) tmem_alloc(tmem_slot, 512);
     // zero this thread's columns of the three 128x128 operand buffers
 #pragma unroll
     for (int cc = 0; cc < 4; ++cc) {
@@ -194,10 +211,8 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (lane >= o) x += y;
     }
     if (hh == 0 && lane == 31) sWarp[wq] = x;
-    tc_fence_before();
     __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = *tmem_slot;
+    const uint32_t tmem = cx.tmem;
     const uint32_t c0 = tmem, c1 = tmem + 128, c2 = tmem + 256, c3 = tmem + 384;
     float gam_i, gam_end;            // Gam_i and Gam at the end of this row's chunk
     {
@@ -224,13 +239,12 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) rf[cc] = (cc < wq && cc >= half_lo) ? fast_exp(gam_i - sGam[cc * 32 + 31]) : 0.f;
 
-    uint32_t ph = 0;
     auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
 
     GDN_STAMP(2);
     // ---- T1: K K^T -> c0, Q K^T -> c1 ------------------------------------------------------------
-    mbar_wait(bar_kq, 0);
+    mbar_wait(bar_kq, par);
     GDN_STAMP(3);
     if (tid == 0) {
         tc_fence_after();
@@ -388,7 +402,7 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     GDN_STAMP(9);
     // ---- T7: W = Tm diag(beta gamma) K -> c2,  Ut = Tm diag(beta) V -> c3 ---------------------------
-    mbar_wait(bar_v, 0);
+    mbar_wait(bar_v, par);
     GDN_STAMP(10);
     if (tid == 0) {
         tc_fence_after();
@@ -487,7 +501,8 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                 for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - pw[8 * q4 + e];
                 st_shared_v4(aQ + off, pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-                st_shared_v4(odst + off, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
+                const uint32_t ooff = FUSED ? (uint32_t)(((cc * 4 + hh * CH + q4) * 128 + row) * 16) : off;   // chunk-major
+                st_shared_v4(odst + ooff, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
                              pack_bf16(pu[8 * q4 + 4], pu[8 * q4 + 5]), pack_bf16(pu[8 * q4 + 6], pu[8 * q4 + 7]));
             }
         }
@@ -501,10 +516,12 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (m_ok) {
                 store_roww_bf16(gdst, SBLK, m, cc * 32 + cb, gv);
 #pragma unroll
-                for (int q4 = 0; q4 < CW / 4; ++q4)
-                    st_shared_v4(ndst + cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4),
-                                 __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]), __float_as_uint(nv[4 * q4 + 2]),
-                                 __float_as_uint(nv[4 * q4 + 3]));
+                for (int q4 = 0; q4 < CW / 4; ++q4) {
+                    const uint32_t noff = FUSED ? (uint32_t)((((cc * 32 + cb) / 4 + q4) * D + m) * 16)                       // chunk-major
+                                                : cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4);
+                    st_shared_v4(ndst + noff, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
+                                 __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
+                }
             }
         }
     };
@@ -512,16 +529,23 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int r0 = (int)(((long long)bh * p.NT + tile) * 128);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
-            tma_store_2d(&tmQt, sQ + nb * kBlk, nb * 64, r0);
-            tma_store_2d(&tmOl, odst + nb * kBlk, nb * 64, r0);
+            tma_store_2d(tmQt, sQ + nb * kBlk, nb * 64, r0);
+            if (!FUSED) tma_store_2d(tmOl, odst + nb * kBlk, nb * 64, r0);
+        }
+        if (FUSED) {
+#pragma unroll
+            for (int nb = 0; nb < NB; ++nb) bulk_store(p.Ol + (long long)r0 * D + nb * (kBlk / 2), odst + nb * kBlk, kBlk);
         }
     };
     auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
         const int z = bh * p.NC + chunk;
 #pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_store_3d(&tmG, gsrc + nb * SBLK, nb * 64, 0, z);
+        for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
 #pragma unroll
-        for (int j = 0; j < D / 32; ++j) tma_store_3d(&tmN, nsrc + j * SBLK, j * 32, 0, z);
+        for (int j = 0; j < D / 32; ++j) {
+            if (FUSED) bulk_store(p.Nw + (long long)z * D * D + j * (SBLK / 4), nsrc + j * SBLK, SBLK);
+            else tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
+        }
     };
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
 
@@ -568,9 +592,34 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     }
 
     GDN_STAMP(14);
+    if (FUSED) __syncthreads();        // the staging buffers are the next tile's operand buffers
+}
+
+template <int D, int C>
+__global__ void __launch_bounds__(kPrepassThreads, 1)
+gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
+                const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmQt,
+                const __grid_constant__ CUtensorMap tmOl, const TokParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    PrepassCtx cx;
+    uint32_t* tmem_slot;
+    prepass_carve<D>(smem, cx, &tmem_slot);
+    if (threadIdx.x == 0) {
+        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
+        mbar_fence_init();
+    }
+    if (threadIdx.x < 32) tmem_alloc(tmem_slot, 512);
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, 512);
+    tc_fence_after();
+    cx.tmem = *tmem_slot;
+    uint32_t ph = 0;
+    prepass_tile<D, C, false>(cx, &tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmOl, p, blockIdx.x / p.NT, blockIdx.x % p.NT, 0u, ph);
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x < 32) tmem_dealloc(cx.tmem, 512);
     GDN_STAMP(15);
 }
 
