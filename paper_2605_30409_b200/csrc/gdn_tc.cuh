@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <string>
+#include <vector>
 
 #include "../../include/gdn.h"
 #include "gdn_profile.cuh"
@@ -134,10 +135,20 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     const size_t oSc = tp.fused ? 0 : carve(BH * NC * D * D * 2);
     const size_t oFl = tp.fused ? carve(BH * NT * 4) : 0;
     if (tp.fused) {
-        // role split: chain workers own (head, 64-column tile) units; heads are processed in groups of HPR
+        // role split: chain workers own (head, 64-column tile) units; heads are processed in groups of HPR.
+        // HPR minimises a two-term estimate: the prepass workers (all SMs but the chain workers) need
+        // ceil(tiles / workers) tile times, the chain workers need groups * NT serial steps.
         const int sms = sm_count > 0 ? sm_count : 148, nct = tp.D / 64;
-        int hpr = tp.BH;
-        if (tp.BH * nct > sms / 3) hpr = (sms / 5) / nct;
+        const double t_tile = tp.D == 128 ? 14.0 : 10.0, t_step = tp.D == 128 ? 2.2 : 1.3;     // microseconds, measured (a chain that trails the prepass pays the TMA latency of its shallow ring every step)
+        int hpr = 1;
+        double best = 1e30;
+        for (int h = 1; h <= tp.BH && h * nct < sms; ++h) {
+            const int nwp = sms - h * nct, groups = (tp.BH + h - 1) / h;
+            const double t_pre = (double)(((long long)BH * NT + nwp - 1) / nwp) * t_tile;
+            const double t_chain = (double)groups * NT * t_step;
+            const double est = (t_pre > t_chain ? t_pre : t_chain) + 0.02 * groups;
+            if (est < best - 1e-9) { best = est; hpr = h; }
+        }
         if (const char* e = getenv("GDN_FUSED_HPR")) { const int v = atoi(e); if (v > 0) hpr = v; }
         if (hpr < 1) hpr = 1;
         if (hpr > tp.BH) hpr = tp.BH;
@@ -249,7 +260,7 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
     fp.epoch = ++tp.epoch;
     fp.NWC = tp.NWC; fp.HPR = tp.HPR; fp.total_tiles = tp.BH * tp.NT;
     if (prof) prof->begin(st);
-    fused::gdn_tok_fused<D><<<tp.grid, fused::kThreads, smem, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmQt, tp.tmO, fp);
+    fused::gdn_tok_fused<D><<<tp.grid, fused::kThreads, smem, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmO, fp);
     if (prof) prof->mark(st, "gdn_tok_fused");
     return cudaGetLastError();
 }
@@ -322,7 +333,9 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.dbg = nullptr;
 #ifdef GDN_PHASE_TIMING
     static long long* dbg_dev = nullptr;
-    if (!dbg_dev) { cudaMalloc(&dbg_dev, 64 * sizeof(long long)); cudaMemset(dbg_dev, 0, 64 * sizeof(long long)); }
+    constexpr size_t kDbgWords = 64 + 160 * 128;      // 64 phase stamps + 128 trace slots per CTA
+    if (!dbg_dev) cudaMalloc(&dbg_dev, kDbgWords * sizeof(long long));
+    cudaMemsetAsync(dbg_dev, 0, kDbgWords * sizeof(long long), st);
     p.dbg = dbg_dev;
 #endif
     cudaError_t e;
@@ -341,6 +354,22 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fprintf(stderr, " total:%lld\n", hst[15] - hst[0]);
         fprintf(stderr, "[gdn chain step cycles] snapshot:%lld premath:%lld wait_mma:%lld ld+sub:%lld publish:%lld fence+sync:%lld total:%lld\n",
                 hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36], hst[38] - hst[37], hst[38] - hst[32]);
+        fprintf(stderr, "[gdn fused chain step 12] prev-publish->top:%lld gfull+gam:%lld Nfma:%lld wait_mma:%lld ld+sub:%lld publish:%lld | mma warp: sready-seen@%lld commit@%lld (rel. to top) state-mma-done@%lld\n",
+                hst[32] - hst[31], hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36],
+                hst[41] - hst[32], hst[42] - hst[32], hst[35] - hst[32]);
+        if (const char* tf = getenv("GDN_TRACE_FILE")) {      // fused kernel: per-CTA globaltimer trace
+            std::vector<long long> tr(kDbgWords);
+            cudaMemcpy(tr.data(), p.dbg, kDbgWords * sizeof(long long), cudaMemcpyDeviceToHost);
+            if (FILE* f = fopen(tf, "w")) {
+                fprintf(f, "grid %d nwc %d\n", tp.grid, tp.NWC);
+                for (int cta = 0; cta < tp.grid && cta < 160; ++cta) {
+                    fprintf(f, "%d", cta);
+                    for (int i = 0; i < 128; ++i) fprintf(f, " %lld", tr[64 + (size_t)cta * 128 + i]);
+                    fprintf(f, "\n");
+                }
+                fclose(f);
+            }
+        }
     }
 #endif
     return GDN_OK;

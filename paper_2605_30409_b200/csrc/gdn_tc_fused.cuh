@@ -49,18 +49,30 @@ __device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) 
 // orders async-proxy accesses (TMA) of any state space with this thread's generic-proxy accesses
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
+#ifdef GDN_PHASE_TIMING
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+// developer trace: 128 slots per CTA behind the 64 phase stamps
+#define GDN_TRACE(slot) do { if (fp.t.dbg && (slot) < 128) fp.t.dbg[64 + (long long)blockIdx.x * 128 + (slot)] = gtime(); } while (0)
+#else
+#define GDN_TRACE(slot) do { } while (0)
+#endif
+
 template <int D>
 struct ChainSmem {
     static constexpr int NB = D / 64;
     static constexpr uint32_t G_BYTES = (uint32_t)D * D * 2;          // NB blocks of [D][64] bf16
-    static constexpr uint32_t Q_BYTES = 128u * D * 2;                 // NB blocks of [128][64] bf16
+    static constexpr uint32_t N_BYTES = (uint32_t)D * 64 * 4;         // 2 blocks of [D][32] fp32 (this CTA's 64 state columns)
+    static constexpr uint32_t GN_BYTES = G_BYTES + N_BYTES;
+    static constexpr uint32_t Q_BYTES = 128u * D * 2;                 // NB blocks of [128][64] bf16; block 0 then stages the out tile
     static constexpr uint32_t S_BYTES = (uint32_t)D * 128;            // [D][64] bf16
-    static constexpr int GST = (D == 128) ? 3 : 4;
-    static constexpr int QST = (D == 128) ? 3 : 4;
-    static constexpr uint32_t OFF_Q = GST * G_BYTES;
+    static constexpr int GST = (D == 128) ? 2 : 3;
+    static constexpr int QST = (D == 128) ? 2 : 3;
+    static constexpr int NSB = (D == 128) ? 2 : 3;                    // bf16 state operand buffers
+    static constexpr uint32_t OFF_Q = GST * GN_BYTES;
     static constexpr uint32_t OFF_S = OFF_Q + QST * Q_BYTES;
-    static constexpr uint32_t OFF_BAR = OFF_S + 2 * S_BYTES;
-    static constexpr uint32_t TOTAL = OFF_BAR + 256;
+    static constexpr uint32_t OFF_BAR = OFF_S + NSB * S_BYTES;
+    static constexpr uint32_t OFF_GAM = OFF_BAR + 384;                // [GST] gamma_c of the chunk in the stage
+    static constexpr uint32_t TOTAL = OFF_BAR + 512;
 };
 
 template <int D>
@@ -70,34 +82,38 @@ constexpr uint32_t fused_smem_bytes() {
 
 // ---------------------------------------------------------------------------------------------------
 // chain worker.  warps 0-7: state rows (thread = row m x 32 columns); 8-11: output epilogue (thread = token
-// row); 12: MMA issuer; 13: flag poller + TMA producer; 14-15: idle.
+// row); 12: MMA issuer (chain first, output behind it); 13: flag poller + TMA producer; 14-15: idle.
+// The chain (warps 0-7) and the output (warps 8-11) only meet at the bf16 state operand buffers: the output
+// of chunk c reads S_c while the chain is already up to NSB - 1 steps further on.
 // ---------------------------------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG, const CUtensorMap* tmQt,
+__device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG, const CUtensorMap* tmN, const CUtensorMap* tmQt,
                                            const CUtensorMap* tmO, const FusedParams& fp) {
     using L = ChainSmem<D>;
-    constexpr int NB = L::NB, GST = L::GST, QST = L::QST, NCT = D / 64;
+    constexpr int NB = L::NB, GST = L::GST, QST = L::QST, NSB = L::NSB, NCT = D / 64;
     const TokParams& p = fp.t;
     uint8_t* sG = smem;
     uint8_t* sQ = smem + L::OFF_Q;
     uint8_t* sS = smem + L::OFF_S;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::OFF_BAR);
-    uint64_t* g_full = bars;                  // [GST] TMA: G_c landed
-    uint64_t* g_empty = g_full + GST;         // [GST] chain MMA of the step has completed
+    uint64_t* g_full = bars;                  // [GST] TMA: G_c and N_c landed (gamma_c written before the arm)
+    uint64_t* g_empty = g_full + GST;         // [GST] chain MMA of the step has completed and the 8 state warps have read gamma_c, N_c
     uint64_t* q_full = g_empty + GST;         // [QST] TMA: Qt tile landed
     uint64_t* q_empty = q_full + QST;         // [QST] the out tile staged in the buffer has left
-    uint64_t* mma_chain = q_empty + QST;      // chain MMA complete
-    uint64_t* s_ready = mma_chain + 1;        // bf16 state operand published (8 warps)
-    uint64_t* out_full = s_ready + 1;         // [2] output MMA complete
+    uint64_t* s_ready = q_empty + QST;        // [NSB] bf16 state operand published (8 warps)
+    uint64_t* s_free = s_ready + NSB;         // [NSB] the output MMA that read the buffer has completed
+    uint64_t* mma_chain = s_free + NSB;       // chain MMA complete
+    uint64_t* out_full = mma_chain + 1;       // [2] output MMA complete
     uint64_t* out_free = out_full + 2;        // [2] output accumulator drained (4 warps)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(out_free + 2);
+    float* sGamma = reinterpret_cast<float*>(smem + L::OFF_GAM);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        for (int s = 0; s < GST; ++s) { mbar_init(&g_full[s], 1); mbar_init(&g_empty[s], 1); }
+        for (int s = 0; s < GST; ++s) { mbar_init(&g_full[s], 1); mbar_init(&g_empty[s], 9); }
         for (int s = 0; s < QST; ++s) { mbar_init(&q_full[s], 1); mbar_init(&q_empty[s], 1); }
+        for (int s = 0; s < NSB; ++s) { mbar_init(&s_ready[s], 8); mbar_init(&s_free[s], 1); }
         mbar_init(mma_chain, 1);
-        mbar_init(s_ready, 8);
         for (int s = 0; s < 2; ++s) { mbar_init(&out_full[s], 1); mbar_init(&out_free[s], 4); }
         mbar_fence_init();
     }
@@ -112,60 +128,100 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
 
     if (warp == 13) {
         // ===== flag poller + TMA producer =====
-        if (lane == 0) {
-            uint32_t gs = 0;
-            for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
-                const int bh = u / NCT;
-                for (int c = 0; c < NT; ++c, ++gs) {
-                    const unsigned int* f = fp.flags + (long long)bh * NT + c;
-                    while (ld_acquire_gpu(f) < fp.epoch) __nanosleep(64);
+        // The 32 lanes poll the flags of the next 32 chunks together (one L2 round trip for all of them);
+        // lane 0 issues the loads of every chunk in the ready prefix.
+        uint32_t gs = 0;
+        for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
+            const int bh = u / NCT, ct = u % NCT;
+            int ready = 0, base = 0;                         // chunks [0, ready) of this unit are published
+            float gam_l = 0.f;                               // gamma of chunk base + lane (valid below `ready`)
+            for (int c = 0; c < NT; ++c, ++gs) {
+                while (c >= ready) {
+                    base = ready;
+                    const int idx = base + lane;
+                    const bool ok = idx < NT && ld_acquire_gpu(fp.flags + (long long)bh * NT + idx) >= fp.epoch;
+                    const uint32_t m = __ballot_sync(0xffffffffu, ok);
+                    ready += (m == 0xffffffffu) ? 32 : (__ffs(~m) - 1);      // length of the ready prefix
+                    if (idx < ready) {                       // accepted exactly once per chunk
+                        gam_l = __ldcg(p.gam + (long long)bh * p.NC + idx);
+                        if (GST < 3) {                       // shallow ring: have the summaries waiting in L2
+                            fence_proxy_async_all();
+                            const int z = bh * p.NC + idx;
+#pragma unroll
+                            for (int nb = 0; nb < NB; ++nb) tma_prefetch_3d(tmG, nb * 64, 0, z);
+                            tma_prefetch_3d(tmN, ct * 64, 0, z);
+                            tma_prefetch_3d(tmN, ct * 64 + 32, 0, z);
+                        }
+                    }
+                    if (c >= ready) __nanosleep(32);
+                }
+                const float gam_c = __shfl_sync(0xffffffffu, gam_l, c - base);
+                if (lane == 0) {
+                    GDN_TRACE(2 * gs);
                     fence_proxy_async_all();
                     const int gst = gs % GST, qst = gs % QST;
                     if (gs >= (uint32_t)GST) mbar_wait(&g_empty[gst], ((gs / GST) - 1) & 1u);
-                    mbar_expect_tx(&g_full[gst], L::G_BYTES);
+                    sGamma[gst] = gam_c;                     // visible to the waiters of g_full through the arrive below
+                    mbar_expect_tx(&g_full[gst], L::GN_BYTES);
+                    uint8_t* gb = sG + gst * L::GN_BYTES;
+                    const int z = bh * p.NC + c;
 #pragma unroll
-                    for (int nb = 0; nb < NB; ++nb)
-                        tma_load_3d(sG + gst * L::G_BYTES + nb * (D * 128), tmG, &g_full[gst], nb * 64, 0, bh * p.NC + c);
+                    for (int nb = 0; nb < NB; ++nb) tma_load_3d(gb + nb * (D * 128), tmG, &g_full[gst], nb * 64, 0, z);
+                    tma_load_3d(gb + L::G_BYTES, tmN, &g_full[gst], ct * 64, 0, z);
+                    tma_load_3d(gb + L::G_BYTES + D * 128, tmN, &g_full[gst], ct * 64 + 32, 0, z);
                     if (gs >= (uint32_t)QST) mbar_wait(&q_empty[qst], ((gs / QST) - 1) & 1u);
                     mbar_expect_tx(&q_full[qst], L::Q_BYTES);
+                    uint8_t* qb = sQ + qst * L::Q_BYTES;
 #pragma unroll
-                    for (int nb = 0; nb < NB; ++nb)
-                        tma_load_2d(sQ + qst * L::Q_BYTES + nb * kBlk, tmQt, &q_full[qst], nb * 64, (bh * NT + c) * 128);
+                    for (int nb = 0; nb < NB; ++nb) tma_load_2d(qb + nb * kBlk, tmQt, &q_full[qst], nb * 64, (bh * NT + c) * 128);
                 }
+                __syncwarp();
             }
         }
     } else if (warp == 12) {
-        // ===== MMA issuer =====
+        // ===== MMA issuer.  chain: acc = G_c (A, K-major) * S_c (B, MN-major); output: acc_out = Qt_c (A) * S_c.
+        // The chain MMA of a step goes out the moment its operand is published; output MMAs follow in the
+        // shadow of the chain's TMEM -> register -> shared-memory round trip and may lag by up to NSB - 1 steps.
         if (lane == 0) {
             const uint32_t idc = umma_idesc(D, 64, false, true);
             const uint32_t ido = umma_idesc(128, 64, false, true);
-            uint32_t gs = 0;
-            for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
-                for (int c = 0; c < NT; ++c, ++gs) {
-                    const int gst = gs % GST, qst = gs % QST;
-                    const uint32_t aS = smem_u32(sS + (gs & 1) * L::S_BYTES);
-                    // chain: acc = G_c (A, K-major) * S_c (B, MN-major)
-                    mbar_wait(&g_full[gst], (gs / GST) & 1u);
-                    mbar_wait(s_ready, gs & 1u);
-                    tc_fence_after();
-                    const uint32_t aG = smem_u32(sG + gst * L::G_BYTES);
+            const uint32_t total = (uint32_t)((nunits - (int)blockIdx.x + fp.NWC - 1) / fp.NWC) * (uint32_t)NT;   // steps of this CTA
+            uint32_t no = 0;                                         // next output MMA to issue
+            auto out_ready = [&](uint32_t o) {
+                return mbar_try_wait(&q_full[o % QST], (o / QST) & 1u) && (o < 2 || mbar_try_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u));
+            };
+            auto issue_out = [&](uint32_t o) {                       // S_o is published (o <= the chain step just issued)
+                const int qst = o % QST, sb = o % NSB;
+                mbar_wait(&q_full[qst], (o / QST) & 1u);
+                if (o >= 2) mbar_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u);
+                tc_fence_after();
+                const uint32_t aQ = smem_u32(sQ + qst * L::Q_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
+                const uint32_t acc_out = tmem + 64 + 64 * (o & 1);
 #pragma unroll
-                    for (int s = 0; s < D / 16; ++s)
-                        umma_bf16(acc_chain, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), idc, s > 0);
-                    umma_commit(mma_chain);
-                    umma_commit(&g_empty[gst]);
-                    // output: acc_out = Qt_c (A, K-major) * S_c
-                    mbar_wait(&q_full[qst], (gs / QST) & 1u);
-                    if (gs >= 2) mbar_wait(&out_free[gs & 1], ((gs >> 1) - 1) & 1u);
-                    tc_fence_after();
-                    const uint32_t aQ = smem_u32(sQ + qst * L::Q_BYTES);
-                    const uint32_t acc_out = tmem + 64 + 64 * (gs & 1);
+                for (int s = 0; s < D / 16; ++s)
+                    umma_bf16(acc_out, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), ido, s > 0);
+                umma_commit(&out_full[o & 1]);
+                umma_commit(&s_free[sb]);
+            };
+            for (uint32_t gs = 0; gs < total; ++gs) {
+                const int gst = gs % GST, sb = gs % NSB;
+                // publication gs reuses the buffer of step gs - NSB: its output MMA must be out before we block on s_ready
+                while (no + NSB <= gs) issue_out(no++);
+                mbar_wait(&g_full[gst], (gs / GST) & 1u);
+                if (gs == 12) GDN_STAMP_ANY(40);
+                mbar_wait(&s_ready[sb], (gs / NSB) & 1u);
+                if (gs == 12) GDN_STAMP_ANY(41);
+                tc_fence_after();
+                const uint32_t aG = smem_u32(sG + gst * L::GN_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
 #pragma unroll
-                    for (int s = 0; s < D / 16; ++s)
-                        umma_bf16(acc_out, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), ido, s > 0);
-                    umma_commit(&out_full[gs & 1]);
-                }
+                for (int s = 0; s < D / 16; ++s)
+                    umma_bf16(acc_chain, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), idc, s > 0);
+                umma_commit(mma_chain);
+                umma_commit(&g_empty[gst]);
+                if (gs == 12) GDN_STAMP_ANY(42);
+                while (no <= gs && out_ready(no)) issue_out(no++);
             }
+            while (no < total) issue_out(no++);
         }
     } else if (warp < 8) {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
@@ -173,8 +229,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
         const int m = (D == 128) ? (wq * 32 + lane) : (16 * wq + lane);     // state row (M = 64 uses lanes 0-15 of a quadrant)
         const bool m_ok = (D == 128) || (lane < 16);
         const int mm = m_ok ? m : 0;
-        float S[32], Nr[32];
-        uint32_t gs = 0;
+        float S[32];
+        uint32_t gs = 0;                                                    // steps done; also the index of the next publication
         for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
             const int bh = u / NCT, ct = u % NCT;
             const int col0 = ct * 64 + half * 32;
@@ -186,9 +242,12 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
 #pragma unroll
                 for (int i = 0; i < 32; ++i) S[i] = 0.f;
             }
-            auto publish = [&](uint32_t buf) {
+            // publication `pi` (= the state at the start of step pi) goes to operand buffer pi % NSB
+            auto publish = [&](uint32_t pi) {
+                const uint32_t sb = pi % NSB;
+                if (pi >= (uint32_t)NSB) mbar_wait(&s_free[sb], ((pi / NSB) - 1) & 1u);   // output MMA of step pi - NSB is done with it
                 if (m_ok) {
-                    const uint32_t sbase = smem_u32(sS + buf * L::S_BYTES);
+                    const uint32_t sbase = smem_u32(sS + sb * L::S_BYTES);
 #pragma unroll
                     for (int ch = 0; ch < 4; ++ch)
                         st_shared_v4(sbase + swz_chunk_off(m, half * 4 + ch, 0), pack_bf16(S[8 * ch], S[8 * ch + 1]), pack_bf16(S[8 * ch + 2], S[8 * ch + 3]),
@@ -196,27 +255,31 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(s_ready);
+                if (lane == 0) mbar_arrive(&s_ready[sb]);
             };
-            // chunk-major N_c: [(col / 4) * D + row] float4
-            auto load_N = [&](int c) {
-                const float4* src = reinterpret_cast<const float4*>(p.Nw + ((long long)bh * p.NC + c) * D * D) + (col0 >> 2) * D + mm;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) { const float4 f = __ldcg(src + i * D); Nr[4 * i] = f.x; Nr[4 * i + 1] = f.y; Nr[4 * i + 2] = f.z; Nr[4 * i + 3] = f.w; }
-            };
-            publish(gs & 1);
-            mbar_wait(&g_full[gs % GST], (gs / GST) & 1u);      // ordered after the poller's acquire of flag (bh, 0)
-            load_N(0);
-            float gamma_c = __ldcg(p.gam + (long long)bh * p.NC);
+            publish(gs);
             for (int c = 0; c < NT; ++c, ++gs) {
+                const int gst = gs % GST;
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(32);
+                mbar_wait(&g_full[gst], (gs / GST) & 1u);
+                const float gamma_c = sGamma[gst];
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(33);
+                {   // state-independent half, while the MMA runs: S <- gamma_c S + N_c
+                    const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES + half * (D * 128));
 #pragma unroll
-                for (int i = 0; i < 32; ++i) S[i] = fmaf(gamma_c, S[i], Nr[i]);          // state-independent half, during the MMA
-                if (c + 1 < NT) {
-                    mbar_wait(&g_full[(gs + 1) % GST], ((gs + 1) / GST) & 1u);
-                    load_N(c + 1);
-                    gamma_c = __ldcg(p.gam + (long long)bh * p.NC + c + 1);
+                    for (int ch = 0; ch < 8; ++ch) {
+                        const uint4 uu = ld_shared_v4(nbase + swz_chunk_off(mm, ch, 0));
+                        S[4 * ch + 0] = fmaf(gamma_c, S[4 * ch + 0], __uint_as_float(uu.x));
+                        S[4 * ch + 1] = fmaf(gamma_c, S[4 * ch + 1], __uint_as_float(uu.y));
+                        S[4 * ch + 2] = fmaf(gamma_c, S[4 * ch + 2], __uint_as_float(uu.z));
+                        S[4 * ch + 3] = fmaf(gamma_c, S[4 * ch + 3], __uint_as_float(uu.w));
+                    }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&g_empty[gst]);                   // gamma_c and N_c of the stage have been read
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(34);
                 mbar_wait(mma_chain, gs & 1u);
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(35);
                 tc_fence_after();
                 {
                     float v[32];
@@ -225,7 +288,11 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     for (int i = 0; i < 32; ++i) S[i] -= v[i];
                 }
                 tc_fence_before();
-                if (c + 1 < NT) publish((gs + 1) & 1);
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(36);
+                if (c + 1 < NT) publish(gs + 1);
+                if (gs == 12 && tid == 0) GDN_STAMP_ANY(37);
+                if (gs == 11 && tid == 0) GDN_STAMP_ANY(31);
+                if (tid == 0) GDN_TRACE(2 * gs + 1);
             }
             if (m_ok) {
                 float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + col0);
@@ -234,7 +301,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             }
         }
     } else if (warp < 12) {
-        // ===== output epilogue: out = scale (acc_out + Ol), staged in the Qt buffer, TMA store =====
+        // ===== output epilogue: out += scale * acc_out (the prepass already stored scale * Ol there): the tile is
+        //       staged as bf16 in block 0 of the Qt buffer and leaves as a TMA reduction (add) =====
         const int ew = warp - 8;
         const int row = ew * 32 + lane;
         uint32_t gs = 0;
@@ -243,33 +311,28 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             const int b = bh / p.H, h = bh % p.H;
             for (int c = 0; c < NT; ++c, ++gs) {
                 const int qst = gs % QST;
-                mbar_wait(&q_full[qst], (gs / QST) & 1u);       // ordered after the poller's acquire of flag (bh, c)
-                uint4 ol[8];
-                {
-                    const uint4* src = reinterpret_cast<const uint4*>(p.Ol + ((long long)bh * NT + c) * 128 * D) + (ct * 8) * 128 + row;
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) ol[i] = __ldcg(src + i * 128);
-                }
-                mbar_wait(&out_full[gs & 1], (gs >> 1) & 1u);
+                mbar_wait(&out_full[gs & 1], (gs >> 1) & 1u);         // implies q_full of the stage
                 tc_fence_after();
-                float v[64];
-                tmem_ld64(tmem_addr(tmem + 64 + 64 * (gs & 1), ew * 32, 0), v);
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&out_free[gs & 1]);
                 const uint32_t stg = smem_u32(sQ + qst * L::Q_BYTES);
 #pragma unroll
-                for (int ch = 0; ch < 8; ++ch) {
-                    float f[8];
-                    unpack8(ol[ch], f);
+                for (int hf = 0; hf < 2; ++hf) {
+                    float v[32];
+                    tmem_ld32(tmem_addr(tmem + 64 + 64 * (gs & 1), ew * 32, hf * 32), v);
+                    if (hf == 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&out_free[gs & 1]);
+                    }
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = p.scale * (v[8 * ch + e] + f[e]);
-                    st_shared_v4(stg + swz_chunk_off(row, ch, 0), pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+                    for (int ch = 0; ch < 4; ++ch)
+                        st_shared_v4(stg + swz_chunk_off(row, hf * 4 + ch, 0),
+                                     pack_bf16(p.scale * v[8 * ch], p.scale * v[8 * ch + 1]), pack_bf16(p.scale * v[8 * ch + 2], p.scale * v[8 * ch + 3]),
+                                     pack_bf16(p.scale * v[8 * ch + 4], p.scale * v[8 * ch + 5]), pack_bf16(p.scale * v[8 * ch + 6], p.scale * v[8 * ch + 7]));
                 }
                 fence_proxy_async();
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 if (warp == 8 && lane == 0) {
-                    tma_store_5d(tmO, sQ + qst * L::Q_BYTES, ct * 64, h, c * 128, 0, b);
+                    tma_reduce_add_5d(tmO, sQ + qst * L::Q_BYTES, ct * 64, h, c * 128, 0, b);
                     tma_store_commit();
                     tma_store_wait_read();
                     mbar_arrive(&q_empty[qst]);
@@ -288,14 +351,15 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
 // ---------------------------------------------------------------------------------------------------
 template <int D>
 __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* tmQ, const CUtensorMap* tmK, const CUtensorMap* tmV,
-                                             const CUtensorMap* tmG, const CUtensorMap* tmQt, const FusedParams& fp) {
+                                             const CUtensorMap* tmG, const CUtensorMap* tmN, const CUtensorMap* tmQt,
+                                             const CUtensorMap* tmOl, const FusedParams& fp) {
     const TokParams& p = fp.t;
     tok::PrepassCtx cx;
     uint32_t* tmem_slot;
     tok::prepass_carve<D>(smem, cx, &tmem_slot);
     const int tid = threadIdx.x;
     if (tid == 0) {
-        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
+        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
         mbar_fence_init();
     }
     if (tid < 32) tmem_alloc(tmem_slot, 512);
@@ -307,18 +371,28 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
     const int BH = p.B * p.H, NT = p.NT;
     const int round_tiles = fp.HPR * NT;
     uint32_t it = 0, ph = 0;
-    for (int i = w; i < fp.total_tiles; i += nwp, ++it) {
+    unsigned int* pending = nullptr;
+    auto tile_of = [&](int i, int& bh, int& tile) {
         // chunk-major inside a head group, so the chain workers of the group can follow closely
         const int r = i / round_tiles, il = i - r * round_tiles;
         const int hr = min(fp.HPR, BH - r * fp.HPR);
-        const int tile = il / hr, bh = r * fp.HPR + il % hr;
-        tok::prepass_tile<D, 128, true>(cx, tmQ, tmK, tmV, tmG, nullptr, tmQt, nullptr, p, bh, tile, it, ph);
-        if (tid == 0) {
-            tma_store_wait_all();                  // the tile's summaries are complete in global memory
-            fence_proxy_async_all();
-            __threadfence();
-            st_release_gpu(fp.flags + (long long)bh * NT + tile, fp.epoch);
-        }
+        tile = il / hr; bh = r * fp.HPR + il % hr;
+    };
+    for (int i = w; i < fp.total_tiles; i += nwp, ++it) {
+        int bh, tile, nbh = -1, ntile = -1;
+        tile_of(i, bh, tile);
+        if (i + nwp < fp.total_tiles) tile_of(i + nwp, nbh, ntile);
+        if (tid == 0) GDN_TRACE(2 * it);
+        // the previous tile's ready flag is published inside this tile, once its stores have completed
+        tok::prepass_tile<D, 128, true>(cx, tmQ, tmK, tmV, tmG, tmN, tmQt, tmOl, p, bh, tile, it, ph, pending, fp.epoch, nbh, ntile);
+        if (tid == 0) GDN_TRACE(2 * it + 1);
+        pending = fp.flags + (long long)bh * NT + tile;
+    }
+    if (tid == 0 && pending) {
+        tma_store_wait_all();                      // the last tile's summaries are complete in global memory
+        fence_proxy_async_all();
+        __threadfence();
+        st_release_gpu(pending, fp.epoch);
     }
     tc_fence_before();
     __syncthreads();
@@ -329,11 +403,12 @@ template <int D>
 __global__ void __launch_bounds__(kThreads, 1)
 gdn_tok_fused(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
               const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
-              const __grid_constant__ CUtensorMap tmQt, const __grid_constant__ CUtensorMap tmO, const FusedParams fp) {
+              const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmQt,
+              const __grid_constant__ CUtensorMap tmO, const FusedParams fp) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    if ((int)blockIdx.x < fp.NWC) chain_role<D>(smem, &tmG, &tmQt, &tmO, fp);
-    else prepass_role<D>(smem, &tmQ, &tmK, &tmV, &tmG, &tmQt, fp);
+    if ((int)blockIdx.x < fp.NWC) chain_role<D>(smem, &tmG, &tmN, &tmQt, &tmO, fp);
+    else prepass_role<D>(smem, &tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmO, fp);
 }
 
 }  // namespace fused

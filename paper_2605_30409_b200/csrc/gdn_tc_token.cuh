@@ -46,7 +46,9 @@ struct TokParams {
 
 #ifdef GDN_PHASE_TIMING
 #define GDN_STAMP(i) do { if (p.dbg && blockIdx.x == 0 && threadIdx.x == 0) p.dbg[i] = clock64(); } while (0)
+#define GDN_STAMP_ANY(i) do { if (p.dbg && blockIdx.x == 0) p.dbg[i] = clock64(); } while (0)      // any one thread of CTA 0
 #else
+#define GDN_STAMP_ANY(i) do { } while (0)
 #define GDN_STAMP(i) do { } while (0)
 #endif
 
@@ -110,7 +112,7 @@ __device__ __forceinline__ void inv32_columns(const float* __restrict__ Lt, int 
 struct PrepassCtx {
     uint8_t *sK, *sQ, *sV, *sA, *sB, *sC;
     float *sGam, *sBeta, *sBG, *sCF, *sWarp, *sL;
-    uint64_t *bar_kq, *bar_v, *bar_mma;
+    uint64_t *bar_kq, *bar_q, *bar_v, *bar_mma;    // bar_kq: K tile landed; bar_q: Q tile; bar_v: V tile
     uint32_t tmem;                                // 512 TMEM columns
 };
 template <int D>
@@ -132,21 +134,24 @@ __device__ __forceinline__ void prepass_carve(uint8_t* smem, PrepassCtx& cx, uin
     cx.sCF = cx.sBG + 128;                        // [128] e^{Gam_ref(j) - Gam_j}, ref = last row of j's 32-chunk
     cx.sWarp = cx.sCF + 128;                      // [4] per-warp sums of log alpha
     uint64_t* bars = reinterpret_cast<uint64_t*>(cx.sWarp + 4);
-    cx.bar_kq = &bars[0]; cx.bar_v = &bars[1]; cx.bar_mma = &bars[2];
-    *tmem_slot = reinterpret_cast<uint32_t*>(bars + 3);
+    cx.bar_kq = &bars[0]; cx.bar_v = &bars[1]; cx.bar_mma = &bars[2]; cx.bar_q = &bars[3];
+    *tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
 }
 
 // One 128-token tile of one (b,h) stream.  `it` = how many tiles this CTA has run before (barrier parity),
 // `ph` = running parity of bar_mma.  FUSED = false: summaries in the layouts of the three-kernel path
 // (N row-major fp32 [D][D], Ol row-major [rows][D]), the call returns after the stores have read their
-// staging.  FUSED = true (gdn_tc_fused.cuh, C = 128): N and Ol leave in "chunk-major" layouts
-// ([16-byte chunk][row]) that the chain workers read with coalesced loads, and the caller publishes the
-// tile's ready flag once the stores have completed.
+// staging.  FUSED = true (gdn_tc_fused.cuh, C = 128): scale * Ol is stored straight into `out` (tmOl is then
+// the map of `out`; the chain workers add scale * Qt S_c to it with a TMA reduction), the stores are left
+// draining while the next tile starts, and the tile's ready flag is published from inside the next tile
+// once they have completed.
 template <int D, int C, bool FUSED>
 __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtensorMap* tmQ, const CUtensorMap* tmK,
                                              const CUtensorMap* tmV, const CUtensorMap* tmG, const CUtensorMap* tmN,
                                              const CUtensorMap* tmQt, const CUtensorMap* tmOl, const TokParams& p,
-                                             int bh, int tile, uint32_t it, uint32_t& ph) {
+                                             int bh, int tile, uint32_t it, uint32_t& ph,
+                                             unsigned int* prev_flag = nullptr, unsigned int epoch = 0,
+                                             int next_bh = -1, int next_tile = -1) {
     static_assert(!FUSED || C == 128, "the fused path runs C = 128");
     constexpr int NH = kPrepassNH;
     constexpr int CW = 32 / NH;                   // columns of each 32-column chunk handled per thread
@@ -157,7 +162,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     constexpr int DS = D / 16;                    // K = 16 steps over the head dim
     uint8_t *sK = cx.sK, *sQ = cx.sQ, *sV = cx.sV, *sA = cx.sA, *sB = cx.sB, *sC = cx.sC;
     float *sGam = cx.sGam, *sBeta = cx.sBeta, *sBG = cx.sBG, *sCF = cx.sCF, *sWarp = cx.sWarp, *sL = cx.sL;
-    uint64_t *bar_kq = cx.bar_kq, *bar_v = cx.bar_v, *bar_mma = cx.bar_mma;
+    uint64_t *bar_kq = cx.bar_kq, *bar_q = cx.bar_q, *bar_v = cx.bar_v, *bar_mma = cx.bar_mma;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wq = warp & 3, hh = warp >> 2;
@@ -179,27 +184,22 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         g = 1.f;
     }
     if (tid == 0) {
-        mbar_expect_tx(bar_kq, 2 * TILE);
+        if (!FUSED || it == 0) {                   // FUSED, it > 0: the previous tile prefetched this tile's K
+            mbar_expect_tx(bar_kq, TILE);
 #pragma unroll
-        for (int nb = 0; nb < NB; ++nb) {
-            tma_load_5d(sK + nb * kBlk, tmK, bar_kq, nb * 64, h, tile * 128, 0, b);
-            tma_load_5d(sQ + nb * kBlk, tmQ, bar_kq, nb * 64, h, tile * 128, 0, b);
+            for (int nb = 0; nb < NB; ++nb) tma_load_5d(sK + nb * kBlk, tmK, bar_kq, nb * 64, h, tile * 128, 0, b);
         }
+        // FUSED: the previous tile's stores are still draining. Its first group (Qt, Ol) was staged in sQ / sV.
+        if (FUSED) tma_store_wait_read_but1();
+        mbar_expect_tx(bar_q, TILE);
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sQ + nb * kBlk, tmQ, bar_q, nb * 64, h, tile * 128, 0, b);
         mbar_expect_tx(bar_v, TILE);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, tmV, bar_v, nb * 64, h, tile * 128, 0, b);
     }
-    // zero this thread's columns of the three 128x128 operand buffers
-#pragma unroll
-    for (int cc = 0; cc < 4; ++cc) {
-#pragma unroll
-        for (int q2 = 0; q2 < CH; ++q2) {
-            const uint32_t off = swz_chunk_off(row, cc * 4 + hh * CH + q2, kBlk);
-            st_shared_v4(aA + off, 0, 0, 0, 0);
-            st_shared_v4(aB + off, 0, 0, 0, 0);
-            st_shared_v4(aC + off, 0, 0, 0, 0);
-        }
-    }
+    // The three 128x128 operand buffers are never pre-zeroed: every phase that fills one writes whole rows
+    // (data where the block structure has some, zeros elsewhere) -- see T2 (sA, sB) and the first X1 (sC).
 
     GDN_STAMP(1);
     // ---- T0: in-tile inclusive scan of log alpha (every warp of a quadrant computes it, hh == 0 publishes) ----
@@ -243,7 +243,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
 
     GDN_STAMP(2);
-    // ---- T1: K K^T -> c0, Q K^T -> c1 ------------------------------------------------------------
+    // ---- T1: K K^T -> c0 (Q K^T -> c1 follows in the shadow of the first doubling round trip) ------
     mbar_wait(bar_kq, par);
     GDN_STAMP(3);
     if (tid == 0) {
@@ -254,27 +254,40 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
             umma_bf16(c0, desc_kmajor(aK + off), desc_kmajor(aK + off), id, s > 0);
         }
-#pragma unroll
-        for (int s = 0; s < DS; ++s) {
-            const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
-            umma_bf16(c1, desc_kmajor(aQ + off), desc_kmajor(aK + off), id, s > 0);
-        }
+        // FUSED: G / N of the previous tile were staged in sA, sB, sC, which T2 overwrites once this commit
+        // has been observed -- their reads must have ended first.
+        if (FUSED) tma_store_wait_read();
         umma_commit(bar_mma);
+        if (FUSED && prev_flag) {                  // the previous tile's summaries are complete in global memory
+            tma_store_wait_all();
+            asm volatile("fence.proxy.async;" ::: "memory");
+            __threadfence();
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(prev_flag), "r"(epoch) : "memory");
+        }
     }
     wait_mma();
 
     GDN_STAMP(4);
     // ---- T2: L (strictly lower, decay-masked) -> sA off-diagonal chunks; diagonal 32x32 block -> Ld ----
 #pragma unroll
-    for (int cc = 0; cc < 3; ++cc) {
-        if (cc < wq && cc >= half_lo) {
-            float v[CW], cf[CW];
+    for (int cc = 0; cc < 4; ++cc) {
+        float v[CW];
+        if (cc < 3 && cc < wq && cc >= half_lo) {
+            float cf[CW];
             tmem_ldw(tmem_addr(c0, lane_base, cc * 32 + cb), v);
             ld_shared_fw(sCF + cc * 32 + cb, cf);
-            const float f = beta_i * rf[cc];
+            const float f = beta_i * rf[cc < 3 ? cc : 0];
 #pragma unroll
             for (int e = 0; e < CW; ++e) v[e] *= f * cf[e];
-            store_roww_bf16(aA, kBlk, row, cc * 32 + cb, v);
+        } else {
+#pragma unroll
+            for (int e = 0; e < CW; ++e) v[e] = 0.f;
+        }
+        store_roww_bf16(aA, kBlk, row, cc * 32 + cb, v);
+        if (cc != wq) {                            // sB = D: zero outside the diagonal block (written below)
+#pragma unroll
+            for (int e = 0; e < CW; ++e) v[e] = 0.f;
+            store_roww_bf16(aB, kBlk, row, cc * 32 + cb, v);
         }
     }
     GDN_STAMP(5);
@@ -320,39 +333,86 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     sync_then_issue();
 
     GDN_STAMP(6);
-    // one doubling level: Y = D (L_off D) -> c0.  X1 = L_off D is non-zero only in chunks cc < wq.
-    auto doubling_mmas = [&]() {
+    // One doubling level: Y = D (L_off D).  Only the blocks the level needs are computed, so the MMAs are
+    // small (the operands are block-structured: D is block-diagonal, L_off strictly block-lower):
+    //   level 1 (32 -> 64): Y[blk 2i+1, blk 2i] = D_{2i+1} L_{2i+1,2i} D_{2i}, i = 0, 1
+    //                       X1[:, blk 2i] = L_off[:, blk 2i] D_{2i}   (N = 32, K = 32) -> c0 columns 64 i
+    //                       Y [:, blk 2i] = D[:, blk 2i+1] X1[blk 2i+1, blk 2i]        -> c0 columns 64 i
+    //   level 2 (64 -> 128): Y[64:128, 0:64] = T_1 L[64:128, 0:64] T_0
+    //                       X1[:, 0:64] = L_off[:, 0:64] T_0        (N = 64, K = 64)   -> c0 columns 0..63
+    //                       Y [:, 0:64] = D'[:, 64:128] X1[64:128, 0:64]
+    // Rows outside the block a level needs hold partial sums and are never read.
+    auto doubling_mmas = [&](int level) {
         if (tid == 0) {           // X1 = L_off * D  (A = sA K-major, B = sB MN-major)
             tc_fence_after();
-            const uint32_t id = umma_idesc(128, 128, false, true);
+            if (level == 1) {
+                const uint32_t id = umma_idesc(128, 32, false, true);
 #pragma unroll
-            for (int s = 0; s < KS; ++s)
-                umma_bf16(c0, desc_kmajor(aA + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aB + s * 2048, kBlk), id, s > 0);
-            umma_commit(bar_mma);
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int s = 0; s < 2; ++s)
+                        umma_bf16(c0 + 64 * i, desc_kmajor(aA + i * kBlk + s * 32), desc_mnmajor(aB + i * kBlk + (4 * i + s) * 2048, kBlk), id, s > 0);
+                umma_commit(bar_mma);
+                // Q K^T -> c1: not needed before the P mask, so it runs while the X1 round trip is under way
+                // (the next commit covers it)
+                mbar_wait(bar_q, par);
+                tc_fence_after();
+                const uint32_t idq = umma_idesc(128, 128, false, false);
+#pragma unroll
+                for (int s = 0; s < DS; ++s) {
+                    const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
+                    umma_bf16(c1, desc_kmajor(aQ + off), desc_kmajor(aK + off), idq, s > 0);
+                }
+            } else {
+                const uint32_t id = umma_idesc(128, 64, false, true);
+#pragma unroll
+                for (int s = 0; s < 4; ++s)
+                    umma_bf16(c0, desc_kmajor(aA + s * 32), desc_mnmajor(aB + s * 2048, kBlk), id, s > 0);
+                umma_commit(bar_mma);
+            }
         }
         wait_mma();
+        if (level == 1) {         // whole rows: the needed block, zeros elsewhere (sC is never pre-zeroed)
 #pragma unroll
-        for (int cc = 0; cc < 3; ++cc) {
-            if (cc < wq && cc >= half_lo) {
+            for (int cc = 0; cc < 4; ++cc) {
                 float v[CW];
-                tmem_ldw(tmem_addr(c0, lane_base, cc * 32 + cb), v);
+                if ((wq & 1) && cc == wq - 1) {
+                    tmem_ldw(tmem_addr(c0, lane_base, cc * 32 + cb), v);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < CW; ++e) v[e] = 0.f;
+                }
                 store_roww_bf16(aC, kBlk, row, cc * 32 + cb, v);
             }
+        } else if (wq >= 2) {
+            float v0[CW], v1[CW];
+            tmem_ldw2(tmem_addr(c0, lane_base, cb), tmem_addr(c0, lane_base, 32 + cb), v0, v1);
+            store_roww_bf16(aC, kBlk, row, cb, v0);
+            store_roww_bf16(aC, kBlk, row, 32 + cb, v1);
         }
         sync_then_issue();
         if (tid == 0) {           // Y = D * X1  (A = sB K-major, B = sC MN-major)
             tc_fence_after();
-            const uint32_t id = umma_idesc(128, 128, false, true);
+            if (level == 1) {
+                const uint32_t id = umma_idesc(128, 32, false, true);
 #pragma unroll
-            for (int s = 0; s < KS; ++s)
-                umma_bf16(c0, desc_kmajor(aB + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aC + s * 2048, kBlk), id, s > 0);
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int s = 2; s < 4; ++s)
+                        umma_bf16(c0 + 64 * i, desc_kmajor(aB + i * kBlk + s * 32), desc_mnmajor(aC + i * kBlk + (4 * i + s) * 2048, kBlk), id, s > 2);
+            } else {
+                const uint32_t id = umma_idesc(128, 64, false, true);
+#pragma unroll
+                for (int s = 0; s < 4; ++s)
+                    umma_bf16(c0, desc_kmajor(aB + kBlk + s * 32), desc_mnmajor(aC + (4 + s) * 2048, kBlk), id, s > 0);
+            }
             umma_commit(bar_mma);
         }
         wait_mma();
     };
 
     // ---- T3/T4: 32 -> 64 blocks: D' = D - mask(D L_off D) ------------------------------------------
-    doubling_mmas();
+    doubling_mmas(1);
     GDN_STAMP(7);
     float Dlow[CW];                                // block (wq, wq-1) of the 64x64 inverse, odd wq
 #pragma unroll
@@ -369,7 +429,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     for (int j = 0; j < 2 * CW; ++j) Tlow[j] = 0.f;
     if (C == 128) {
         sync_then_issue();
-        doubling_mmas();
+        doubling_mmas(2);
         if (wq >= 2) {
             float v0[CW], v1[CW];
             tmem_ldw2(tmem_addr(c0, lane_base, cb), tmem_addr(c0, lane_base, 32 + cb), v0, v1);
@@ -501,8 +561,11 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
 #pragma unroll
                 for (int e = 0; e < 8; ++e) f[e] = gamma_i * f[e] - pw[8 * q4 + e];
                 st_shared_v4(aQ + off, pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
-                const uint32_t ooff = FUSED ? (uint32_t)(((cc * 4 + hh * CH + q4) * 128 + row) * 16) : off;   // chunk-major
-                st_shared_v4(odst + ooff, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
+                if (FUSED) {                       // this is the local part of the output itself: out = scale (Ol + Qt S_c)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) pu[8 * q4 + e] *= p.scale;
+                }
+                st_shared_v4(odst + off, pack_bf16(pu[8 * q4], pu[8 * q4 + 1]), pack_bf16(pu[8 * q4 + 2], pu[8 * q4 + 3]),
                              pack_bf16(pu[8 * q4 + 4], pu[8 * q4 + 5]), pack_bf16(pu[8 * q4 + 6], pu[8 * q4 + 7]));
             }
         }
@@ -517,8 +580,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                 store_roww_bf16(gdst, SBLK, m, cc * 32 + cb, gv);
 #pragma unroll
                 for (int q4 = 0; q4 < CW / 4; ++q4) {
-                    const uint32_t noff = FUSED ? (uint32_t)((((cc * 32 + cb) / 4 + q4) * D + m) * 16)                       // chunk-major
-                                                : cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4);
+                    const uint32_t noff = cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4);
                     st_shared_v4(ndst + noff, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
                                  __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
                 }
@@ -530,11 +592,8 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
             tma_store_2d(tmQt, sQ + nb * kBlk, nb * 64, r0);
-            if (!FUSED) tma_store_2d(tmOl, odst + nb * kBlk, nb * 64, r0);
-        }
-        if (FUSED) {
-#pragma unroll
-            for (int nb = 0; nb < NB; ++nb) bulk_store(p.Ol + (long long)r0 * D + nb * (kBlk / 2), odst + nb * kBlk, kBlk);
+            if (FUSED) tma_store_5d(tmOl, odst + nb * kBlk, nb * 64, h, tile * 128, 0, b);    // tmOl = map of `out` (rows past T are clipped)
+            else tma_store_2d(tmOl, odst + nb * kBlk, nb * 64, r0);
         }
     };
     auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
@@ -543,8 +602,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
 #pragma unroll
         for (int j = 0; j < D / 32; ++j) {
-            if (FUSED) bulk_store(p.Nw + (long long)z * D * D + j * (SBLK / 4), nsrc + j * SBLK, SBLK);
-            else tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
+            tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
         }
     };
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
@@ -552,6 +610,13 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     if (tid == 0) issue_summary(0);
     wait_mma();
     GDN_STAMP(13);
+    if (FUSED && tid == 0 && next_bh >= 0) {
+        // sK is free (the summary MMAs were its last readers): fetch the next tile's K ahead of this tile's
+        // stores, so the next K K^T does not queue behind them
+        mbar_expect_tx(bar_kq, TILE);
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sK + nb * kBlk, tmK, bar_kq, nb * 64, next_bh % p.H, next_tile * 128, 0, next_bh / p.H);
+    }
     if (C == 128) {
         // everything is free now: Qt in place, Ol -> sV, G -> sA, N -> sB (+ sC)
         stage_QO(c2, aV);
@@ -560,9 +625,10 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         publish_staging();
         if (tid == 0) {
             store_QO(sV);
+            if (FUSED) tma_store_commit();         // group 1: Qt, Ol (sQ, sV); group 2: G, N (sA, sB, sC)
             store_NG(sA, sB, tile);
             tma_store_commit();
-            tma_store_wait_read();
+            if (!FUSED) tma_store_wait_read();     // FUSED: the next tile waits where it reuses the staging
         }
     } else {
         // first half: drain [PUt | PW] (c2), send Qt / Ol off, then reuse c2 for the second chunk's [N | G]
@@ -592,7 +658,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
 
     GDN_STAMP(14);
-    if (FUSED) __syncthreads();        // the staging buffers are the next tile's operand buffers
 }
 
 template <int D, int C>
@@ -607,7 +672,7 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t* tmem_slot;
     prepass_carve<D>(smem, cx, &tmem_slot);
     if (threadIdx.x == 0) {
-        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
+        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
         mbar_fence_init();
     }
     if (threadIdx.x < 32) tmem_alloc(tmem_slot, 512);
