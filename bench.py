@@ -67,7 +67,7 @@ def bytes_per_call(wl):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons of one GPU during the timed region (pynvml)."""
 
-    def __init__(self, index: int, period: float = 0.02):
+    def __init__(self, index: int, period: float = 0.002):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -168,7 +168,7 @@ def cpu_baseline(wl, budget_s=12.0):
     t0 = time.perf_counter()
     _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=wl.group)
     one = time.perf_counter() - t0
-    reps = max(1, min(50, int(budget_s / max(one, 1e-3))))
+    reps = max(1, min(5000, int(budget_s / max(one, 1e-4))))
     t0 = time.perf_counter()
     for _ in range(reps):
         _, st = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, st, group=wl.group)
@@ -308,6 +308,21 @@ def plan_kernel_times(plan, step, steps, barrier):
     return [{"name": nm, "avg_us": 1e3 * m} for nm, m in zip(names, ms)]
 
 
+def ncu_traffic(kernel, wl):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on this workload, from the committed
+    ncu --set full summaries (profiles/ncu_traffic.csv); None when that kernel/workload was not captured."""
+    f = ROOT / "profiles" / "ncu_traffic.csv"
+    if not f.exists():
+        return None
+    key = (kernel, wl.name, "token" if wl.group == 1 else "frame")
+    best = None
+    for line in f.read_text().splitlines():
+        c = [x.strip() for x in line.split(",")]
+        if len(c) >= 5 and not line.startswith("#") and (c[0], c[1], c[2]) == key:
+            best = float(c[3]) + float(c[4])          # later rows (later rounds) win
+    return best
+
+
 def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
     """Roofline of the dominant kernel. HBM-bound: achieved = algorithmic bytes / duration."""
     dur_ms, name = ms_per_step, "whole step"
@@ -316,8 +331,8 @@ def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
         dur_ms, name = top["avg_us"] * 1e-3, top["name"]
     achieved = by / (dur_ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
-            "frac": achieved / pk["hbm_gbs"], "traffic": None, "peak_source": pk_src,
-            "algorithmic_bytes": by}
+            "frac": achieved / pk["hbm_gbs"], "traffic": ncu_traffic(name, wl), "peak_source": pk_src,
+            "algorithmic_bytes": by, "kernel_avg_us": dur_ms * 1e3}
 
 
 def main():
@@ -337,8 +352,8 @@ def main():
         args.warmup = 1 if args.warmup is None else args.warmup
         run_reference(args)
     else:
-        args.steps = 300 if args.steps is None else args.steps
-        args.warmup = max(3, 20 if args.warmup is None else args.warmup)
+        args.steps = 2000 if args.steps is None else args.steps
+        args.warmup = max(3, 50 if args.warmup is None else args.warmup)
         run_ours(args)
 
 

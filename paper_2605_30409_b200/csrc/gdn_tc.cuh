@@ -48,7 +48,7 @@ inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, in
     if (c.group != 1) {                                               // frame-wise (the paper's variant)
         *path = GDN_PATH_TC_FRAME;
         *chunk = 0;
-        *launches = 4;
+        *launches = 3;
         return true;
     }
     *path = GDN_PATH_TC_TOKEN;
@@ -59,7 +59,8 @@ inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, in
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// token splits per frame for Phase A: minimise (waves x tiles per split), small penalty per extra partial
+// token splits per frame for Phase A.  A split CTA streams `per` tiles and then pays for its partial (write, and
+// a share of the last CTA's fixed-order reduction): about two tile times each.  Minimise waves x that.
 inline int frame_splits(int units, int tpf, int sms) {
     int best = 1;
     double best_cost = 1e30;
@@ -67,8 +68,9 @@ inline int frame_splits(int units, int tpf, int sms) {
         const int per = (tpf + ns - 1) / ns;
         if ((ns - 1) * per >= tpf) continue;                   // would leave an empty split
         const long long ctas = (long long)units * ns;
-        const double cost = (double)((ctas + sms - 1) / sms) * per + 0.3 * ns;
-        if (cost < best_cost) { best_cost = cost; best = ns; }
+        const double epi = ns > 1 ? 2.0 + 0.5 * ns : 1.0;
+        const double cost = (double)((ctas + sms - 1) / sms) * (per + epi);
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = ns; }
     }
     return best;
 }
@@ -79,12 +81,12 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.D = c.d_k; tp.C = 0; tp.BH = c.B * c.H;
     tp.G = c.group; tp.F = c.T / c.group; tp.TPF = (c.group + 127) / 128;
     tp.NC = tp.F; tp.NSc = tp.F + 1; tp.NT = tp.F * tp.TPF;
-    tp.NSPLIT = frame_splits(tp.BH * tp.F, tp.TPF, sm_count > 0 ? sm_count : 148);
+    tp.NSPLIT = frame_splits(tp.BH * tp.F * (tp.D == 128 ? 2 : 1), tp.TPF, sm_count > 0 ? sm_count : 148);
     const size_t D = tp.D, BH = tp.BH, F = tp.F, NS = tp.NSPLIT;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
-    const size_t oP = carve(BH * F * NS * D * 2 * D * 4), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
-    const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2);
+    const size_t oP = carve(NS > 1 ? BH * F * NS * D * 2 * D * 4 : 16), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
+    const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -97,6 +99,12 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.Nw = reinterpret_cast<float*>(w + oN);
     tp.gam = reinterpret_cast<float*>(w + oGam);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
+    tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
+    if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
+        if (err) *err = "counter initialisation failed";
+        return GDN_ERR_CUDA;
+    }
     bool ok = true;
     {
         const uint64_t dims[3] = {D, D, BH * F}, str[3] = {2, D * 2, D * D * 2};
@@ -268,10 +276,9 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof) {
     using namespace frm;
-    constexpr int NB = D / 64;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
-    const size_t smem3 = NB * tok::kBlk + D * D * 2 + 256 + 1024;
+    const size_t smem3 = ReadSmem<D>::TOTAL;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = set_smem(gdn_frm_summaries<D>, smem1);
@@ -280,14 +287,14 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokPar
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
+    const int sms = tp.sm_count > 0 ? tp.sm_count : 148;
+    const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
     if (prof) prof->begin(st);
-    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT, kSumThreads, smem1, st>>>(tp.tmK, tp.tmV, fp);
+    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tp.tmK, tp.tmV, fp);
     if (prof) prof->mark(st, "gdn_frm_summaries");
-    gdn_frm_reduce<D><<<dim3(tp.BH * tp.F, kReduceSlices), 256, 0, st>>>(fp);
-    if (prof) prof->mark(st, "gdn_frm_reduce");
     tok::gdn_tok_chain<D><<<tp.BH * (D / 64), tok::kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, cp);
     if (prof) prof->mark(st, "gdn_tok_chain");
-    gdn_frm_readout<D><<<tp.BH * tp.F * tp.TPF, 128, smem3, st>>>(tp.tmQ, tp.tmSc, fp);
+    gdn_frm_readout<D><<<grid3, kReadThreads, smem3, st>>>(tp.tmQ, tp.tmSc, tp.tmO, fp);
     if (prof) prof->mark(st, "gdn_frm_readout");
     return cudaGetLastError();
 }
@@ -305,13 +312,15 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
     }
-    if (tp.fused && out != tp.co) {
-        if (!tc::make_act_tmap(&tp.tmO, out, c.B, c.T, c.H, c.d_v, c.T, ts(c.o_token_stride, c.d_v), 128, err)) { tp.co = nullptr; return GDN_ERR_CUDA; }
+    if ((tp.fused || tp.mode == GDN_PATH_TC_FRAME) && out != tp.co) {
+        const int Gm = (tp.mode == GDN_PATH_TC_FRAME) ? c.group : c.T;
+        if (!tc::make_act_tmap(&tp.tmO, out, c.B, c.T, c.H, c.d_v, Gm, ts(c.o_token_stride, c.d_v), 128, err)) { tp.co = nullptr; return GDN_ERR_CUDA; }
         tp.co = out;
     }
     if (tp.mode == GDN_PATH_TC_FRAME) {
         FrmParams fp{};
-        fp.alpha = alpha; fp.beta = beta; fp.out = out; fp.part = tp.part; fp.Gw = tp.Gw; fp.Nw = tp.Nw; fp.gam = tp.gam;
+        fp.alpha = alpha; fp.beta = beta; fp.out = out; fp.part = tp.part; fp.counters = tp.flags; fp.Gw = tp.Gw; fp.Nw = tp.Nw; fp.gam = tp.gam;
+        fp.total_tiles = tp.BH * tp.F * tp.TPF;
         fp.B = c.B; fp.H = c.H; fp.T = c.T; fp.G = tp.G; fp.F = tp.F; fp.NSPLIT = tp.NSPLIT; fp.TPF = tp.TPF; fp.NSc = tp.NSc;
         fp.o_ts = ts(c.o_token_stride, c.d_v);
         fp.scale = c.scale;
@@ -330,13 +339,14 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
-    p.dbg = nullptr;
+    p.dbg = nullptr; p.dbg_cta = 0;
 #ifdef GDN_PHASE_TIMING
     static long long* dbg_dev = nullptr;
     constexpr size_t kDbgWords = 64 + 160 * 128;      // 64 phase stamps + 128 trace slots per CTA
     if (!dbg_dev) cudaMalloc(&dbg_dev, kDbgWords * sizeof(long long));
     cudaMemsetAsync(dbg_dev, 0, kDbgWords * sizeof(long long), st);
     p.dbg = dbg_dev;
+    p.dbg_cta = tp.fused ? tp.NWC : 0;
 #endif
     cudaError_t e;
     if (tp.fused) e = (tp.D == 64) ? tc_launch_fused<64>(tp, p, st, prof) : tc_launch_fused<128>(tp, p, st, prof);
@@ -351,7 +361,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fprintf(stderr, "[gdn phase cycles]");
         for (int i = 1; i < 16; ++i) fprintf(stderr, " %d:%lld", i, hst[i] - hst[i - 1]);
         fprintf(stderr, " [5->19:%lld 19->20:%lld 20->21:%lld 21->16:%lld 16->18:%lld 18->17:%lld 17->6:%lld]", hst[19] - hst[5], hst[20] - hst[19], hst[21] - hst[20], hst[16] - hst[21], hst[18] - hst[16], hst[17] - hst[18], hst[6] - hst[17]);
-        fprintf(stderr, " total:%lld\n", hst[15] - hst[0]);
+        fprintf(stderr, " tile(0->14):%lld total:%lld\n", hst[14] - hst[0], hst[15] - hst[0]);
         fprintf(stderr, "[gdn chain step cycles] snapshot:%lld premath:%lld wait_mma:%lld ld+sub:%lld publish:%lld fence+sync:%lld total:%lld\n",
                 hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36], hst[38] - hst[37], hst[38] - hst[32]);
         fprintf(stderr, "[gdn fused chain step 12] prev-publish->top:%lld gfull+gam:%lld Nfma:%lld wait_mma:%lld ld+sub:%lld publish:%lld | mma warp: sready-seen@%lld commit@%lld (rel. to top) state-mma-done@%lld\n",

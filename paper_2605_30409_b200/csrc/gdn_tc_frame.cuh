@@ -1,17 +1,22 @@
 // gdn_tc_frame.cuh -- frame-wise (G = tokens per frame) Gated DeltaNet forward on tcgen05 tensor cores:
 // the paper's own variant (Eq. 4-5, Alg. 1), re-designed for sm_100a.
 //
-//   Phase A  gdn_frm_summaries : per (b,h,f) and token split, [Gram | A] = (sqrt(beta) K)^T [sqrt(beta) K | sqrt(beta) V]
-//                                token-contraction MMAs (M = d, N = 2d, K = tokens) fed by a TMA ring;
-//                                both operands are MN-major views of the TMA tiles, no transposes.
-//            gdn_frm_reduce    : fixed-order sum of the token-split partials -> G_f = alpha_f Gram_f (bf16),
-//                                N_f = A_f (fp32), gamma_f = alpha_f           (deterministic, no atomics)
+//   Phase A  gdn_frm_summaries : per (b,h,f) and token split, [Gram | A] = (diag(beta) K)^T [K | V]
+//                                token-contraction MMAs (M = d, N = 2d, K = tokens) fed by a TMA ring.  The B
+//                                operand [K | V] is the TMA tile itself; only the A operand diag(beta) K is a
+//                                thread-written copy.  Both are MN-major views, no transposes.
+//                                Token splits of a frame leave fp32 partials in the workspace; the LAST split CTA
+//                                to finish (a counter per frame) sums them in fixed split order -> G_f = alpha_f
+//                                Gram_f (bf16), N_f = A_f (fp32), gamma_f = alpha_f: deterministic, no atomics on
+//                                data, no separate reduction launch.
 //   Phase B  gdn_tok_chain     : S_f = alpha_f S_{f-1} - G_f S_{f-1} + N_f  -- the same one-MMA-per-step chain
 //                                kernel as the token-wise path (Eq. 5: S_f = alpha_f (I - Gram_f) S_{f-1} + A_f)
 //   Phase C  gdn_frm_readout   : O_f = scale * Q_f S_f  (every token of frame f reads the post-update state, Eq. 22)
+//                                persistent CTAs over contiguous tile ranges: TMA ring for Q, S_f reloaded only when
+//                                the frame changes, two TMEM accumulators, bf16 tiles leave by TMA store.
 //
 // Tokens beyond the end of a frame inside a 128-token tile are zero-filled by the 5-D tensor map
-// (d, H, G, F, B) and get beta = 0: they contribute nothing and are never stored.
+// (d, H, G, F, B) and get beta = 0: they contribute nothing; on the way out the same map clips them.
 #pragma once
 #include <cuda.h>
 
@@ -23,12 +28,14 @@ struct FrmParams {
     const float* alpha;          // [BH][F]
     const float* beta;           // [BH][T]
     void* out;                   // [B][T][H][D] bf16
-    float* part;                 // [BH*F][NSPLIT][D][2D] fp32 partial summaries
+    float* part;                 // [BH*F][NSPLIT][D][2D] fp32 partial summaries (NSPLIT > 1)
+    unsigned int* counters;      // [BH*F] split CTAs that have delivered their partial (self-resetting)
     __nv_bfloat16* Gw;           // [BH][F][D][D]
     float* Nw;                   // [BH][F][D][D]
     float* gam;                  // [BH][F]
     int B, H, T, G, F, NSPLIT, TPF;   // TPF = 128-token tiles per frame
     int NSc;                     // snapshot slots per (b,h) = F + 1
+    int total_tiles;             // BH * F * TPF (readout)
     long long o_ts;
     float scale;
     int log_alpha;
@@ -42,35 +49,54 @@ using tok::st_global_v4;
 
 constexpr int kSumThreads = 192;       // warps 0-3: beta scaling + epilogue; warp 4: MMA issuer; warp 5: TMA producer
 
+// NC = column split of the summary [Gram | A] across CTAs (d = 128: 2).  CTA j of a frame computes the 64-column
+// block j of Gram and of A over the tokens of its split: it loads K whole (the A operand is diag(beta) K with all d
+// features) plus V block j, and its B operand is [K block j | V block j].  No CTA adds to another one's columns,
+// so without a token split there are no partials and no reduction at all.
+template <int D>
+constexpr int sum_nc() { return D == 128 ? 2 : 1; }
+
 template <int D>
 struct SumSmem {
     static constexpr int NB = D / 64;
-    static constexpr uint32_t STAGE = 2u * NB * kBlk;                 // K tile then V tile (contiguous: one N = 2D operand)
-    static constexpr int STAGES = (D == 128) ? 3 : 5;
-    static constexpr uint32_t TOTAL = STAGES * STAGE + 512 + 1024;
+    static constexpr int NC = sum_nc<D>();
+    static constexpr uint32_t KTILE = NB * kBlk;                      // [128 tokens][D] bf16
+    static constexpr int VB = NB / NC;                                // V blocks of this CTA
+    static constexpr uint32_t STAGE = KTILE + VB * kBlk;              // K tile, then this CTA's V block(s)
+    static constexpr int STAGES = (D == 128) ? 3 : 4;
+    static constexpr int SCB = 2;                                     // diag(beta) K copies (the A operand)
+    static constexpr uint32_t OFF_SC = STAGES * STAGE;
+    static constexpr uint32_t OFF_BAR = OFF_SC + SCB * KTILE;
+    static constexpr uint32_t TOTAL = OFF_BAR + 512 + 1024;
 };
 
 // ---------------------------------------------------------------------------------------------------
-// Phase A.  grid = BH*F*NSPLIT, block = 192.
+// Phase A.  grid = BH*F*NSPLIT*NC, block = 192.
 // ---------------------------------------------------------------------------------------------------
 template <int D>
 __global__ void __launch_bounds__(kSumThreads, 1)
 gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const FrmParams p) {
     using L = SumSmem<D>;
-    constexpr int NB = L::NB;
-    constexpr int STAGES = L::STAGES;
+    constexpr int NB = L::NB, NC = L::NC;
+    constexpr int STAGES = L::STAGES, SCB = L::SCB;
+    constexpr int NW = 2 * D / NC;                // accumulator columns of this CTA: [Gram cols | A cols]
+    constexpr int HW = D / NC;                    // columns of each of the two halves
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + STAGES * L::STAGE);   // full[S], scaled[S], empty[S], done
-    uint64_t* bar_full = bars;
-    uint64_t* bar_scaled = bars + STAGES;
-    uint64_t* bar_empty = bars + 2 * STAGES;
-    uint64_t* bar_done = bars + 3 * STAGES;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 3 * STAGES + 1);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::OFF_BAR);
+    uint64_t* bar_full = bars;                    // [STAGES] TMA: K and V tiles landed
+    uint64_t* bar_empty = bar_full + STAGES;      // [STAGES] the MMAs that read the stage have completed
+    uint64_t* bar_scaled = bar_empty + STAGES;    // [SCB] diag(beta) K written (4 warps)
+    uint64_t* bar_sfree = bar_scaled + SCB;       // [SCB] the MMAs that read the copy have completed
+    uint64_t* bar_done = bar_sfree + SCB;
+    uint8_t* sSc = smem + L::OFF_SC;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar_done + 1);
+    uint32_t* last_flag = tmem_slot + 1;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int split = blockIdx.x % p.NSPLIT;
-    const int bhf = blockIdx.x / p.NSPLIT;
+    const int j = blockIdx.x % NC;                // column block
+    const int split = (blockIdx.x / NC) % p.NSPLIT;
+    const int bhf = blockIdx.x / (NC * p.NSPLIT);
     const int f = bhf % p.F, bh = bhf / p.F;
     const int b = bh / p.H, h = bh % p.H;
     // contiguous range of 128-token tiles of this frame handled by this split
@@ -80,8 +106,251 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     const int ntiles = max(0, tile_hi - tile_lo);
 
     if (tid == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_scaled[s], 128); mbar_init(&bar_empty[s], 1); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
+        for (int s = 0; s < SCB; ++s) { mbar_init(&bar_scaled[s], 4); mbar_init(&bar_sfree[s], 1); }
         mbar_init(bar_done, 1);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc(tmem_slot, NW);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 5) {
+        // ===== TMA producer =====
+        if (elect_one()) {
+            for (int i = 0; i < ntiles; ++i) {
+                const int st = i % STAGES;
+                if (i >= STAGES) mbar_wait(&bar_empty[st], (uint32_t)((i / STAGES) - 1) & 1u);
+                uint8_t* base = smem + st * L::STAGE;
+                mbar_expect_tx(&bar_full[st], L::STAGE);
+                const int n0 = (tile_lo + i) * 128;
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + nb * kBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
+                if (NC == 1) {
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + (NB + nb) * kBlk, &tmV, &bar_full[st], nb * 64, h, n0, f, b);
+                } else {
+                    tma_load_5d(base + NB * kBlk, &tmV, &bar_full[st], j * 64, h, n0, f, b);
+                }
+            }
+        }
+    } else if (warp == 4) {
+        // ===== MMA issuer: [Gram | A] += (beta K)^T [K | V]  (A = the scaled copy, B = the stage's 64-column blocks; MN-major) =====
+        if (elect_one()) {
+            const uint32_t id = umma_idesc(D, NW, true, true);
+            // B: all of K then all of V (NC = 1), or K block j then the V block (NC = 2)
+            const uint32_t b_off = (NC == 1) ? 0u : (uint32_t)j * kBlk;
+            const uint32_t b_lbo = (NC == 1) ? kBlk : (uint32_t)(NB - j) * kBlk;
+            for (int i = 0; i < ntiles; ++i) {
+                const int st = i % STAGES, sb = i % SCB;
+                mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
+                mbar_wait(&bar_scaled[sb], (uint32_t)(i / SCB) & 1u);
+                tc_fence_after();
+                const uint32_t a = smem_u32(sSc + sb * L::KTILE), bq = smem_u32(smem + st * L::STAGE) + b_off;
+#pragma unroll
+                for (int s = 0; s < 8; ++s)
+                    umma_bf16(tmem, desc_mnmajor(a + s * 2048, kBlk), desc_mnmajor(bq + s * 2048, b_lbo), id, (i > 0 || s > 0) ? 1u : 0u);
+                umma_commit(&bar_empty[st]);
+                umma_commit(&bar_sfree[sb]);
+            }
+            umma_commit(bar_done);
+        }
+    } else {
+        // ===== diag(beta) K copy (thread = token row of the tile), then the epilogue =====
+        const int row = tid;
+        const float* beta_f = p.beta + (long long)bh * p.T + (long long)f * p.G;
+        auto load_beta = [&](int i) { const int n = (tile_lo + i) * 128 + row; return (i < ntiles && n < p.G) ? __ldg(beta_f + n) : 0.f; };
+        float b_next = load_beta(0);               // one tile ahead: the global-load latency stays off the per-tile path
+        for (int i = 0; i < ntiles; ++i) {
+            const int st = i % STAGES, sb = i % SCB;
+            const float bt = b_next;
+            b_next = load_beta(i + 1);
+            if (i >= SCB) mbar_wait(&bar_sfree[sb], (uint32_t)((i / SCB) - 1) & 1u);
+            mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
+            const uint32_t src = smem_u32(smem + st * L::STAGE) + (uint32_t)row * 128u;
+            const uint32_t dst = smem_u32(sSc + sb * L::KTILE) + (uint32_t)row * 128u;
+#pragma unroll
+            for (int blk = 0; blk < NB; ++blk) {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) {
+                    // the scale is per row, so the copy keeps every 16-byte chunk where the swizzle put it; rotating
+                    // the chunk order by the row index keeps the 8 lanes of a quarter-warp on distinct banks
+                    const uint32_t off = blk * kBlk + (uint32_t)(((c + row) & 7) << 4);
+                    float x[8];
+                    unpack8(ld_shared_v4(src + off), x);
+                    st_shared_v4(dst + off, pack_bf16(x[0] * bt, x[1] * bt), pack_bf16(x[2] * bt, x[3] * bt),
+                                 pack_bf16(x[4] * bt, x[5] * bt), pack_bf16(x[6] * bt, x[7] * bt));
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_scaled[sb]);
+        }
+    }
+
+    // ---- epilogue (warps 0-3; thread = summary row m).  Accumulator column c: half c / HW (0 = Gram, 1 = A),
+    //      global column j * HW + c % HW --------------------------------------------------------------------
+    const int m = (D == 128) ? tid : (16 * warp + lane);
+    const bool m_ok = warp < 4 && ((D == 128) || (lane < 16));
+    float a_f = p.alpha[bhf];
+    if (p.log_alpha) a_f = expf(a_f);
+    if (p.NSPLIT == 1) {
+        // no token split: G_f = alpha_f Gram_f (bf16), N_f = A_f (fp32) straight from TMEM
+        if (warp < 4) {
+            mbar_wait(bar_done, 0);
+            tc_fence_after();
+            __nv_bfloat16* gdst = p.Gw + ((long long)bhf * D + m) * D + j * HW;
+            float* ndst = p.Nw + ((long long)bhf * D + m) * D + j * HW;
+#pragma unroll 1
+            for (int cc = 0; cc < NW / 32; ++cc) {
+                float v[32];
+                tmem_ld32(tmem_addr(tmem, warp * 32, cc * 32), v);
+                if (m_ok) {
+                    if (cc < HW / 32) {
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4)
+                            st_global_v4(gdst + cc * 32 + q4 * 8, pack_bf16(a_f * v[8 * q4], a_f * v[8 * q4 + 1]),
+                                         pack_bf16(a_f * v[8 * q4 + 2], a_f * v[8 * q4 + 3]), pack_bf16(a_f * v[8 * q4 + 4], a_f * v[8 * q4 + 5]),
+                                         pack_bf16(a_f * v[8 * q4 + 6], a_f * v[8 * q4 + 7]));
+                    } else {
+#pragma unroll
+                        for (int q4 = 0; q4 < 8; ++q4)
+                            st_global_v4(ndst + (cc - HW / 32) * 32 + q4 * 4, __float_as_uint(v[4 * q4]), __float_as_uint(v[4 * q4 + 1]),
+                                         __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
+                    }
+                }
+            }
+            if (tid == 0 && j == 0) p.gam[bhf] = a_f;
+        }
+    } else {
+        // partial [Gram | A] of this split -> workspace (fp32, full-width rows [D][2D]; this CTA owns its columns)
+        if (warp < 4) {
+            float* dst = p.part + (((long long)bhf * p.NSPLIT + split) * D + m) * (2 * D) + j * HW;
+            if (ntiles > 0) {
+                mbar_wait(bar_done, 0);
+                tc_fence_after();
+            }
+#pragma unroll 1
+            for (int cc = 0; cc < NW / 32; ++cc) {
+                float v[32];
+                if (ntiles > 0) {
+                    tmem_ld32(tmem_addr(tmem, warp * 32, cc * 32), v);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) v[e] = 0.f;
+                }
+                float* d2 = dst + (cc / (HW / 32)) * D + (cc % (HW / 32)) * 32;
+                if (m_ok) {
+#pragma unroll
+                    for (int q4 = 0; q4 < 8; ++q4)
+                        st_global_v4(d2 + q4 * 4, __float_as_uint(v[4 * q4]), __float_as_uint(v[4 * q4 + 1]),
+                                     __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
+                }
+            }
+        }
+        // the last CTA of the frame to get here reduces all partials in split order
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned int prev = atomicAdd(p.counters + bhf, 1u);
+            const bool last = prev == (unsigned int)(p.NSPLIT * NC) - 1u;
+            if (last) p.counters[bhf] = 0u;          // ready for the next call (stream order)
+            *last_flag = last ? 1u : 0u;
+        }
+        __syncthreads();
+        if (*last_flag) {
+            __threadfence();
+            const float4* src = reinterpret_cast<const float4*>(p.part + (long long)bhf * p.NSPLIT * D * 2 * D);
+            constexpr int ROW4 = 2 * D / 4;             // float4 per summary row
+            constexpr int TOT4 = D * ROW4;
+            constexpr int UN = 4;                       // independent float4 columns per thread per pass (loads in flight)
+            for (int e0 = tid; e0 < TOT4; e0 += UN * kSumThreads) {
+                float4 acc[UN];
+#pragma unroll
+                for (int u = 0; u < UN; ++u) {
+                    const int e = e0 + u * kSumThreads;
+                    acc[u] = (e < TOT4) ? __ldcg(src + e) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+                for (int s = 1; s < p.NSPLIT; ++s) {
+                    float4 v[UN];
+#pragma unroll
+                    for (int u = 0; u < UN; ++u) {
+                        const int e = e0 + u * kSumThreads;
+                        v[u] = (e < TOT4) ? __ldcg(src + (long long)s * TOT4 + e) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+#pragma unroll
+                    for (int u = 0; u < UN; ++u) { acc[u].x += v[u].x; acc[u].y += v[u].y; acc[u].z += v[u].z; acc[u].w += v[u].w; }
+                }
+#pragma unroll
+                for (int u = 0; u < UN; ++u) {
+                    const int e = e0 + u * kSumThreads;
+                    if (e >= TOT4) continue;
+                    const int mm = e / ROW4, c4 = e % ROW4;
+                    if (c4 < D / 4) {
+                        __nv_bfloat16* g = p.Gw + ((long long)bhf * D + mm) * D + c4 * 4;
+                        uint2 uu;
+                        uu.x = pack_bf16(a_f * acc[u].x, a_f * acc[u].y);
+                        uu.y = pack_bf16(a_f * acc[u].z, a_f * acc[u].w);
+                        *reinterpret_cast<uint2*>(g) = uu;
+                    } else {
+                        float* n = p.Nw + ((long long)bhf * D + mm) * D + (c4 - D / 4) * 4;
+                        *reinterpret_cast<float4*>(n) = acc[u];
+                    }
+                }
+            }
+            if (tid == 0) p.gam[bhf] = a_f;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, NW);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Phase C.  grid = min(#SM, tiles), block = 192.   O = scale * Q_f S_f   (S_f = snapshot slot f + 1)
+//   CTA c runs the contiguous tile range [c n / grid, (c+1) n / grid) of the (b,h,f,tile) order.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kReadThreads = 192;      // warps 0-3: epilogue (thread = token row); warp 4: MMA issuer; warp 5: TMA producer
+
+template <int D>
+struct ReadSmem {
+    static constexpr int NB = D / 64;
+    static constexpr uint32_t Q_BYTES = NB * kBlk;                    // [128][D] bf16
+    static constexpr uint32_t S_BYTES = (uint32_t)D * D * 2;          // NB blocks of [D][64] bf16
+    static constexpr int QST = (D == 128) ? 3 : 4;
+    static constexpr uint32_t OFF_S = QST * Q_BYTES;
+    static constexpr uint32_t OFF_O = OFF_S + 2 * S_BYTES;            // 2 x out staging [128][D] bf16
+    static constexpr uint32_t OFF_BAR = OFF_O + 2 * Q_BYTES;
+    static constexpr uint32_t TOTAL = OFF_BAR + 512 + 1024;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kReadThreads, 1)
+gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmSc,
+                const __grid_constant__ CUtensorMap tmO, const FrmParams p) {
+    using L = ReadSmem<D>;
+    constexpr int NB = L::NB, QST = L::QST;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* sS = smem + L::OFF_S;
+    uint8_t* sO = smem + L::OFF_O;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::OFF_BAR);
+    uint64_t* q_full = bars;                  // [QST]
+    uint64_t* q_empty = q_full + QST;         // [QST] the MMAs that read the Q tile have completed
+    uint64_t* s_full = q_empty + QST;         // [2]
+    uint64_t* s_empty = s_full + 2;           // [2]   the last MMA that reads this state has completed
+    uint64_t* acc_full = s_empty + 2;         // [2]
+    uint64_t* acc_empty = acc_full + 2;       // [2]   drained by the 4 epilogue warps
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long long nt = p.total_tiles;
+    const int t_lo = (int)(nt * blockIdx.x / gridDim.x), t_hi = (int)(nt * (blockIdx.x + 1) / gridDim.x);
+    if (tid == 0) {
+        for (int s = 0; s < QST; ++s) { mbar_init(&q_full[s], 1); mbar_init(&q_empty[s], 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], 1); mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); }
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(tmem_slot, 2 * D);
@@ -91,192 +360,92 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     const uint32_t tmem = *tmem_slot;
 
     if (warp == 5) {
-        // ===== TMA producer =====
-        if (lane == 0) {
-            for (int i = 0; i < ntiles; ++i) {
-                const int st = i % STAGES;
-                if (i >= STAGES) mbar_wait(&bar_empty[st], (uint32_t)((i / STAGES) - 1) & 1u);
-                uint8_t* base = smem + st * L::STAGE;
-                mbar_expect_tx(&bar_full[st], L::STAGE);
-                const int n0 = (tile_lo + i) * 128;
+        // ===== TMA producer: Q tiles through the ring, S_f whenever the frame changes =====
+        if (elect_one()) {
+            int cur = -1, ns = 0;
+            for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
+                const int bhf = t / p.TPF, tile = t % p.TPF;
+                const int f = bhf % p.F, bh = bhf / p.F;
+                if (bhf != cur) {
+                    const int sb = ns & 1;
+                    if (ns >= 2) mbar_wait(&s_empty[sb], (uint32_t)((ns >> 1) - 1) & 1u);
+                    mbar_expect_tx(&s_full[sb], L::S_BYTES);
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) {
-                    tma_load_5d(base + nb * kBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
-                    tma_load_5d(base + (NB + nb) * kBlk, &tmV, &bar_full[st], nb * 64, h, n0, f, b);
+                    for (int nb = 0; nb < NB; ++nb) tma_load_3d(sS + sb * L::S_BYTES + nb * (D * 128), &tmSc, &s_full[sb], nb * 64, 0, bh * p.NSc + f + 1);
+                    cur = bhf; ++ns;
                 }
+                const int st = i % QST;
+                if (i >= QST) mbar_wait(&q_empty[st], (uint32_t)((i / QST) - 1) & 1u);
+                mbar_expect_tx(&q_full[st], L::Q_BYTES);
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
             }
         }
     } else if (warp == 4) {
-        // ===== MMA issuer: [Gram | A] += K'^T [K' | V']  (A and B both MN-major views of the stage) =====
-        if (lane == 0) {
-            const uint32_t id = umma_idesc(D, 2 * D, true, true);
-            for (int i = 0; i < ntiles; ++i) {
-                const int st = i % STAGES;
-                mbar_wait(&bar_scaled[st], (uint32_t)(i / STAGES) & 1u);
+        // ===== MMA issuer: acc[i & 1] = Q tile (A, K-major) * S_f (B, MN-major) =====
+        if (elect_one()) {
+            const uint32_t id = umma_idesc(128, D, false, true);
+            int cur = -1, ns = 0;
+            for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
+                const int bhf = t / p.TPF;
+                if (bhf != cur) {
+                    if (cur >= 0) umma_commit(&s_empty[(ns - 1) & 1]);       // every MMA on the previous state has been issued
+                    mbar_wait(&s_full[ns & 1], (uint32_t)(ns >> 1) & 1u);
+                    cur = bhf; ++ns;
+                }
+                const int st = i % QST, a = i & 1;
+                mbar_wait(&q_full[st], (uint32_t)(i / QST) & 1u);
+                if (i >= 2) mbar_wait(&acc_empty[a], (uint32_t)((i >> 1) - 1) & 1u);
                 tc_fence_after();
-                const uint32_t a = smem_u32(smem + st * L::STAGE);
+                const uint32_t aQ = smem_u32(smem + st * L::Q_BYTES), aS = smem_u32(sS + ((ns - 1) & 1) * L::S_BYTES);
 #pragma unroll
-                for (int s = 0; s < 8; ++s)
-                    umma_bf16(tmem, desc_mnmajor(a + s * 2048, kBlk), desc_mnmajor(a + s * 2048, kBlk), id, (i > 0 || s > 0) ? 1u : 0u);
-                umma_commit(&bar_empty[st]);
+                for (int s = 0; s < D / 16; ++s)
+                    umma_bf16(tmem + a * D, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, D * 128), id, s > 0);
+                umma_commit(&acc_full[a]);
+                umma_commit(&q_empty[st]);
             }
-            umma_commit(bar_done);
         }
     } else {
-        // ===== beta scaling (thread = token row of the tile), then the epilogue =====
+        // ===== epilogue: TMEM -> registers -> scale -> bf16 -> swizzled staging -> TMA store =====
         const int row = tid;
-        for (int i = 0; i < ntiles; ++i) {
-            const int st = i % STAGES;
-            const int n = (tile_lo + i) * 128 + row;
-            float sb = 0.f;
-            if (n < p.G) sb = sqrtf(p.beta[(long long)bh * p.T + (long long)f * p.G + n]);
-            mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
-            const uint32_t base = smem_u32(smem + st * L::STAGE) + (uint32_t)row * 128u;
+        for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
+            const int bhf = t / p.TPF, tile = t % p.TPF;
+            const int f = bhf % p.F, bh = bhf / p.F;
+            const int a = i & 1;
+            // the store that read staging buffer `a` two tiles ago must have finished reading it
+            if (tid == 0) tma_store_wait_read_but1();
+            mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
+            tc_fence_after();
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            const uint32_t stg = smem_u32(sO + a * L::Q_BYTES);
 #pragma unroll
-            for (int blk = 0; blk < 2 * NB; ++blk) {
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    // the scale is per row, so any order of the row's 16-byte chunks works: rotate by the
-                    // row index to keep the 8 lanes of a quarter-warp on distinct banks
-                    const uint32_t addr = base + blk * kBlk + (uint32_t)(((c + row) & 7) << 4);
-                    float x[8];
-                    unpack8(ld_shared_v4(addr), x);
-                    st_shared_v4(addr, pack_bf16(x[0] * sb, x[1] * sb), pack_bf16(x[2] * sb, x[3] * sb),
-                                 pack_bf16(x[4] * sb, x[5] * sb), pack_bf16(x[6] * sb, x[7] * sb));
+            for (int cc = 0; cc < D / 32; ++cc) {
+                float v[32];
+                tmem_ld32(tmem_addr(tmem + a * D, warp * 32, cc * 32), v);
+                if (cc == D / 32 - 1) {
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&acc_empty[a]);
                 }
+#pragma unroll
+                for (int q4 = 0; q4 < 4; ++q4)
+                    st_shared_v4(stg + swz_chunk_off(row, cc * 4 + q4, kBlk),
+                                 pack_bf16(p.scale * v[8 * q4], p.scale * v[8 * q4 + 1]), pack_bf16(p.scale * v[8 * q4 + 2], p.scale * v[8 * q4 + 3]),
+                                 pack_bf16(p.scale * v[8 * q4 + 4], p.scale * v[8 * q4 + 5]), pack_bf16(p.scale * v[8 * q4 + 6], p.scale * v[8 * q4 + 7]));
             }
             fence_proxy_async();
-            mbar_arrive(&bar_scaled[st]);
-        }
-        // epilogue: partial [Gram | A] of this split -> workspace (fp32)
-        const int m = (D == 128) ? tid : (16 * warp + lane);
-        const bool m_ok = (D == 128) || (lane < 16);
-        float* dst = p.part + (((long long)bhf * p.NSPLIT + split) * D + m) * (2 * D);
-        if (ntiles > 0) {
-            mbar_wait(bar_done, 0);
-            tc_fence_after();
-#pragma unroll 1
-            for (int cc = 0; cc < 2 * D / 32; ++cc) {
-                float v[32];
-                tmem_ld32(tmem_addr(tmem, warp * 32, cc * 32), v);
-                if (m_ok) {
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (tid == 0) {
 #pragma unroll
-                    for (int q4 = 0; q4 < 8; ++q4)
-                        st_global_v4(dst + cc * 32 + q4 * 4, __float_as_uint(v[4 * q4]), __float_as_uint(v[4 * q4 + 1]),
-                                     __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
-                }
+                for (int nb = 0; nb < NB; ++nb) tma_store_5d(&tmO, sO + a * L::Q_BYTES + nb * kBlk, nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+                tma_store_commit();
             }
-        } else if (m_ok) {
-            for (int cc = 0; cc < 2 * D / 4; ++cc) st_global_v4(dst + cc * 4, 0, 0, 0, 0);
         }
+        if (tid == 0) tma_store_wait_all();
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, 2 * D);
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Fixed-order reduction of the split partials.  grid = (BH*F, kReduceSlices), block = 256.
-//   G_f = alpha_f * Gram_f (bf16),  N_f = A_f (fp32),  gamma_f = alpha_f
-// ---------------------------------------------------------------------------------------------------
-constexpr int kReduceSlices = 8;       // row slices per (b,h,f): enough CTAs to pull the partials at full bandwidth
-
-template <int D>
-__global__ void __launch_bounds__(256)
-gdn_frm_reduce(const FrmParams p) {
-    const int bhf = blockIdx.x;
-    float a = p.alpha[bhf];
-    if (p.log_alpha) a = expf(a);
-    if (threadIdx.x == 0 && blockIdx.y == 0) p.gam[bhf] = a;
-    const float4* src = reinterpret_cast<const float4*>(p.part + (long long)bhf * p.NSPLIT * D * 2 * D);
-    constexpr int ROW4 = 2 * D / 4;                 // float4 per summary row
-    constexpr int PER = D * ROW4 / kReduceSlices;
-    for (int e = blockIdx.y * PER + threadIdx.x; e < (blockIdx.y + 1) * PER; e += blockDim.x) {
-        float4 acc = src[e];
-        for (int s = 1; s < p.NSPLIT; ++s) {
-            const float4 v = src[(long long)s * D * ROW4 + e];
-            acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
-        }
-        const int m = e / ROW4, c4 = e % ROW4;
-        if (c4 < D / 4) {
-            __nv_bfloat16* g = p.Gw + ((long long)bhf * D + m) * D + c4 * 4;
-            uint2 u;
-            u.x = pack_bf16(a * acc.x, a * acc.y);
-            u.y = pack_bf16(a * acc.z, a * acc.w);
-            *reinterpret_cast<uint2*>(g) = u;
-        } else {
-            float* n = p.Nw + ((long long)bhf * D + m) * D + (c4 - D / 4) * 4;
-            *reinterpret_cast<float4*>(n) = acc;
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Phase C.  grid = BH*F*TPF, block = 128.   O = scale * Q_f S_f   (S_f = snapshot slot f + 1)
-// ---------------------------------------------------------------------------------------------------
-template <int D>
-__global__ void __launch_bounds__(128)
-gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmSc, const FrmParams p) {
-    constexpr int NB = D / 64;
-    constexpr uint32_t Q_BYTES = NB * kBlk;
-    constexpr uint32_t S_BYTES = (uint32_t)D * D * 2;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint8_t* sQ = smem;
-    uint8_t* sS = smem + Q_BYTES;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sS + S_BYTES);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
-
-    const int tid = threadIdx.x, warp = tid >> 5;
-    const int tile = blockIdx.x % p.TPF;
-    const int bhf = blockIdx.x / p.TPF;
-    const int f = bhf % p.F, bh = bhf / p.F;
-    const int b = bh / p.H, h = bh % p.H;
-    if (tid == 0) {
-        mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init();
-        mbar_expect_tx(&bars[0], Q_BYTES + S_BYTES);
-#pragma unroll
-        for (int nb = 0; nb < NB; ++nb) {
-            tma_load_5d(sQ + nb * kBlk, &tmQ, &bars[0], nb * 64, h, tile * 128, f, b);
-            tma_load_3d(sS + nb * (D * 128), &tmSc, &bars[0], nb * 64, 0, bh * p.NSc + f + 1);
-        }
-    }
-    if (warp == 0) tmem_alloc(tmem_slot, D);
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = *tmem_slot;
-    mbar_wait(&bars[0], 0);
-    if (tid == 0) {
-        tc_fence_after();
-        const uint32_t id = umma_idesc(128, D, false, true);
-        const uint32_t aQ = smem_u32(sQ), aS = smem_u32(sS);
-#pragma unroll
-        for (int s = 0; s < D / 16; ++s)
-            umma_bf16(tmem, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, D * 128), id, s > 0);
-        umma_commit(&bars[1]);
-    }
-    mbar_wait(&bars[1], 0);
-    tc_fence_after();
-    const int n = tile * 128 + tid;
-    const long long t = (long long)f * p.G + n;
-    __nv_bfloat16* dst = reinterpret_cast<__nv_bfloat16*>(p.out) + ((long long)b * p.T + t) * p.o_ts + (long long)h * D;
-#pragma unroll
-    for (int cc = 0; cc < D / 32; ++cc) {
-        float v[32];
-        tmem_ld32(tmem_addr(tmem, warp * 32, cc * 32), v);
-        if (n < p.G) {
-#pragma unroll
-            for (int q4 = 0; q4 < 4; ++q4)
-                st_global_v4(dst + cc * 32 + q4 * 8, pack_bf16(p.scale * v[8 * q4], p.scale * v[8 * q4 + 1]),
-                             pack_bf16(p.scale * v[8 * q4 + 2], p.scale * v[8 * q4 + 3]),
-                             pack_bf16(p.scale * v[8 * q4 + 4], p.scale * v[8 * q4 + 5]),
-                             pack_bf16(p.scale * v[8 * q4 + 6], p.scale * v[8 * q4 + 7]));
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, D);
 }
 
 }  // namespace frm

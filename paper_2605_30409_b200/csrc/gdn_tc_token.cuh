@@ -41,11 +41,12 @@ struct TokParams {
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
-    long long* dbg;              // developer builds (-DGDN_PHASE_TIMING): per-phase clock64 stamps of CTA 0
+    long long* dbg;              // developer builds (-DGDN_PHASE_TIMING): per-phase clock64 stamps of CTA dbg_cta
+    int dbg_cta;                 // the CTA whose prepass phases are stamped (fused kernel: the first prepass worker)
 };
 
 #ifdef GDN_PHASE_TIMING
-#define GDN_STAMP(i) do { if (p.dbg && blockIdx.x == 0 && threadIdx.x == 0) p.dbg[i] = clock64(); } while (0)
+#define GDN_STAMP(i) do { if (p.dbg && blockIdx.x == p.dbg_cta && threadIdx.x == 0) p.dbg[i] = clock64(); } while (0)
 #define GDN_STAMP_ANY(i) do { if (p.dbg && blockIdx.x == 0) p.dbg[i] = clock64(); } while (0)      // any one thread of CTA 0
 #else
 #define GDN_STAMP_ANY(i) do { } while (0)
