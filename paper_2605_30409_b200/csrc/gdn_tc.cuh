@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/gdn.h"
@@ -223,6 +224,18 @@ inline void tc_plan_free(TcPlan& tp) {
     tp.ready = false;
 }
 
+// Launch `kern` as a programmatic dependent of the previous kernel in the stream (see tc::pdl_wait).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 template <typename Kern>
 inline cudaError_t set_smem(Kern kern, size_t bytes) {
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
@@ -246,9 +259,11 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
     if (prof) prof->begin(st);
     gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmOl, p);
     if (prof) prof->mark(st, "gdn_tok_prepass");
-    gdn_tok_chain<D><<<tp.BH * (D / 64), kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, p);
+    cudaError_t le = launch_pdl(gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, p);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_chain");
-    gdn_tok_output<D, C><<<tp.BH * tp.NT, 128, smem3, st>>>(tp.tmQt, tp.tmSc, p);
+    le = launch_pdl(gdn_tok_output<D, C>, dim3(tp.BH * tp.NT), dim3(128), smem3, st, tp.tmQt, tp.tmSc, p);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_output");
     return cudaGetLastError();
 }
@@ -292,9 +307,11 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokPar
     if (prof) prof->begin(st);
     gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tp.tmK, tp.tmV, fp);
     if (prof) prof->mark(st, "gdn_frm_summaries");
-    tok::gdn_tok_chain<D><<<tp.BH * (D / 64), tok::kChainThreads, smem2, st>>>(tp.tmG, tp.tmN, tp.tmScS, cp);
+    cudaError_t le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_chain");
-    gdn_frm_readout<D><<<grid3, kReadThreads, smem3, st>>>(tp.tmQ, tp.tmSc, tp.tmO, fp);
+    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tp.tmQ, tp.tmSc, tp.tmO, fp);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
     return cudaGetLastError();
 }

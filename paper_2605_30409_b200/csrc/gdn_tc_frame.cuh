@@ -116,6 +116,7 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_launch_dependents();
 
     if (warp == 5) {
         // ===== TMA producer =====
@@ -358,6 +359,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();                                    // the chain's state snapshots are complete
 
     if (warp == 5) {
         // ===== TMA producer: Q tiles through the ring, S_f whenever the frame changes =====

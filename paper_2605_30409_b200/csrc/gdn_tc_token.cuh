@@ -681,6 +681,7 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     cx.tmem = *tmem_slot;
+    pdl_launch_dependents();
     uint32_t ph = 0;
     prepass_tile<D, C, false>(cx, &tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmOl, p, blockIdx.x / p.NT, blockIdx.x % p.NT, 0u, ph);
     tc_fence_before();
@@ -740,6 +741,8 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_launch_dependents();
+    pdl_wait();                                    // the summaries of the previous kernel are complete
 
     auto issue_loads = [&](int c) {
         const int st = c % STAGES;
@@ -899,6 +902,7 @@ gdn_tok_output(const __grid_constant__ CUtensorMap tmQt, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();                                    // the chain's state snapshots are complete
     const long long row = ((long long)bh * p.NT + tile) * 128 + tid;
     if (tid == 0) {
         mbar_expect_tx(&bars[0], QT_BYTES + NS * S_BYTES);

@@ -34,6 +34,13 @@ __device__ __forceinline__ float fast_exp(float x) {
     return y;
 }
 
+// Programmatic dependent launch (the host sets cudaLaunchAttributeProgrammaticStreamSerialization on the dependent
+// kernel).  pdl_launch_dependents: the next kernel in the stream may start its prologue on free SMs once every CTA of
+// this grid has got here.  pdl_wait: blocks until the previous kernel has completed and its writes are visible; a no-op
+// for a kernel launched without the attribute.  Nothing the previous kernel wrote may be touched before pdl_wait.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA / tcgen05 operand reads)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
