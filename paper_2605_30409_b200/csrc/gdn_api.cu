@@ -15,14 +15,26 @@
 #include "gdn_simt.cuh"
 #include "gdn_tc.cuh"
 
+struct gdn_plan;
+
 namespace {
 
 thread_local std::string g_plan_error;
 
-struct Staging {                 // device buffers for gdn_forward_chunk_host
-    void *q = nullptr, *k = nullptr, *v = nullptr, *out = nullptr;
-    float *alpha = nullptr, *beta = nullptr, *state = nullptr;
+// gdn_forward_chunk_host: device staging plus a copy/compute pipeline over token segments.  The call is cut into
+// up to kMaxSeg segments of Tseg tokens (whole 128-token tiles, resp. whole frames; exact by the split invariance of
+// the recurrence, PAPER.md L72 / App. G.6): segment s+1 travels host->device on a copy stream while segment s is
+// computed on the caller's stream and the output of segment s-1 travels back on a second copy stream.
+constexpr int kMaxSeg = 8;
+struct Staging {
+    void *q = nullptr, *k = nullptr, *v = nullptr, *out = nullptr;     // per segment compact [B,Tseg,H,d]
+    float *alpha = nullptr, *beta = nullptr, *state = nullptr;          // per segment compact [B,H,Tseg/G], [B,H,Tseg]
     bool ready = false;
+    int nseg = 1, Tseg = 0, Ttail = 0;           // nseg-1 segments of Tseg tokens, then one of Ttail (== Tseg if it divides)
+    gdn_plan_t* seg_plan = nullptr;               // plan for T = Tseg (nullptr: the owning plan itself, nseg == 1)
+    gdn_plan_t* tail_plan = nullptr;               // plan for T = Ttail when Ttail != Tseg
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_out = nullptr, ev_in[kMaxSeg] = {}, ev_comp[kMaxSeg] = {};
 };
 
 }  // namespace
@@ -261,26 +273,96 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
     const size_t ns = (size_t)c.B * c.H * c.d_k * c.d_v * 4;
     Staging& h = p->host;
     if (!h.ready) {
+        // segmentation: about 16 MB of input per segment (below that the per-copy overheads outweigh the overlap),
+        // whole 128-token tiles (G = 1) or whole frames
+        const int unit = c.group == 1 ? 128 : c.group;
+        const int units = (c.T + unit - 1) / unit;
+        int nseg = (int)((2 * nq + nv + na + nb) / (16u << 20));
+        if (nseg > kMaxSeg) nseg = kMaxSeg;
+        if (nseg > units) nseg = units;
+        if (nseg < 1) nseg = 1;
+        h.Tseg = c.T > 0 ? ((units + nseg - 1) / nseg) * unit : 0;
+        h.nseg = c.T > 0 ? (c.T + h.Tseg - 1) / h.Tseg : 1;
+        h.Ttail = c.T > 0 ? c.T - (h.nseg - 1) * h.Tseg : 0;
+        if (h.nseg == 1) { h.Tseg = h.Ttail = c.T; }
         cudaError_t e = cudaSuccess;
         auto alloc = [&](void** ptr, size_t n) { if (e == cudaSuccess) e = cudaMalloc(ptr, n ? n : 16); };
         alloc(&h.q, nq); alloc(&h.k, nq); alloc(&h.v, nv); alloc(&h.out, nv);
         alloc((void**)&h.alpha, na); alloc((void**)&h.beta, nb); alloc((void**)&h.state, ns);
         if (e != cudaSuccess) { cudaGetLastError(); return fail(p, GDN_ERR_NOMEM, "host-path staging allocation failed"); }
+        if (h.nseg > 1) {
+            gdn_config_t sc = c;
+            sc.T = h.Tseg;
+            if (gdn_plan(&sc, &h.seg_plan) != GDN_OK) return fail(p, GDN_ERR_NOMEM, std::string("segment plan: ") + g_plan_error);
+            if (h.Ttail != h.Tseg) {
+                sc.T = h.Ttail;
+                if (gdn_plan(&sc, &h.tail_plan) != GDN_OK) return fail(p, GDN_ERR_NOMEM, std::string("tail segment plan: ") + g_plan_error);
+            }
+            if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h.s_in, cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h.s_out, cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h.ev_start, cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h.ev_out, cudaEventDisableTiming);
+            for (int i = 0; i < h.nseg && e == cudaSuccess; ++i) {
+                e = cudaEventCreateWithFlags(&h.ev_in[i], cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h.ev_comp[i], cudaEventDisableTiming);
+            }
+            if (e != cudaSuccess) return cuda_fail(p, e, "host-path pipeline set-up");
+        }
         h.ready = true;
         p->workspace_bytes += 2 * nq + 2 * nv + na + nb + ns;
     }
     cudaError_t e = cudaSuccess;
-    auto h2d = [&](void* d, const void* s, size_t n) { if (e == cudaSuccess && n) e = cudaMemcpyAsync(d, s, n, cudaMemcpyHostToDevice, st); };
-    h2d(h.q, q_host, nq); h2d(h.k, k_host, nq); h2d(h.v, v_host, nv);
-    h2d(h.alpha, alpha_host, na); h2d(h.beta, beta_host, nb);
-    if (state_in_host) h2d(h.state, state_in_host, ns);
-    if (e != cudaSuccess) return cuda_fail(p, e, "host->device copy");
-    gdn_status_t fs = forward_impl(p, h.q, h.k, h.v, nullptr, nullptr, h.alpha, h.beta,
-                                   state_in_host ? h.state : nullptr, nullptr, h.out, h.state, nullptr, st, false);
-    if (fs != GDN_OK) return fs;
-    if (nv) e = cudaMemcpyAsync(out_host, h.out, nv, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(state_out_host, h.state, ns, cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return cuda_fail(p, e, "device->host copy");
+    if (h.nseg == 1) {                                 // small call: one copy in, one launch sequence, one copy out
+        auto h2d = [&](void* d, const void* s, size_t n) { if (e == cudaSuccess && n) e = cudaMemcpyAsync(d, s, n, cudaMemcpyHostToDevice, st); };
+        h2d(h.q, q_host, nq); h2d(h.k, k_host, nq); h2d(h.v, v_host, nv);
+        h2d(h.alpha, alpha_host, na); h2d(h.beta, beta_host, nb);
+        if (state_in_host) h2d(h.state, state_in_host, ns);
+        if (e != cudaSuccess) return cuda_fail(p, e, "host->device copy");
+        gdn_status_t fs = forward_impl(p, h.q, h.k, h.v, nullptr, nullptr, h.alpha, h.beta,
+                                       state_in_host ? h.state : nullptr, nullptr, h.out, h.state, nullptr, st, false);
+        if (fs != GDN_OK) return fs;
+        if (nv) e = cudaMemcpyAsync(out_host, h.out, nv, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(state_out_host, h.state, ns, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(p, e, "device->host copy");
+        return GDN_OK;
+    }
+    // ---- pipelined: copy-in stream | caller's stream (compute) | copy-out stream --------------------------------
+    auto ck = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    ck(cudaEventRecord(h.ev_start, st));               // everything queued on `st` before this call comes first
+    ck(cudaStreamWaitEvent(h.s_in, h.ev_start, 0));
+    ck(cudaStreamWaitEvent(h.s_out, h.ev_start, 0));
+    if (state_in_host) ck(cudaMemcpyAsync(h.state, state_in_host, ns, cudaMemcpyHostToDevice, h.s_in));
+    const size_t rowq = (size_t)c.H * c.d_k * es, rowv = (size_t)c.H * c.d_v * es;      // bytes per token
+    const int BH = c.B * c.H;
+    size_t oq = 0, ov = 0, oa = 0, ob = 0;              // byte offsets of the segment inside the staging buffers
+    for (int sgi = 0; sgi < h.nseg; ++sgi) {
+        const int t0 = sgi * h.Tseg, Ts = (sgi == h.nseg - 1) ? h.Ttail : h.Tseg;
+        const int Fs = Ts / c.group, f0 = t0 / c.group, Ftot = c.T / c.group;
+        uint8_t *dq = (uint8_t*)h.q + oq, *dk = (uint8_t*)h.k + oq, *dv = (uint8_t*)h.v + ov, *dout = (uint8_t*)h.out + ov;
+        float *da = (float*)((uint8_t*)h.alpha + oa), *db = (float*)((uint8_t*)h.beta + ob);
+        // [B,T,H,d] -> compact [B,Ts,H,d]: B rows of Ts*H*d elements, source pitch T*H*d
+        ck(cudaMemcpy2DAsync(dq, Ts * rowq, (const uint8_t*)q_host + t0 * rowq, c.T * rowq, Ts * rowq, c.B, cudaMemcpyHostToDevice, h.s_in));
+        ck(cudaMemcpy2DAsync(dk, Ts * rowq, (const uint8_t*)k_host + t0 * rowq, c.T * rowq, Ts * rowq, c.B, cudaMemcpyHostToDevice, h.s_in));
+        ck(cudaMemcpy2DAsync(dv, Ts * rowv, (const uint8_t*)v_host + t0 * rowv, c.T * rowv, Ts * rowv, c.B, cudaMemcpyHostToDevice, h.s_in));
+        // [B,H,T/G] -> [B,H,Ts/G] and [B,H,T] -> [B,H,Ts]
+        ck(cudaMemcpy2DAsync(da, (size_t)Fs * 4, alpha_host + f0, (size_t)Ftot * 4, (size_t)Fs * 4, BH, cudaMemcpyHostToDevice, h.s_in));
+        ck(cudaMemcpy2DAsync(db, (size_t)Ts * 4, beta_host + t0, (size_t)c.T * 4, (size_t)Ts * 4, BH, cudaMemcpyHostToDevice, h.s_in));
+        ck(cudaEventRecord(h.ev_in[sgi], h.s_in));
+        if (e != cudaSuccess) return cuda_fail(p, e, "host->device segment copy");
+        ck(cudaStreamWaitEvent(st, h.ev_in[sgi], 0));
+        gdn_plan_t* sp = (Ts == h.Tseg) ? h.seg_plan : h.tail_plan;
+        const float* sin = (sgi == 0 && !state_in_host) ? nullptr : h.state;
+        gdn_status_t fs = forward_impl(sp, dq, dk, dv, nullptr, nullptr, da, db, sin, nullptr, dout, h.state, nullptr, st, false);
+        if (fs != GDN_OK) return fail(p, fs, std::string("segment forward: ") + sp->err);
+        ck(cudaEventRecord(h.ev_comp[sgi], st));
+        ck(cudaStreamWaitEvent(h.s_out, h.ev_comp[sgi], 0));
+        ck(cudaMemcpy2DAsync((uint8_t*)out_host + t0 * rowv, c.T * rowv, dout, Ts * rowv, Ts * rowv, c.B, cudaMemcpyDeviceToHost, h.s_out));
+        oq += (size_t)c.B * Ts * rowq; ov += (size_t)c.B * Ts * rowv; oa += (size_t)BH * Fs * 4; ob += (size_t)BH * Ts * 4;
+    }
+    ck(cudaMemcpyAsync(state_out_host, h.state, ns, cudaMemcpyDeviceToHost, st));
+    ck(cudaEventRecord(h.ev_out, h.s_out));
+    ck(cudaStreamWaitEvent(st, h.ev_out, 0));          // `stream` completes only when every output byte is on the host
+    if (e != cudaSuccess) return cuda_fail(p, e, "host pipeline");
     return GDN_OK;
 }
 
@@ -292,6 +374,13 @@ gdn_status_t gdn_destroy(gdn_plan_t* plan) {
     Staging& h = plan->host;
     void* bufs[] = {h.q, h.k, h.v, h.out, h.alpha, h.beta, h.state};
     for (void* b : bufs) if (b) cudaFree(b);
+    if (h.seg_plan) gdn_destroy(h.seg_plan);
+    if (h.tail_plan) gdn_destroy(h.tail_plan);
+    if (h.s_in) cudaStreamDestroy(h.s_in);
+    if (h.s_out) cudaStreamDestroy(h.s_out);
+    if (h.ev_start) cudaEventDestroy(h.ev_start);
+    if (h.ev_out) cudaEventDestroy(h.ev_out);
+    for (int i = 0; i < kMaxSeg; ++i) { if (h.ev_in[i]) cudaEventDestroy(h.ev_in[i]); if (h.ev_comp[i]) cudaEventDestroy(h.ev_comp[i]); }
     delete plan;
     return GDN_OK;
 }

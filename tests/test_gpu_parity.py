@@ -142,6 +142,28 @@ def test_host_entry_point_matches_device_call():
     assert torch.equal(out, o_dev) and torch.equal(S_out, s_dev)
 
 
+@pytest.mark.parametrize("B,H,T,d,G", [(2, 16, 4096, 128, 1), (1, 16, 6144, 128, 2048), (2, 8, 4000, 128, 1)])
+def test_host_entry_point_pipelined_segments(B, H, T, d, G):
+    """Large enough for the host entry point to cut the call into token segments (copy-in | compute | copy-out
+    pipeline, incl. a shorter tail segment and B > 1 strided segment copies): same result as one device call."""
+    wl = gin.GdnWorkload("host_seg", B, H, T, d, d, group=G, seed=77)
+    inp = gin.make_inputs(wl)
+    o_dev, s_dev, _ = run_cuda(inp)
+    pin = lambda t: t.contiguous().pin_memory()
+    q, k, v, a, b, st = map(pin, (inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state))
+    out = torch.full_like(inp.v, float("nan")).pin_memory()
+    S_out = torch.full_like(inp.state, float("nan")).pin_memory()
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d, group=G) as p:
+        for _ in range(2):                                   # second call reuses the pipeline (events, staging)
+            p.forward_host(q, k, v, a, b, st, out, S_out)
+            torch.cuda.synchronize()
+    o_ref, S_ref = run_oracle(inp)
+    assert rel_err(out, o_ref) <= TOL_BF16 and rel_err(S_out, S_ref) <= TOL_BF16
+    # one device call vs segments: the state crosses a segment boundary as fp32 S_out/S_in instead of staying in
+    # registers, so single bf16 roundings of out may flip (one ulp of bf16 = 3.9e-3 relative)
+    assert rel_err(out, o_dev.double().numpy()) <= 1e-2 and rel_err(S_out, s_dev.double().numpy()) <= 1e-3
+
+
 # ---- normaliser path (paper Eq. 20-22) --------------------------------------------------------------
 @pytest.mark.parametrize("G", [1, 64])
 def test_normalizer_readout(G):
