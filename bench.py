@@ -179,6 +179,27 @@ def cpu_baseline(wl, budget_s=12.0):
             "sample": f"full {wl.name} workload x {reps} carried-state repeats ({dt:.1f} s of CPU work)"}
 
 
+def max_over_ranks(ms, dist, device=None):
+    """Device time of the slowest rank (every rank gets it). `dist` is torch.distributed or None (one process)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms)
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_tokens_per_s(world, wl, steps, ms):
+    """Whole-job throughput of `world` independent replicas (replicas only, weak scaling):
+    the tokens all ranks processed divided by the slowest rank's time."""
+    return world * wl.B * wl.T * steps / (ms * 1e-3)
+
+
+def rank_seed(wl, rank, i):
+    """Seed of input set i on `rank`: every replica streams its own data."""
+    return wl.seed + 17 * i + 1000 * rank
+
+
 def run_ours(args):
     import torch
     import paper_2605_30409_b200 as gdn
@@ -201,7 +222,7 @@ def run_ours(args):
     n_sets = min(n_sets, 16)
     sets = []
     for i in range(n_sets):
-        inp = gin.make_inputs(wl, seed=wl.seed + 17 * i + 1000 * rank)
+        inp = gin.make_inputs(wl, seed=rank_seed(wl, rank, i))
         sets.append(dict(q=inp.q.to(dev), k=inp.k.to(dev), v=inp.v.to(dev), alpha=inp.alpha.to(dev),
                          beta=inp.beta.to(dev), out=torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=wl.dtype, device=dev)))
     state = gin.make_inputs(wl).state.to(dev)
@@ -230,15 +251,11 @@ def run_ours(args):
         step(i)
     e1.record(stream)
     barrier()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev)
     clocks = sampler.stop()
     assert torch.isfinite(state).all(), "state diverged"
     ms_per_step = ms / args.steps
-    tokens_per_s = world * wl.B * wl.T * args.steps / (ms * 1e-3)
+    tokens_per_s = job_tokens_per_s(world, wl, args.steps, ms)
 
     # ---- per-kernel durations (separate pass with CUDA events between the launches) ----------------
     kernels = plan_kernel_times(plan, step, args.steps, barrier)
@@ -259,13 +276,9 @@ def run_ours(args):
             plan.forward_host(hq, hk, hv, ha, hb, hs, hout, hs, stream)
         e1.record(stream)
         barrier()
-        ms_e = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms_e], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e = float(t.item())
+        ms_e = max_over_ranks(e0.elapsed_time(e1), dist, dev)
         nbytes = lambda *ts: int(sum(t.numel() * t.element_size() for t in ts))
-        e2e = {"value": world * wl.B * wl.T * k_e2e / (ms_e * 1e-3), "unit": UNIT,
+        e2e = {"value": job_tokens_per_s(world, wl, k_e2e, ms_e), "unit": UNIT,
                "h2d_bytes_per_step": nbytes(hq, hk, hv, ha, hb, hs), "d2h_bytes_per_step": nbytes(hout, hs),
                "steps": k_e2e, "ms_per_step": ms_e / k_e2e}
 
