@@ -127,9 +127,10 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
     gdn_status_t ds = check_device(p);
     if (ds != GDN_OK) return ds;
 
-    if (p->path != GDN_PATH_SIMT_FP32 && !normalizer) {
+    if (p->path != GDN_PATH_SIMT_FP32) {
         std::string msg;
-        gdn_status_t ts = gdn::tc_forward(p->tc, c, q, k, v, alpha, beta, S_in, out, S_out, st, &p->prof, &msg);
+        gdn::NormArgs na{q_raw, k_raw, z_in, z_out};
+        gdn_status_t ts = gdn::tc_forward(p->tc, c, q, k, v, alpha, beta, S_in, out, S_out, st, &p->prof, &msg, normalizer ? &na : nullptr);
         if (ts != GDN_OK) return fail(p, ts, msg);
         return GDN_OK;
     }
@@ -206,8 +207,9 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
     p->path = GDN_PATH_SIMT_FP32;
     p->chunk = 0;
     p->launches = 1;
-    const bool want_tc = c.io_dtype == GDN_BF16 && !(c.flags & (GDN_FLAG_FORCE_SIMT | GDN_FLAG_NORMALIZER)) &&
-                         c.B > 0 && c.H > 0 && c.T > 0;
+    // the normalised readout has a tensor-core path in the frame-wise form only (the paper's case)
+    const bool want_tc = c.io_dtype == GDN_BF16 && !(c.flags & GDN_FLAG_FORCE_SIMT) &&
+                         !((c.flags & GDN_FLAG_NORMALIZER) && c.group == 1) && c.B > 0 && c.H > 0 && c.T > 0;
     if (want_tc) {
         std::string msg;
         gdn_path_t path;
@@ -217,7 +219,7 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
                 gdn_status_t ts = gdn::tc_plan_init(p->tc, c, p->sm_count, &msg);
                 if (ts != GDN_OK) { delete p; return fail(nullptr, ts, msg); }
             }
-            p->path = path; p->chunk = chunk; p->launches = launches;
+            p->path = path; p->chunk = chunk; p->launches = (c.flags & GDN_FLAG_NORMALIZER) ? 2 * launches : launches;
             p->workspace_bytes = p->tc.workspace_bytes;
         }
     }

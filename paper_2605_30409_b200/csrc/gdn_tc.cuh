@@ -38,6 +38,16 @@ struct TcPlan {
     unsigned int* flags = nullptr;
     unsigned int epoch = 0;
     int HPR = 0, NWC = 0, grid = 0;
+    // normaliser on the frame path: z as column 0 of a [D][D] fp32 state, den = q_raw . z per token
+    float *Sz = nullptr, *den = nullptr;
+    const void *cqr = nullptr, *ckr = nullptr;
+    CUtensorMap tmQr, tmKr;
+};
+
+struct NormArgs {                                  // the extra operands of gdn_forward_chunk_norm
+    const void *q_raw, *k_raw;
+    const float* z_in;
+    float* z_out;
 };
 
 inline int tc_default_chunk(const gdn_config_t& c) { return c.chunk ? c.chunk : 128; }
@@ -88,6 +98,8 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
     const size_t oP = carve(NS > 1 ? BH * F * NS * D * 2 * D * 4 : 16), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
     const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
+    const bool norm = (c.flags & GDN_FLAG_NORMALIZER) != 0;
+    const size_t oSz = norm ? carve(BH * D * D * 4) : 0, oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -101,6 +113,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.gam = reinterpret_cast<float*>(w + oGam);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
+    if (norm) { tp.Sz = reinterpret_cast<float*>(w + oSz); tp.den = reinterpret_cast<float*>(w + oDen); }
     if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "counter initialisation failed";
@@ -289,7 +302,8 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
 }
 
 template <int D>
-inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof) {
+inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
+                                   const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -305,12 +319,12 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokPar
     const int sms = tp.sm_count > 0 ? tp.sm_count : 148;
     const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
     if (prof) prof->begin(st);
-    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tp.tmK, tp.tmV, fp);
+    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tmK, tmV, fp);
     if (prof) prof->mark(st, "gdn_frm_summaries");
     cudaError_t le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_chain");
-    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tp.tmQ, tp.tmSc, tp.tmO, fp);
+    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
     return cudaGetLastError();
@@ -318,7 +332,7 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const FrmParams& fp, const TokPar
 
 inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q, const void* k, const void* v,
                                const float* alpha, const float* beta, const float* S_in, void* out, float* S_out,
-                               cudaStream_t st, Profiler* prof, std::string* err) {
+                               cudaStream_t st, Profiler* prof, std::string* err, const NormArgs* na = nullptr) {
     if (!tp.ready) { if (err) *err = "tensor-core plan was not initialised (no sm_100 device at plan time)"; return GDN_ERR_ARCH; }
     auto ts = [&](long long s, int d) { return s ? s : (long long)c.H * d; };
     if (q != tp.cq || k != tp.ck || v != tp.cv) {
@@ -345,7 +359,32 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         TokParams cp{};
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
         cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
-        const cudaError_t e = (tp.D == 64) ? tc_launch_frame<64>(tp, fp, cp, st, prof) : tc_launch_frame<128>(tp, fp, cp, st, prof);
+        cudaError_t e = cudaSuccess;
+        if (na) {
+            // z pass (Eq. 20-21 through the same three kernels): K_raw summaries with the constant block as V, the scan on
+            // a [D][D] state whose column 0 is z, q_raw . z_f per token -> den
+            if (na->q_raw != tp.cqr || na->k_raw != tp.ckr) {
+                bool ok = tc::make_act_tmap(&tp.tmQr, na->q_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.q_token_stride, c.d_k), 128, err) &&
+                          tc::make_act_tmap(&tp.tmKr, na->k_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.k_token_stride, c.d_k), 128, err);
+                if (!ok) { tp.cqr = tp.ckr = nullptr; return GDN_ERR_CUDA; }
+                tp.cqr = na->q_raw; tp.ckr = na->k_raw;
+            }
+            const size_t D = tp.D, rows = (size_t)tp.BH * D;
+            e = cudaMemsetAsync(tp.Sz, 0, rows * D * 4, st);
+            if (e == cudaSuccess && na->z_in) e = cudaMemcpy2DAsync(tp.Sz, D * 4, na->z_in, 4, 4, rows, cudaMemcpyDeviceToDevice, st);
+            if (e != cudaSuccess) { if (err) *err = std::string("z state staging: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+            FrmParams zf = fp;
+            zf.zpass = 1; zf.den = tp.den; zf.den_mode = 1; zf.scale = 1.f;
+            TokParams zc = cp;
+            zc.S_in = tp.Sz; zc.S_out = tp.Sz;
+            e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, st, prof)
+                             : tc_launch_frame<128>(tp, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, st, prof);
+            if (e == cudaSuccess) e = cudaMemcpy2DAsync(na->z_out, 4, tp.Sz, D * 4, 4, rows, cudaMemcpyDeviceToDevice, st);
+            if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+            fp.den = tp.den; fp.den_mode = 2; fp.eps = c.eps;
+        }
+        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof)
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

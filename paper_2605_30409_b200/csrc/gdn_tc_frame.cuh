@@ -39,6 +39,13 @@ struct FrmParams {
     long long o_ts;
     float scale;
     int log_alpha;
+    // normaliser (Eq. 20-22): the vector state z is run through the SAME kernels as column 0 of a matrix state
+    // ("the z path is the matrix path with v = 1", SURVEY pin 13): zpass = 1 replaces V by a constant block whose
+    // column 0 is one, so N_f[:, 0] = K^T beta = b_f and Gram is that of the un-rotated keys.
+    int zpass;
+    float* den;                  // [B][T][H] fp32: q_raw . z_f per token
+    int den_mode;                // readout: 0 = plain, 1 = write den (column 0 of Q_raw S^z), 2 = out = scale Q S / (den + eps)
+    float eps;
 };
 
 namespace frm {
@@ -66,7 +73,8 @@ struct SumSmem {
     static constexpr int STAGES = (D == 128) ? 3 : 4;
     static constexpr int SCB = 2;                                     // diag(beta) K copies (the A operand)
     static constexpr uint32_t OFF_SC = STAGES * STAGE;
-    static constexpr uint32_t OFF_BAR = OFF_SC + SCB * KTILE;
+    static constexpr uint32_t OFF_ONE = OFF_SC + SCB * KTILE;         // z pass: constant [128][64] block standing in for V
+    static constexpr uint32_t OFF_BAR = OFF_ONE + kBlk;
     static constexpr uint32_t TOTAL = OFF_BAR + 512 + 1024;
 };
 
@@ -112,6 +120,14 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(tmem_slot, NW);
+    const bool zp = p.zpass != 0;
+    if (zp && tid < 128) {
+        // row `tid` of the constant block: column 0 = 1 (first column block only), everything else 0
+        const uint32_t one = smem_u32(smem + L::OFF_ONE);
+#pragma unroll
+        for (int c = 0; c < 8; ++c) st_shared_v4(one + swz_chunk_off(tid, c, 0), (c == 0 && j == 0) ? 0x00003F80u : 0u, 0u, 0u, 0u);
+        fence_proxy_async();
+    }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -125,10 +141,11 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
                 const int st = i % STAGES;
                 if (i >= STAGES) mbar_wait(&bar_empty[st], (uint32_t)((i / STAGES) - 1) & 1u);
                 uint8_t* base = smem + st * L::STAGE;
-                mbar_expect_tx(&bar_full[st], L::STAGE);
+                mbar_expect_tx(&bar_full[st], zp ? L::KTILE : L::STAGE);
                 const int n0 = (tile_lo + i) * 128;
 #pragma unroll
                 for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + nb * kBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
+                if (zp) continue;                  // no V: the constant block stands in
                 if (NC == 1) {
 #pragma unroll
                     for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + (NB + nb) * kBlk, &tmV, &bar_full[st], nb * 64, h, n0, f, b);
@@ -150,9 +167,11 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
                 mbar_wait(&bar_scaled[sb], (uint32_t)(i / SCB) & 1u);
                 tc_fence_after();
                 const uint32_t a = smem_u32(sSc + sb * L::KTILE), bq = smem_u32(smem + st * L::STAGE) + b_off;
+                // z pass: the block after the K block(s) of this CTA is the constant block (any distance is a legal LBO)
+                const uint32_t lbo = zp ? smem_u32(smem + L::OFF_ONE) - (bq + (uint32_t)(NB / NC - 1) * kBlk) : b_lbo;
 #pragma unroll
                 for (int s = 0; s < 8; ++s)
-                    umma_bf16(tmem, desc_mnmajor(a + s * 2048, kBlk), desc_mnmajor(bq + s * 2048, b_lbo), id, (i > 0 || s > 0) ? 1u : 0u);
+                    umma_bf16(tmem, desc_mnmajor(a + s * 2048, kBlk), desc_mnmajor(bq + s * 2048, lbo), id, (i > 0 || s > 0) ? 1u : 0u);
                 umma_commit(&bar_empty[st]);
                 umma_commit(&bar_sfree[sb]);
             }
@@ -408,12 +427,28 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
         }
     } else {
-        // ===== epilogue: TMEM -> registers -> scale -> bf16 -> swizzled staging -> TMA store =====
+        // ===== epilogue: TMEM -> registers -> scale (/ normaliser) -> bf16 -> swizzled staging -> TMA store =====
         const int row = tid;
         for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
             const int bhf = t / p.TPF, tile = t % p.TPF;
             const int f = bhf % p.F, bh = bhf / p.F;
             const int a = i & 1;
+            const int n = tile * 128 + row;                      // token inside the frame
+            const long long tok = ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.H + (bh % p.H);   // index into den [B][T][H]
+            float mul = p.scale;
+            if (p.den_mode == 2 && n < p.G) mul = p.scale / (__ldg(p.den + tok) + p.eps);          // Eq. 22: eps after the dot product, no clamp
+            if (p.den_mode == 1) {
+                // z pass: only column 0 of Q_raw S^z is the normaliser q_raw . z_f; nothing goes to `out`
+                mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
+                tc_fence_after();
+                float v[8];
+                tmem_ld8(tmem_addr(tmem + a * D, warp * 32, 0), v);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[a]);
+                if (n < p.G) p.den[tok] = v[0];
+                continue;
+            }
             // the store that read staging buffer `a` two tiles ago must have finished reading it
             if (tid == 0) tma_store_wait_read_but1();
             mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
@@ -432,8 +467,8 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4)
                     st_shared_v4(stg + swz_chunk_off(row, cc * 4 + q4, kBlk),
-                                 pack_bf16(p.scale * v[8 * q4], p.scale * v[8 * q4 + 1]), pack_bf16(p.scale * v[8 * q4 + 2], p.scale * v[8 * q4 + 3]),
-                                 pack_bf16(p.scale * v[8 * q4 + 4], p.scale * v[8 * q4 + 5]), pack_bf16(p.scale * v[8 * q4 + 6], p.scale * v[8 * q4 + 7]));
+                                 pack_bf16(mul * v[8 * q4], mul * v[8 * q4 + 1]), pack_bf16(mul * v[8 * q4 + 2], mul * v[8 * q4 + 3]),
+                                 pack_bf16(mul * v[8 * q4 + 4], mul * v[8 * q4 + 5]), pack_bf16(mul * v[8 * q4 + 6], mul * v[8 * q4 + 7]));
             }
             fence_proxy_async();
             asm volatile("bar.sync 1, 128;" ::: "memory");

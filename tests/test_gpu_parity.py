@@ -185,6 +185,33 @@ def test_normalizer_readout(G):
     assert rel_err(S_out.cpu(), S_ref) <= TOL_FP32 and rel_err(z.cpu(), z_ref) <= TOL_FP32
 
 
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("B,H,G,F", [(1, 2, 352, 2), (2, 3, 880, 3), (1, 20, 256, 1)])
+def test_normalizer_readout_tensor_core_frame_path(d, B, H, G, F):
+    """Paper Eq. 20-22 on the tcgen05 frame path (bf16): the z recurrence runs through the same three kernels as
+    column 0 of a matrix state; out = scale q S / (q_raw . z + eps).  z updated in place."""
+    import oracle
+    T = G * F
+    wl = gin.GdnWorkload("norm_tc", B, H, T, d, d, group=G, seed=31)
+    inp = gin.make_normalizer_inputs(wl)
+    dev = torch.device("cuda:0")
+    ex = inp.extras
+    out = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+    S_out = torch.empty(B, H, d, d, device=dev)
+    z = ex["z_in"].to(dev)
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d, group=G, scale=0.5, flags=gdn.GDN_FLAG_NORMALIZER) as p:
+        assert gdn.PATH_NAMES[p.info.path] == "tc_frame"
+        for _ in range(2):                                        # the second call must not depend on leftovers of the first
+            z.copy_(ex["z_in"])
+            p.forward_norm(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), ex["q_raw"].to(dev), ex["k_raw"].to(dev),
+                           inp.alpha.to(dev), inp.beta.to(dev), inp.state.to(dev), z, out, S_out, z)
+            torch.cuda.synchronize()
+    o_ref, S_ref, z_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=G, scale=0.5,
+                                             q_raw=ex["q_raw"], k_raw=ex["k_raw"], z_in=ex["z_in"], normalizer=True)
+    assert rel_err(out.cpu(), o_ref) <= TOL_BF16
+    assert rel_err(S_out.cpu(), S_ref) <= TOL_BF16 and rel_err(z.cpu(), z_ref) <= TOL_BF16
+
+
 # ---- streaming carry: split invariance on the device path -------------------------------------------
 @pytest.mark.parametrize("G", [1, 32])
 def test_split_invariance_device(G):
