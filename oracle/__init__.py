@@ -47,6 +47,8 @@ def _load():
         lib.gdn_oracle_forward.argtypes = [ctypes.c_int] * 6 + [fp, sp] * 5 + [fp, fp, dp, dp,
                                           ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                           dp, dp, dp, ctypes.c_int]
+        lib.gdn_oracle_forward_bidir.restype = ctypes.c_int
+        lib.gdn_oracle_forward_bidir.argtypes = lib.gdn_oracle_forward.argtypes
         lib.gdn_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -85,8 +87,10 @@ def _ptr_strides(a):
 
 def gdn_forward(q, k, v, alpha, beta, S_in=None, *, group: int = 1, scale: float = 1.0,
                 q_raw=None, k_raw=None, z_in=None, eps: float = 1e-6, normalizer: bool = False,
-                nthreads: int = 0):
-    """Run the oracle.
+                bidir: bool = False, nthreads: int = 0):
+    """Run the oracle.  ``bidir``: the bidirectional in-chunk scan of PAPER.md Alg. 1 lines 8-22 (forward scan from
+    the cache plus a reverse scan over the frames of this call, one readout on the summed histories); S_out / z_out
+    stay the forward terminal states.
 
     q,k: [B,T,H,d_k]; v: [B,T,H,d_v]; alpha: [B,H,T/group]; beta: [B,H,T]; S_in: [B,H,d_k,d_v] or None.
     Returns (out [B,T,H,d_v] fp64, S_out [B,H,d_k,d_v] fp64) and, with ``normalizer``, also z_out.
@@ -130,7 +134,7 @@ def gdn_forward(q, k, v, alpha, beta, S_in=None, *, group: int = 1, scale: float
              z_in.ctypes.data_as(dp) if z_in is not None else ctypes.cast(None, dp),
              float(scale), float(eps), int(bool(normalizer)),
              out.ctypes.data_as(dp), S_out.ctypes.data_as(dp), z_out.ctypes.data_as(dp), int(nthreads)]
-    rc = lib.gdn_oracle_forward(*args)
+    rc = (lib.gdn_oracle_forward_bidir if bidir else lib.gdn_oracle_forward)(*args)
     if rc != 0:
         raise RuntimeError(f"gdn_oracle_forward failed with code {rc}")
     if normalizer:

@@ -282,3 +282,112 @@ def test_state_none_equals_zeros():
     o1, s1 = oracle.gdn_forward(q, k, v, a, b, None)
     o2, s2 = oracle.gdn_forward(q, k, v, a, b, np.zeros_like(S0))
     assert np.array_equal(o1, o2) and np.array_equal(s1, s2)
+
+
+# ---- bidirectional in-chunk scan (Alg. 1 lines 8-22, L337-L359; L122, L145) ----------------------
+def _dense_alg1(q, k, v, alpha, beta, S0, G, q_raw=None, k_raw=None, z0=None, eps=1e-6, scale=1.0):
+    """Alg. 1 written with explicit frame summaries (Eq. 4-5): P_f = I - K^T diag(beta) K, A_f = K^T diag(beta) V,
+    forward / reverse recursions on the matrices, one readout on the summed histories.  One stream, fp64."""
+    T, dk = q.shape
+    F = T // G
+    P, A, Pz, bz = [], [], [], []
+    for f in range(F):
+        sl = slice(f * G, (f + 1) * G)
+        Bm = np.diag(beta[sl])
+        P.append(np.eye(dk) - k[sl].T @ Bm @ k[sl])
+        A.append(k[sl].T @ Bm @ v[sl])
+        if k_raw is not None:
+            Pz.append(np.eye(dk) - k_raw[sl].T @ Bm @ k_raw[sl])
+            bz.append(k_raw[sl].T @ beta[sl])
+    fwd, S = [], S0.copy()
+    for f in range(F):
+        S = alpha[f] * P[f] @ S + A[f]
+        fwd.append(S)
+    rev = [None] * F
+    rev[F - 1] = np.zeros_like(S0)
+    for f in range(F - 1, 0, -1):
+        rev[f - 1] = alpha[f] * P[f] @ rev[f] + A[f]
+    if k_raw is not None:
+        zf, z = [], z0.copy()
+        for f in range(F):
+            z = alpha[f] * Pz[f] @ z + bz[f]
+            zf.append(z)
+        zr = [None] * F
+        zr[F - 1] = np.zeros_like(z0)
+        for f in range(F - 1, 0, -1):
+            zr[f - 1] = alpha[f] * Pz[f] @ zr[f] + bz[f]
+    out = np.empty((T, v.shape[1]))
+    for f in range(F):
+        sl = slice(f * G, (f + 1) * G)
+        num = scale * q[sl] @ (fwd[f] + rev[f])
+        if k_raw is not None:
+            num = num / (q_raw[sl] @ (zf[f] + zr[f]) + eps)[:, None]
+        out[sl] = num
+    return out, fwd[-1], (zf[-1] if k_raw is not None else None)
+
+
+@pytest.mark.parametrize("G,F", [(1, 5), (3, 4), (8, 3)])
+def test_bidir_matches_dense_algorithm_1(G, F):
+    q, k, v, alpha, beta, S0 = make(40 + G, G * F, 5, 4, G=G, H=2)
+    out, S = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=G, scale=0.7, bidir=True)
+    for h in range(2):
+        o_ref, S_ref, _ = _dense_alg1(stream(q, 0, h), stream(k, 0, h), stream(v, 0, h), alpha[0, h].astype(np.float64),
+                                      beta[0, h].astype(np.float64), S0[0, h], G, scale=0.7)
+        assert np.abs(out[0, :, h] - o_ref).max() < 1e-12 and np.abs(S[0, h] - S_ref).max() < 1e-12
+
+
+def test_bidir_with_normaliser_matches_dense_algorithm_1():
+    G, F, dk = 4, 3, 6
+    r = rnd(77)
+    q, k, v, alpha, beta, S0 = make(41, G * F, dk, 3, G=G)
+    q_raw = np.abs(r.standard_normal(q.shape)).astype(np.float32)
+    k_raw = (np.abs(r.standard_normal(k.shape)) / np.sqrt(dk * G)).astype(np.float32)
+    z0 = np.abs(r.standard_normal((1, 1, dk)))
+    out, S, z = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=G, q_raw=q_raw, k_raw=k_raw, z_in=z0, normalizer=True, bidir=True)
+    o_ref, S_ref, z_ref = _dense_alg1(stream(q), stream(k), stream(v), alpha[0, 0].astype(np.float64), beta[0, 0].astype(np.float64),
+                                      S0[0, 0], G, q_raw=stream(q_raw), k_raw=stream(k_raw), z0=z0[0, 0])
+    assert np.abs(out[0, :, 0] - o_ref).max() < 1e-12 and np.abs(S[0, 0] - S_ref).max() < 1e-12 and np.abs(z[0, 0] - z_ref).max() < 1e-12
+
+
+def test_bidir_single_frame_is_the_forward_scan_and_last_frame_never_changes():
+    q, k, v, alpha, beta, S0 = make(42, 12, 4, 4, G=12)
+    o1, s1 = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=12)
+    o2, s2 = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=12, bidir=True)
+    assert np.array_equal(o1, o2) and np.array_equal(s1, s2)                    # F = 1: S<_0 = 0
+    q, k, v, alpha, beta, S0 = make(43, 12, 4, 4, G=4)
+    o1, s1 = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=4)
+    o2, s2 = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=4, bidir=True)
+    assert np.array_equal(s1, s2) and np.array_equal(o1[:, 8:], o2[:, 8:])      # the cache and the last frame are forward-only
+    assert np.abs(o1[:, :8] - o2[:, :8]).max() > 1e-2                           # negative control: earlier frames see the future
+
+
+def test_bidir_two_frames_closed_form():
+    """F = 2: S<_0 = alpha_1 P_1 0 + A_1 = K_1^T diag(beta_1) V_1, so frame 0 reads S>_0 + A_1."""
+    G = 5
+    q, k, v, alpha, beta, S0 = make(44, 2 * G, 4, 3, G=G)
+    out, _ = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=G, bidir=True)
+    _, S_f0 = oracle.gdn_forward(q[:, :G], k[:, :G], v[:, :G], alpha[:, :, :1], beta[:, :, :G], S0, group=G)   # forward state after frame 0
+    K1, V1 = stream(k)[G:], stream(v)[G:]
+    A1 = K1.T @ np.diag(beta[0, 0, G:].astype(np.float64)) @ V1
+    assert np.abs(out[0, :G, 0] - stream(q)[:G] @ (S_f0[0, 0] + A1)).max() < 1e-12
+
+
+def test_bidir_reverse_history_is_the_forward_scan_of_the_reversed_chunk():
+    """S<_f is what a forward scan from zero over the frames F-1, F-2, ..., f+1 (in that order) leaves behind, so with
+    the unidirectional oracle (pinned above) run on prefixes of the chunk and of the frame-reversed chunk:
+    out_f = q_f (S>_f + S'>_{F-2-f})."""
+    G, F, dk = 3, 4, 4
+    q, k, v, alpha, beta, S0 = make(45, G * F, dk, 5, G=G)
+    out, _ = oracle.gdn_forward(q, k, v, alpha, beta, S0, group=G, bidir=True)
+    def rev_frames(x, axis):
+        idx = np.concatenate([np.arange(f * G, (f + 1) * G) for f in range(F - 1, -1, -1)])
+        return np.take(x, idx, axis=axis)
+    kr, vr, br, ar = rev_frames(k, 1), rev_frames(v, 1), rev_frames(beta, 2), alpha[:, :, ::-1].copy()
+    for f in range(F):
+        _, Sf = oracle.gdn_forward(q[:, :(f + 1) * G], k[:, :(f + 1) * G], v[:, :(f + 1) * G], alpha[:, :, :f + 1], beta[:, :, :(f + 1) * G], S0, group=G)
+        n = F - 1 - f                                                           # frames after f, scanned from the far end
+        Sb = np.zeros_like(S0)
+        if n > 0:
+            _, Sb = oracle.gdn_forward(q[:, :n * G], kr[:, :n * G], vr[:, :n * G], ar[:, :, :n], br[:, :, :n * G], None, group=G)
+        ref = stream(q)[f * G:(f + 1) * G] @ (Sf[0, 0] + Sb[0, 0])
+        assert np.abs(out[0, f * G:(f + 1) * G, 0] - ref).max() < 1e-12
