@@ -54,7 +54,9 @@ typedef enum { GDN_BF16 = 0, GDN_FP32 = 1 } gdn_dtype_t;     /* element type of 
 
 enum {
     GDN_FLAG_NORMALIZER = 1u,  /* also run the z path and divide (gdn_forward_chunk_norm only)          */
-    GDN_FLAG_BIDIR      = 2u,  /* in-chunk reverse scan (Alg. 1 l.14-22); NOT implemented -> UNSUPPORTED */
+    GDN_FLAG_BIDIR      = 2u,  /* bidirectional in-chunk scan (Alg. 1 l.8-22): forward scan from the cache + reverse scan over the
+                                  frames of this call, readout on S> + S<; state_out stays the forward terminal state.
+                                  Frame-wise bf16 tensor-core plans only, else UNSUPPORTED */
     GDN_FLAG_LOG_ALPHA  = 4u,  /* `alpha` holds log(alpha) (<= 0) instead of alpha in (0,1]             */
     GDN_FLAG_FORCE_SIMT = 8u,  /* use the fp32 CUDA-core kernel even where a tensor-core path exists    */
     GDN_FLAG_UNFUSED    = 16u  /* token-wise tensor-core path as three kernels (prepass / chain / output)

@@ -180,7 +180,10 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
     if (c.flags & ~known) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown flag bits");
     if (!head_dim_ok(c.d_k) || !head_dim_ok(c.d_v))
         return fail(nullptr, GDN_ERR_UNSUPPORTED, "d_k and d_v must each be 32, 64 or 128 (112 via padding is not implemented)");
-    if (c.flags & GDN_FLAG_BIDIR) return fail(nullptr, GDN_ERR_UNSUPPORTED, "GDN_FLAG_BIDIR (in-chunk reverse scan) is not implemented");
+    // the bidirectional in-chunk scan exists on the frame-wise tensor-core path only (the paper's case, Alg. 1)
+    if ((c.flags & GDN_FLAG_BIDIR) && !(c.group > 1 && c.io_dtype == GDN_BF16 && c.d_k == c.d_v && (c.d_k == 64 || c.d_k == 128) &&
+                                        !(c.flags & GDN_FLAG_FORCE_SIMT)))
+        return fail(nullptr, GDN_ERR_UNSUPPORTED, "GDN_FLAG_BIDIR needs a frame-wise (group > 1) bf16 plan with d_k = d_v in {64,128}");
     const long long strides[4] = {c.q_token_stride, c.k_token_stride, c.v_token_stride, c.o_token_stride};
     const int dims[4] = {c.d_k, c.d_k, c.d_v, c.d_v};
     for (int i = 0; i < 4; ++i) {

@@ -40,6 +40,10 @@ struct TcPlan {
     int HPR = 0, NWC = 0, grid = 0;
     // normaliser on the frame path: z as column 0 of a [D][D] fp32 state, den = q_raw . z per token
     float *Sz = nullptr, *den = nullptr;
+    // bidirectional in-chunk scan: reverse-scan snapshots S<_f, bf16 [BH][F][D][D]
+    bool bidir = false;
+    __nv_bfloat16* ScR = nullptr;
+    CUtensorMap tmScR;
     const void *cqr = nullptr, *ckr = nullptr;
     CUtensorMap tmQr, tmKr;
 };
@@ -100,6 +104,8 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
     const bool norm = (c.flags & GDN_FLAG_NORMALIZER) != 0;
     const size_t oSz = norm ? carve(BH * D * D * 4) : 0, oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
+    tp.bidir = (c.flags & GDN_FLAG_BIDIR) != 0;
+    const size_t oScR = tp.bidir ? carve(BH * F * D * D * 2) : 0;
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -114,6 +120,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
     if (norm) { tp.Sz = reinterpret_cast<float*>(w + oSz); tp.den = reinterpret_cast<float*>(w + oDen); }
+    if (tp.bidir) tp.ScR = reinterpret_cast<__nv_bfloat16*>(w + oScR);
     if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "counter initialisation failed";
@@ -127,6 +134,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
         const uint64_t dimsS[3] = {D, D, BH * (F + 1)};
         ok = ok && tc::make_tmap(&tp.tmSc, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
         ok = ok && tc::make_tmap(&tp.tmScS, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        if (tp.bidir) ok = ok && tc::make_tmap(&tp.tmScR, tp.ScR, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
     {
         const uint64_t dims[3] = {D, D, BH * F}, str[3] = {4, D * 4, D * D * 4};
@@ -324,6 +332,19 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     cudaError_t le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_chain");
+    if (tp.bidir && tp.F > 1) {
+        // Alg. 1 l.14-21: reverse scan over the frames F-1 .. 1 from a zero state, then S^hist = S> + S< in place
+        TokParams rp = cp;
+        rp.rev = 1; rp.NCa = tp.F; rp.NC = tp.F - 1; rp.NSc = tp.F; rp.S_in = nullptr; rp.S_out = nullptr;
+        le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScR, rp);
+        if (le != cudaSuccess) return le;
+        if (prof) prof->mark(st, "gdn_tok_chain(rev)");
+        const long long total8 = (long long)tp.BH * tp.F * D * D / 8;
+        const int blocks = (int)((total8 + 255) / 256 < 4 * sms ? (total8 + 255) / 256 : 4 * sms);
+        le = launch_pdl(gdn_frm_hist_add, dim3(blocks), dim3(256), 0, st, tp.Sc, (const __nv_bfloat16*)tp.ScR, tp.F, D * D / 8, total8);
+        if (le != cudaSuccess) return le;
+        if (prof) prof->mark(st, "gdn_frm_hist_add");
+    }
     le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
@@ -358,7 +379,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
         TokParams cp{};
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
-        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
+        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
         cudaError_t e = cudaSuccess;
         if (na) {
             // z pass (Eq. 20-21 through the same three kernels): K_raw summaries with the constant block as V, the scan on
@@ -391,7 +412,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     TokParams p{};
     p.alpha = alpha; p.beta = beta; p.S_in = S_in; p.S_out = S_out; p.out = out;
     p.Gw = tp.Gw; p.Nw = tp.Nw; p.gam = tp.gam; p.Qt = tp.Qt; p.Ol = tp.Ol; p.Sc = tp.Sc;
-    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC; p.NSc = tp.NSc;
+    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC; p.NCa = tp.NC; p.NSc = tp.NSc;
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;

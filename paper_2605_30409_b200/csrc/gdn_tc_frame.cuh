@@ -329,6 +329,31 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Bidirectional in-chunk scan (Alg. 1 l.19-21): S^hist_f = S>_f + S<_f.  The forward snapshot of frame f (slot f + 1
+// of Sc, bf16) takes the reverse scan's S<_f (slot f of ScR) in place, so Phase C reads the summed history with no
+// second output pass.  8 bf16 per thread and step.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+gdn_frm_hist_add(__nv_bfloat16* Sc, const __nv_bfloat16* ScR, int F, int DD8, long long total8) {
+    pdl_launch_dependents();
+    pdl_wait();                                    // both scans are complete
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total8; e += (long long)gridDim.x * blockDim.x) {
+        const long long bhf = e / DD8;
+        const int within = (int)(e % DD8), f = (int)(bhf % F);
+        const long long bh = bhf / F;
+        uint4* dst = reinterpret_cast<uint4*>(Sc) + (bh * (F + 1) + f + 1) * DD8 + within;
+        const uint4 r = __ldcg(reinterpret_cast<const uint4*>(ScR) + bhf * DD8 + within);
+        const uint4 a = __ldcg(dst);
+        float x[8], y[8];
+        unpack8(a, x); unpack8(r, y);
+        uint4 o;
+        o.x = pack_bf16(x[0] + y[0], x[1] + y[1]); o.y = pack_bf16(x[2] + y[2], x[3] + y[3]);
+        o.z = pack_bf16(x[4] + y[4], x[5] + y[5]); o.w = pack_bf16(x[6] + y[6], x[7] + y[7]);
+        *dst = o;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Phase C.  grid = min(#SM, tiles), block = 192.   O = scale * Q_f S_f   (S_f = snapshot slot f + 1)
 //   CTA c runs the contiguous tile range [c n / grid, (c+1) n / grid) of the (b,h,f,tile) order.
 // ---------------------------------------------------------------------------------------------------

@@ -38,6 +38,10 @@ struct TokParams {
     __nv_bfloat16* Sc;           // [BH][NC][D][D]     state at chunk start (bf16 MMA operand)
     int B, H, T, NT, NC;
     int NSc;                     // snapshot slots per (b,h) in Sc: NC (token-wise) or NC + 1 (frame-wise: also the final state)
+    // chain kernel only.  NCa = entries per (b,h) in Gw / Nw / gam (= NC except for the reverse scan of the bidirectional
+    // frame path, Alg. 1 l.14-17: rev = 1 runs NC = NCa - 1 steps over the entries NCa-1, NCa-2, ..., 1 from a zero
+    // state and stores the state BEFORE entry e is applied (= S<_e) in snapshot slot e; S_out may be NULL).
+    int NCa, rev;
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
@@ -744,11 +748,12 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
     pdl_launch_dependents();
     pdl_wait();                                    // the summaries of the previous kernel are complete
 
+    auto ent = [&](int c) { return p.rev ? p.NCa - 1 - c : c; };      // summary entry of step c / snapshot slot of state c
     auto issue_loads = [&](int c) {
         const int st = c % STAGES;
         uint8_t* base = sStage + st * L::STAGE;
         mbar_expect_tx(&bars[st], L::STAGE);
-        const int z = bh * p.NC + c;
+        const int z = bh * p.NCa + ent(c);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) tma_load_3d(base + nb * (D * 128), &tmG, &bars[st], nb * 64, 0, z);
         tma_load_3d(base + L::G_BYTES, &tmN, &bars[st], n0, 0, z);
@@ -805,7 +810,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
         //       operand tile sS (= state at the start of chunk c) to the workspace for kernel 3 with one TMA
         //       store straight from shared memory (no per-thread global stores on the chain) =====
         auto store_snapshot = [&](int c) {           // sS[c & 1] holds the state at the start of chunk c
-            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + c);
+            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + ent(c));
             tma_store_commit();
         };
         if (lane == 0) store_snapshot(0);
@@ -821,11 +826,11 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
     } else {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
         uint32_t ph_mma = 0;
-        float gamma_c = p.gam[(long long)bh * p.NC];
+        float gamma_c = p.NC > 0 ? p.gam[(long long)bh * p.NCa + ent(0)] : 0.f;
         for (int c = 0; c < p.NC; ++c) {
             const int st = c % STAGES;
             uint8_t* base = sStage + st * L::STAGE;
-            const float gamma_next = (c + 1 < p.NC) ? p.gam[(long long)bh * p.NC + c + 1] : 0.f;
+            const float gamma_next = (c + 1 < p.NC) ? p.gam[(long long)bh * p.NCa + ent(c + 1)] : 0.f;
             if (c == 10) GDN_STAMP(32);
             if (c == 10) GDN_STAMP(33);
             mbar_wait(&bars[st], (uint32_t)(c / STAGES) & 1u);
@@ -863,7 +868,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
             if (c == 10) GDN_STAMP(38);
             gamma_c = gamma_next;
         }
-        if (m_ok) {
+        if (m_ok && p.S_out) {
             float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + n0);
 #pragma unroll
             for (int i = 0; i < 16; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);

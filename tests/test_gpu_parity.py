@@ -212,6 +212,59 @@ def test_normalizer_readout_tensor_core_frame_path(d, B, H, G, F):
     assert rel_err(S_out.cpu(), S_ref) <= TOL_BF16 and rel_err(z.cpu(), z_ref) <= TOL_BF16
 
 
+# ---- bidirectional in-chunk scan (Alg. 1 l.8-22) on the frame path ------------------------------------
+@pytest.mark.parametrize("d", [64, 128])
+@pytest.mark.parametrize("B,H,G,F", [(1, 2, 256, 1), (1, 3, 352, 2), (2, 2, 880, 3), (1, 20, 200, 5)])
+def test_bidirectional_frame_path(d, B, H, G, F):
+    T = G * F
+    wl = gin.GdnWorkload("bidir", B, H, T, d, d, group=G, seed=51)
+    inp = gin.make_inputs(wl)
+    out, S, info = run_cuda(inp, flags=gdn.GDN_FLAG_BIDIR, scale=0.8)
+    assert gdn.PATH_NAMES[info[0]] == "tc_frame"
+    import oracle
+    o_ref, S_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=G, scale=0.8, bidir=True)
+    assert rel_err(out, o_ref) <= TOL_BF16 and rel_err(S, S_ref) <= TOL_BF16
+    if F > 1:                                                   # negative control: the forward-only result is far away
+        o_fwd, _ = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=G, scale=0.8)
+        assert rel_err(out, o_fwd) > 5 * TOL_BF16
+
+
+def test_bidirectional_stream_with_normaliser_carries_forward_states():
+    """Two chunks of the paper's shape (3 frames of 880 tokens, 20 heads, d = 128), bidirectional + normalised
+    readout; the carried S and z are the FORWARD terminal states (L145: forward scan with the previous cache)."""
+    import oracle
+    B, H, G, F, d = 1, 20, 880, 3, 128
+    T = G * F
+    dev = torch.device("cuda:0")
+    S_d = z_d = None
+    S_o = z_o = None
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d, group=G, flags=gdn.GDN_FLAG_NORMALIZER | gdn.GDN_FLAG_BIDIR) as p:
+        for ci in range(2):
+            wl = gin.GdnWorkload("bidir_norm", B, H, T, d, d, group=G, seed=60 + ci)
+            inp = gin.make_normalizer_inputs(wl)
+            ex = inp.extras
+            if ci == 0:
+                S_d, z_d = inp.state.to(dev), ex["z_in"].to(dev)
+                S_o, z_o = inp.state, ex["z_in"]
+            out = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+            p.forward_norm(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), ex["q_raw"].to(dev), ex["k_raw"].to(dev),
+                           inp.alpha.to(dev), inp.beta.to(dev), S_d, z_d, out, S_d, z_d)
+            torch.cuda.synchronize()
+            o_ref, S_o, z_o = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, S_o, group=G, q_raw=ex["q_raw"],
+                                                 k_raw=ex["k_raw"], z_in=z_o, normalizer=True, bidir=True)
+            assert rel_err(out.cpu(), o_ref) <= TOL_BF16
+            assert rel_err(S_d.cpu(), S_o) <= TOL_BF16 and rel_err(z_d.cpu(), z_o) <= TOL_BF16
+
+
+def test_bidirectional_flag_is_refused_where_it_has_no_path():
+    for kw in (dict(group=1), dict(group=64, io_dtype=gdn.GDN_FP32), dict(group=64, d_k=32, d_v=32)):
+        args = dict(B=1, H=2, T=256, d_k=64, d_v=64, flags=gdn.GDN_FLAG_BIDIR)
+        args.update(kw)
+        with pytest.raises(gdn.GdnError) as ei:
+            gdn.GdnPlan(**args)
+        assert ei.value.status == gdn.GDN_ERR_UNSUPPORTED
+
+
 # ---- streaming carry: split invariance on the device path -------------------------------------------
 @pytest.mark.parametrize("G", [1, 32])
 def test_split_invariance_device(G):
