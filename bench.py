@@ -40,6 +40,8 @@ def peaks():
 
 def workload(args):
     from paper_2605_30409_b200 import inputs as gin
+    if args.paper_shape:
+        return gin.paper_shape(3)                  # 3 x 880 tokens, 20 heads, d = 128
     wl = gin.config(args.config, frame=(args.mode == "frame"), chunk=args.chunk)
     return wl
 
@@ -147,7 +149,8 @@ def run_reference(args):
 
 
 def config_dict(wl, info, extra=None):
-    d = {"workload": f"BASELINE.json configs[{int(wl.name[3]) - 1}] ({wl.name}): B={wl.B} H={wl.H} T={wl.T} "
+    src = f"BASELINE.json configs[{int(wl.name[3]) - 1}]" if wl.name.startswith("cfg") else "the paper's production chunk"
+    d = {"workload": f"{src} ({wl.name}): B={wl.B} H={wl.H} T={wl.T} "
                      f"d_k=d_v={wl.d_k} {str(wl.dtype).split('.')[-1]}, "
                      + ("token-wise (G=1)" if wl.group == 1 else f"frame-wise (G={wl.group})"),
          "B": wl.B, "H": wl.H, "T": wl.T, "d_k": wl.d_k, "d_v": wl.d_v, "group": wl.group,
@@ -220,20 +223,34 @@ def run_ours(args):
     set_bytes = wl.B * wl.T * wl.H * (2 * wl.d_k + 2 * wl.d_v) * es
     n_sets = max(2, int(L2_BYTES * 1.5 // set_bytes) + 1)         # rotate so the inputs of a step are cold in L2
     n_sets = min(n_sets, 16)
+    norm = bool(args.normalizer)
+    if norm:
+        set_bytes += wl.B * wl.T * wl.H * 2 * wl.d_k * es
+        n_sets = min(16, max(2, int(L2_BYTES * 1.5 // set_bytes) + 1))
     sets = []
     for i in range(n_sets):
-        inp = gin.make_inputs(wl, seed=rank_seed(wl, rank, i))
-        sets.append(dict(q=inp.q.to(dev), k=inp.k.to(dev), v=inp.v.to(dev), alpha=inp.alpha.to(dev),
-                         beta=inp.beta.to(dev), out=torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=wl.dtype, device=dev)))
-    state = gin.make_inputs(wl).state.to(dev)
-    plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, chunk=wl.chunk,
+        inp = (gin.make_normalizer_inputs if norm else gin.make_inputs)(wl, seed=rank_seed(wl, rank, i))
+        d = dict(q=inp.q.to(dev), k=inp.k.to(dev), v=inp.v.to(dev), alpha=inp.alpha.to(dev),
+                 beta=inp.beta.to(dev), out=torch.empty(wl.B, wl.T, wl.H, wl.d_v, dtype=wl.dtype, device=dev))
+        if norm:
+            d.update(q_raw=inp.extras["q_raw"].to(dev), k_raw=inp.extras["k_raw"].to(dev))
+        sets.append(d)
+    first = (gin.make_normalizer_inputs if norm else gin.make_inputs)(wl)
+    state = first.state.to(dev)
+    zstate = first.extras["z_in"].to(dev) if norm else None
+    flags = (gdn.GDN_FLAG_NORMALIZER if norm else 0) | (gdn.GDN_FLAG_BIDIR if args.bidir else 0)
+    plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, chunk=wl.chunk, flags=flags,
                        io_dtype=gdn.GDN_BF16 if wl.dtype == torch.bfloat16 else gdn.GDN_FP32)
     info = plan.info
     stream = torch.cuda.current_stream()
 
     def step(i):
         s = sets[i % n_sets]
-        plan.forward(s["q"], s["k"], s["v"], s["alpha"], s["beta"], state, s["out"], state, stream)
+        if norm:
+            plan.forward_norm(s["q"], s["k"], s["v"], s["q_raw"], s["k_raw"], s["alpha"], s["beta"], state, zstate,
+                              s["out"], state, zstate, stream=stream)
+        else:
+            plan.forward(s["q"], s["k"], s["v"], s["alpha"], s["beta"], state, s["out"], state, stream)
 
     def barrier():
         if dist is not None:
@@ -262,7 +279,7 @@ def run_ours(args):
 
     # ---- end to end through the host entry point (pinned host buffers, copies inside the timing) ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not norm:
         inp = gin.make_inputs(wl)
         pin = lambda t: t.contiguous().pin_memory()
         hq, hk, hv, ha, hb, hs = map(pin, (inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state))
@@ -285,6 +302,9 @@ def run_ours(args):
     pk, pk_src = peaks()
     fl = flops_per_call(wl, info.chunk)
     by = bytes_per_call(wl)
+    if norm:                                       # + 2 d^2 flops and + 4 d bytes per token-head (q_raw, k_raw), + z in/out
+        fl += wl.B * wl.H * wl.T * 2 * wl.d_k * wl.d_k
+        by += wl.B * wl.H * wl.T * 2 * wl.d_k * es + 2 * wl.B * wl.H * wl.d_k * 4
     tflops = fl / (ms_per_step * 1e-3) / 1e12
     roof = roofline(wl, info, kernels, ms_per_step, pk, pk_src, by)
     line = {
@@ -298,7 +318,9 @@ def run_ours(args):
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * info.launches_per_call,
         "roofline": roof, "kernels": kernels,
     }
-    if rank == 0 and world == 1 and not args.no_cpu:
+    if norm or args.bidir:
+        line["config"]["variant"] = "+".join(x for x, on in (("normalizer", norm), ("bidir", args.bidir)) if on)
+    if rank == 0 and world == 1 and not args.no_cpu and not norm and not args.bidir:
         line["cpu_baseline"] = cpu_baseline(wl)
     plan.close()
     if rank == 0:
@@ -378,6 +400,9 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 5])
     ap.add_argument("--mode", default="token", choices=["token", "frame"])
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--normalizer", action="store_true", help="frame mode: the paper's normalised readout (Eq. 20-22)")
+    ap.add_argument("--bidir", action="store_true", help="frame mode: bidirectional in-chunk scan (Alg. 1)")
+    ap.add_argument("--paper-shape", action="store_true", help="3 x 880 tokens, 20 heads, d = 128, frame-wise")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

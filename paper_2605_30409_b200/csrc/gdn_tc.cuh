@@ -5,6 +5,7 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <new>
 #include <string>
 #include <utility>
 #include <vector>
@@ -38,8 +39,11 @@ struct TcPlan {
     unsigned int* flags = nullptr;
     unsigned int epoch = 0;
     int HPR = 0, NWC = 0, grid = 0;
-    // normaliser on the frame path: z as column 0 of a [D][D] fp32 state, den = q_raw . z per token
-    float *Sz = nullptr, *den = nullptr;
+    // normaliser on the frame path: z as column 0 of the chain kernel's state, den = q_raw . z per token
+    float* den = nullptr;
+    TcPlan* zplan = nullptr;                   // the z pass runs concurrently on its own workspace, stream and events
+    cudaStream_t zs = nullptr;
+    cudaEvent_t zev0 = nullptr, zev1 = nullptr;
     // bidirectional in-chunk scan: reverse-scan snapshots S<_f, bf16 [BH][F][D][D]
     bool bidir = false;
     __nv_bfloat16* ScR = nullptr;
@@ -103,7 +107,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     const size_t oP = carve(NS > 1 ? BH * F * NS * D * 2 * D * 4 : 16), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
     const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
     const bool norm = (c.flags & GDN_FLAG_NORMALIZER) != 0;
-    const size_t oSz = norm ? carve(BH * D * D * 4) : 0, oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
+    const size_t oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
     tp.bidir = (c.flags & GDN_FLAG_BIDIR) != 0;
     const size_t oScR = tp.bidir ? carve(BH * F * D * D * 2) : 0;
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
@@ -119,7 +123,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.gam = reinterpret_cast<float*>(w + oGam);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
-    if (norm) { tp.Sz = reinterpret_cast<float*>(w + oSz); tp.den = reinterpret_cast<float*>(w + oDen); }
+    if (norm) tp.den = reinterpret_cast<float*>(w + oDen);
     if (tp.bidir) tp.ScR = reinterpret_cast<__nv_bfloat16*>(w + oScR);
     if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
@@ -142,6 +146,21 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
         ok = ok && tc::make_tmap(&tp.tmN, tp.Nw, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
     if (!ok) { cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
+    if (norm) {
+        tp.zplan = new (std::nothrow) TcPlan();
+        gdn_config_t zc = c;
+        zc.flags &= ~(uint32_t)GDN_FLAG_NORMALIZER;
+        gdn_status_t zs = tp.zplan ? tc_plan_init_frame(*tp.zplan, zc, sm_count, err) : GDN_ERR_NOMEM;
+        if (zs == GDN_OK && (cudaStreamCreateWithFlags(&tp.zs, cudaStreamNonBlocking) != cudaSuccess ||
+                             cudaEventCreateWithFlags(&tp.zev0, cudaEventDisableTiming) != cudaSuccess ||
+                             cudaEventCreateWithFlags(&tp.zev1, cudaEventDisableTiming) != cudaSuccess)) {
+            cudaGetLastError();
+            if (err) *err = "normaliser stream / event creation failed";
+            zs = GDN_ERR_CUDA;
+        }
+        if (zs != GDN_OK) { cudaFree(tp.workspace); tp.workspace = nullptr; return zs; }
+        tp.workspace_bytes += tp.zplan->workspace_bytes;
+    }
     tp.ready = true;
     return GDN_OK;
 }
@@ -240,6 +259,11 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
 }
 
 inline void tc_plan_free(TcPlan& tp) {
+    if (tp.zplan) { tc_plan_free(*tp.zplan); delete tp.zplan; tp.zplan = nullptr; }
+    if (tp.zs) cudaStreamDestroy(tp.zs);
+    if (tp.zev0) cudaEventDestroy(tp.zev0);
+    if (tp.zev1) cudaEventDestroy(tp.zev1);
+    tp.zs = nullptr; tp.zev0 = tp.zev1 = nullptr;
     if (tp.workspace) cudaFree(tp.workspace);
     tp.workspace = nullptr;
     tp.ready = false;
@@ -311,7 +335,8 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
 
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
-                                   const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof) {
+                                   const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
+                                   cudaEvent_t before_readout = nullptr) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -320,6 +345,7 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     if (!attr_done) {
         cudaError_t e = set_smem(gdn_frm_summaries<D>, smem1);
         if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain<D>, smem2);
+        if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain_bidir<D>, smem2);
         if (e == cudaSuccess) e = set_smem(gdn_frm_readout<D>, smem3);
         if (e != cudaSuccess) return e;
         attr_done = true;
@@ -329,22 +355,28 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     if (prof) prof->begin(st);
     gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tmK, tmV, fp);
     if (prof) prof->mark(st, "gdn_frm_summaries");
-    cudaError_t le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
-    if (le != cudaSuccess) return le;
-    if (prof) prof->mark(st, "gdn_tok_chain");
+    cudaError_t le;
+    const int nchain = tp.BH * (D / 64);
     if (tp.bidir && tp.F > 1) {
-        // Alg. 1 l.14-21: reverse scan over the frames F-1 .. 1 from a zero state, then S^hist = S> + S< in place
+        // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero
+        // state; then S^hist = S> + S< in place in the forward snapshots
         TokParams rp = cp;
         rp.rev = 1; rp.NCa = tp.F; rp.NC = tp.F - 1; rp.NSc = tp.F; rp.S_in = nullptr; rp.S_out = nullptr;
-        le = launch_pdl(tok::gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScR, rp);
+        rp.z_vec_in = nullptr; rp.z_vec_out = nullptr;              // z< starts from zero as well and is not carried
+        le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScR, cp, rp, nchain);
         if (le != cudaSuccess) return le;
-        if (prof) prof->mark(st, "gdn_tok_chain(rev)");
+        if (prof) prof->mark(st, "gdn_tok_chain_bidir");
         const long long total8 = (long long)tp.BH * tp.F * D * D / 8;
         const int blocks = (int)((total8 + 255) / 256 < 4 * sms ? (total8 + 255) / 256 : 4 * sms);
         le = launch_pdl(gdn_frm_hist_add, dim3(blocks), dim3(256), 0, st, tp.Sc, (const __nv_bfloat16*)tp.ScR, tp.F, D * D / 8, total8);
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_frm_hist_add");
+    } else {
+        le = launch_pdl(tok::gdn_tok_chain<D>, dim3(nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
+        if (le != cudaSuccess) return le;
+        if (prof) prof->mark(st, "gdn_tok_chain");
     }
+    if (before_readout) { le = cudaStreamWaitEvent(st, before_readout, 0); if (le != cudaSuccess) return le; }   // den of the z pass
     le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
@@ -381,31 +413,38 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
         cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
         cudaError_t e = cudaSuccess;
+        cudaEvent_t den_ready = nullptr;
         if (na) {
             // z pass (Eq. 20-21 through the same three kernels): K_raw summaries with the constant block as V, the scan on
-            // a [D][D] state whose column 0 is z, q_raw . z_f per token -> den
+            // a [D][D] state whose column 0 is z, q_raw . z_f per token -> den.  It shares nothing with the matrix pass
+            // until the division in Phase C, so it runs beside it on its own stream and workspace.
+            TcPlan& zt = *tp.zplan;
             if (na->q_raw != tp.cqr || na->k_raw != tp.ckr) {
                 bool ok = tc::make_act_tmap(&tp.tmQr, na->q_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.q_token_stride, c.d_k), 128, err) &&
                           tc::make_act_tmap(&tp.tmKr, na->k_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.k_token_stride, c.d_k), 128, err);
                 if (!ok) { tp.cqr = tp.ckr = nullptr; return GDN_ERR_CUDA; }
                 tp.cqr = na->q_raw; tp.ckr = na->k_raw;
             }
-            const size_t D = tp.D, rows = (size_t)tp.BH * D;
-            e = cudaMemsetAsync(tp.Sz, 0, rows * D * 4, st);
-            if (e == cudaSuccess && na->z_in) e = cudaMemcpy2DAsync(tp.Sz, D * 4, na->z_in, 4, 4, rows, cudaMemcpyDeviceToDevice, st);
-            if (e != cudaSuccess) { if (err) *err = std::string("z state staging: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+            zt.tmO = tp.tmO;                         // unused by the z pass (den_mode 1 stores no tile)
+            e = cudaEventRecord(tp.zev0, st);         // after everything queued on the caller's stream so far
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
+            if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             FrmParams zf = fp;
+            zf.part = zt.part; zf.counters = zt.flags; zf.Gw = zt.Gw; zf.Nw = zt.Nw; zf.gam = zt.gam;
             zf.zpass = 1; zf.den = tp.den; zf.den_mode = 1; zf.scale = 1.f;
             TokParams zc = cp;
-            zc.S_in = tp.Sz; zc.S_out = tp.Sz;
-            e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, st, prof)
-                             : tc_launch_frame<128>(tp, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, st, prof);
-            if (e == cudaSuccess) e = cudaMemcpy2DAsync(na->z_out, 4, tp.Sz, D * 4, 4, rows, cudaMemcpyDeviceToDevice, st);
+            zc.Gw = zt.Gw; zc.Nw = zt.Nw; zc.gam = zt.gam; zc.Sc = zt.Sc;
+            zc.S_in = nullptr; zc.S_out = nullptr;
+            zc.zvec = 1; zc.z_vec_in = na->z_in; zc.z_vec_out = na->z_out;      // z <-> column 0 of the state, in the chain kernel
+            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr)
+                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr);
+            if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
             if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             fp.den = tp.den; fp.den_mode = 2; fp.eps = c.eps;
+            den_ready = tp.zev1;
         }
-        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof)
-                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof);
+        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready)
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

@@ -42,6 +42,11 @@ struct TokParams {
     // frame path, Alg. 1 l.14-17: rev = 1 runs NC = NCa - 1 steps over the entries NCa-1, NCa-2, ..., 1 from a zero
     // state and stores the state BEFORE entry e is applied (= S<_e) in snapshot slot e; S_out may be NULL).
     int NCa, rev;
+    // chain kernel, normaliser z pass: the state is a vector living in column 0 of the matrix state.  z_vec_in [BH][D] (or
+    // NULL = zeros) initialises it instead of S_in, z_vec_out [BH][D] receives it instead of S_out (either may be NULL).
+    int zvec;
+    const float* z_vec_in;
+    float* z_vec_out;
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
@@ -713,9 +718,8 @@ struct ChainSmem {
 constexpr int kChainThreads = 192;     // warps 0-3: state rows (epilogue); warp 4: MMA issuer; warp 5: TMA producer
 
 template <int D>
-__global__ void __launch_bounds__(kChainThreads, 1)
-gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN,
-              const __grid_constant__ CUtensorMap tmSc, const TokParams p) {
+__device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtensorMap* tmNp, const CUtensorMap* tmScp,
+                                           const TokParams& p, const int cta) {
     using L = ChainSmem<D>;
     constexpr int NB = L::NB;
     constexpr int STAGES = L::STAGES;
@@ -728,7 +732,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     constexpr int NT_COL = D / 64;
-    const int ct = blockIdx.x % NT_COL, bh = blockIdx.x / NT_COL;
+    const int ct = cta % NT_COL, bh = cta / NT_COL;
     const int n0 = ct * 64;
     const bool worker = warp < 4;
     const int m = (D == 128) ? tid : (16 * warp + lane);              // state row of a worker thread
@@ -755,16 +759,20 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
         mbar_expect_tx(&bars[st], L::STAGE);
         const int z = bh * p.NCa + ent(c);
 #pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_load_3d(base + nb * (D * 128), &tmG, &bars[st], nb * 64, 0, z);
-        tma_load_3d(base + L::G_BYTES, &tmN, &bars[st], n0, 0, z);
-        tma_load_3d(base + L::G_BYTES + D * 128, &tmN, &bars[st], n0 + 32, 0, z);
+        for (int nb = 0; nb < NB; ++nb) tma_load_3d(base + nb * (D * 128), tmGp, &bars[st], nb * 64, 0, z);
+        tma_load_3d(base + L::G_BYTES, tmNp, &bars[st], n0, 0, z);
+        tma_load_3d(base + L::G_BYTES + D * 128, tmNp, &bars[st], n0 + 32, 0, z);
     };
     if (warp == 5 && lane == 0)
         for (int c = 0; c < STAGES && c < p.NC; ++c) issue_loads(c);
 
     // state row m, columns n0..n0+63, fp32 master copy in registers
     float S[64];
-    if (m_ok && p.S_in) {
+    if (p.zvec) {
+#pragma unroll
+        for (int i = 0; i < 64; ++i) S[i] = 0.f;
+        if (m_ok && ct == 0 && p.z_vec_in) S[0] = p.z_vec_in[(long long)bh * D + m];
+    } else if (m_ok && p.S_in) {
         const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * D + m) * D + n0);
 #pragma unroll
         for (int i = 0; i < 16; ++i) { const float4 f = src[i]; S[4 * i] = f.x; S[4 * i + 1] = f.y; S[4 * i + 2] = f.z; S[4 * i + 3] = f.w; }
@@ -810,7 +818,7 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
         //       operand tile sS (= state at the start of chunk c) to the workspace for kernel 3 with one TMA
         //       store straight from shared memory (no per-thread global stores on the chain) =====
         auto store_snapshot = [&](int c) {           // sS[c & 1] holds the state at the start of chunk c
-            tma_store_3d(&tmSc, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + ent(c));
+            tma_store_3d(tmScp, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + ent(c));
             tma_store_commit();
         };
         if (lane == 0) store_snapshot(0);
@@ -868,7 +876,9 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
             if (c == 10) GDN_STAMP(38);
             gamma_c = gamma_next;
         }
-        if (m_ok && p.S_out) {
+        if (p.zvec) {
+            if (m_ok && ct == 0 && p.z_vec_out) p.z_vec_out[(long long)bh * D + m] = S[0];
+        } else if (m_ok && p.S_out) {
             float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + n0);
 #pragma unroll
             for (int i = 0; i < 16; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
@@ -877,6 +887,24 @@ gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ C
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, 64);
+}
+
+template <int D>
+__global__ void __launch_bounds__(kChainThreads, 1)
+gdn_tok_chain(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN,
+              const __grid_constant__ CUtensorMap tmSc, const TokParams p) {
+    chain_body<D>(&tmG, &tmN, &tmSc, p, (int)blockIdx.x);
+}
+
+// Both scans of the bidirectional frame path in ONE launch (they share the summaries and do not depend on each other,
+// Alg. 1 l.9-17): CTAs [0, n_fwd) run the forward scan `pf` (snapshots -> tmScF), the rest the reverse scan `pr`.
+template <int D>
+__global__ void __launch_bounds__(kChainThreads, 1)
+gdn_tok_chain_bidir(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN,
+                    const __grid_constant__ CUtensorMap tmScF, const __grid_constant__ CUtensorMap tmScR,
+                    const TokParams pf, const TokParams pr, const int n_fwd) {
+    if ((int)blockIdx.x < n_fwd) chain_body<D>(&tmG, &tmN, &tmScF, pf, (int)blockIdx.x);
+    else chain_body<D>(&tmG, &tmN, &tmScR, pr, (int)blockIdx.x - n_fwd);
 }
 
 // ---------------------------------------------------------------------------------------------------
