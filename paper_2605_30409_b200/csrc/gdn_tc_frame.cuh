@@ -119,6 +119,7 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
         mbar_init(bar_done, 1);
         mbar_fence_init();
     }
+    if (tid == 160) { tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV); }      // descriptor fetch off the first loads' path
     if (warp == 0) tmem_alloc(tmem_slot, NW);
     const bool zp = p.zpass != 0;
     if (zp && tid < 128) {
@@ -398,6 +399,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         for (int s = 0; s < 2; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], 1); mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); }
         mbar_fence_init();
     }
+    if (tid == 160) { tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmSc); tma_prefetch_desc(&tmO); }
     if (warp == 0) tmem_alloc(tmem_slot, 2 * D);
     tc_fence_before();
     __syncthreads();

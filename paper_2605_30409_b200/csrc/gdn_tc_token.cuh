@@ -744,6 +744,7 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
         mbar_init(bar_mma, 1);
         mbar_fence_init();
     }
+    if (tid == 160) { tma_prefetch_desc(tmGp); tma_prefetch_desc(tmNp); tma_prefetch_desc(tmScp); }   // descriptor fetch off the first loads' path
     if (warp == 0) tmem_alloc(tmem_slot, 64);
     tc_fence_before();
     __syncthreads();
@@ -830,7 +831,7 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
                 if (c + STAGES < p.NC) issue_loads(c + STAGES);
             }
         }
-        if (lane == 0) tma_store_wait_all();
+        if (lane == 0) tma_store_wait_read();        // the snapshots have left shared memory; their writes complete with the kernel
     } else {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
         uint32_t ph_mma = 0;
