@@ -256,6 +256,52 @@ def test_bidirectional_stream_with_normaliser_carries_forward_states():
             assert rel_err(S_d.cpu(), S_o) <= TOL_BF16 and rel_err(z_d.cpu(), z_o) <= TOL_BF16
 
 
+def test_bidirectional_log_alpha_zero_state_and_rerun_is_bit_identical():
+    """log-alpha input, state_in = NULL, and determinism: two runs of the same call give the same bits (fixed reduction
+    orders everywhere: DESIGN.md reading 17), also with a token split in Phase A (few heads -> NSPLIT > 1)."""
+    import oracle
+    B, H, G, F, d = 1, 2, 1000, 3, 128
+    wl = gin.GdnWorkload("bidir_log", B, H, G * F, d, d, group=G, seed=52)
+    inp = gin.make_inputs(wl)
+    dev = torch.device("cuda:0")
+    q, k, v, b = inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), inp.beta.to(dev)
+    la = torch.log(inp.alpha).to(dev)
+    outs = []
+    with gdn.GdnPlan(B=B, H=H, T=G * F, d_k=d, d_v=d, group=G, flags=gdn.GDN_FLAG_BIDIR | gdn.GDN_FLAG_LOG_ALPHA) as p:
+        for _ in range(2):
+            out = torch.empty(B, G * F, H, d, device=dev, dtype=torch.bfloat16)
+            S = torch.empty(B, H, d, d, device=dev)
+            p.forward(q, k, v, la, b, None, out, S)
+            torch.cuda.synchronize()
+            outs.append((out.cpu(), S.cpu()))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    o_ref, S_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, None, group=G, bidir=True)
+    assert rel_err(outs[0][0], o_ref) <= TOL_BF16 and rel_err(outs[0][1], S_ref) <= TOL_BF16
+
+
+def test_normalizer_tensor_core_zero_z_and_separate_output_and_errors():
+    import oracle
+    B, H, G, F, d = 1, 3, 300, 2, 64
+    wl = gin.GdnWorkload("norm_tc0", B, H, G * F, d, d, group=G, seed=33)
+    inp = gin.make_normalizer_inputs(wl)
+    ex = inp.extras
+    dev = torch.device("cuda:0")
+    out = torch.empty(B, G * F, H, d, device=dev, dtype=torch.bfloat16)
+    S_out = torch.empty(B, H, d, d, device=dev)
+    z_out = torch.full((B, H, d), float("nan"), device=dev)
+    args = [inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), ex["q_raw"].to(dev), ex["k_raw"].to(dev), inp.alpha.to(dev), inp.beta.to(dev)]
+    with gdn.GdnPlan(B=B, H=H, T=G * F, d_k=d, d_v=d, group=G, flags=gdn.GDN_FLAG_NORMALIZER) as p:
+        p.forward_norm(*args, None, None, out, S_out, z_out)               # S_in = z_in = NULL: zeros
+        torch.cuda.synchronize()
+        with pytest.raises(gdn.GdnError):                                  # q_raw missing
+            p.forward_norm(args[0], args[1], args[2], None, args[4], args[5], args[6], None, None, out, S_out, z_out)
+        with pytest.raises(gdn.GdnError):                                  # plain entry point on a normaliser plan
+            p.forward(args[0], args[1], args[2], args[5], args[6], None, out, S_out)
+    o_ref, S_ref, z_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, None, group=G, q_raw=ex["q_raw"],
+                                             k_raw=ex["k_raw"], z_in=None, normalizer=True)
+    assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S_out.cpu(), S_ref) <= TOL_BF16 and rel_err(z_out.cpu(), z_ref) <= TOL_BF16
+
+
 def test_bidirectional_flag_is_refused_where_it_has_no_path():
     for kw in (dict(group=1), dict(group=64, io_dtype=gdn.GDN_FP32), dict(group=64, d_k=32, d_v=32)):
         args = dict(B=1, H=2, T=256, d_k=64, d_v=64, flags=gdn.GDN_FLAG_BIDIR)
