@@ -41,7 +41,7 @@ def peaks():
 def workload(args):
     from paper_2605_30409_b200 import inputs as gin
     if args.paper_shape:
-        return gin.paper_shape(3)                  # 3 x 880 tokens, 20 heads, d = 128
+        return gin.paper_shape(3, d=112 if args.d112 else 128)   # 3 x 880 tokens, 20 heads, d = 112 or padded 128
     wl = gin.config(args.config, frame=(args.mode == "frame"), chunk=args.chunk)
     return wl
 
@@ -403,6 +403,7 @@ def main():
     ap.add_argument("--normalizer", action="store_true", help="frame mode: the paper's normalised readout (Eq. 20-22)")
     ap.add_argument("--bidir", action="store_true", help="frame mode: bidirectional in-chunk scan (Alg. 1)")
     ap.add_argument("--paper-shape", action="store_true", help="3 x 880 tokens, 20 heads, d = 128, frame-wise")
+    ap.add_argument("--d112", action="store_true", help="with --paper-shape: unpadded head dim 112")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -66,7 +66,8 @@ enum {
 typedef struct {
     uint32_t struct_size;      /* = sizeof(gdn_config_t); ABI versioning                                 */
     int32_t  B, H, T;          /* T = tokens per call (one streaming chunk); B,H,T >= 0                  */
-    int32_t  d_k, d_v;         /* head dims, each in {32, 64, 128}                                       */
+    int32_t  d_k, d_v;               /* each in {32,64,128}; or both 112 (the paper's head dim): bf16 tensor-core plans
+                                        compute it as 128 with the padding done by the tensor maps (Alg. 1 l.1)        */
     int32_t  group;            /* G: 1 = token-wise; tokens-per-frame = frame-wise (paper). T % G == 0   */
     int32_t  chunk;            /* token-wise compute tile C in {64, 128}; 0 = auto. Ignored when G > 1.
                                   Results do not depend on C beyond rounding.                           */

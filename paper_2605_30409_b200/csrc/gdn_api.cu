@@ -178,10 +178,15 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
     if (!(c.chunk == 0 || c.chunk == 64 || c.chunk == 128)) return fail(nullptr, GDN_ERR_INVALID_ARG, "chunk must be 0, 64 or 128");
     const uint32_t known = GDN_FLAG_NORMALIZER | GDN_FLAG_BIDIR | GDN_FLAG_LOG_ALPHA | GDN_FLAG_FORCE_SIMT | GDN_FLAG_UNFUSED;
     if (c.flags & ~known) return fail(nullptr, GDN_ERR_INVALID_ARG, "unknown flag bits");
-    if (!head_dim_ok(c.d_k) || !head_dim_ok(c.d_v))
-        return fail(nullptr, GDN_ERR_UNSUPPORTED, "d_k and d_v must each be 32, 64 or 128 (112 via padding is not implemented)");
+    const bool d112 = c.d_k == 112 && c.d_v == 112;     // the paper's head dim, zero-padded to 128 inside the tensor-core kernels
+    if (d112) {
+        gdn_path_t pth; int ch = 0, ln = 0;
+        if ((c.flags & GDN_FLAG_FORCE_SIMT) || ((c.flags & GDN_FLAG_NORMALIZER) && c.group == 1) || !gdn::tc_supported(c, &pth, &ch, &ln))
+            return fail(nullptr, GDN_ERR_UNSUPPORTED, "d = 112 needs a bf16 tensor-core plan (frame-wise, or token-wise with the fused kernel)");
+    } else if (!head_dim_ok(c.d_k) || !head_dim_ok(c.d_v))
+        return fail(nullptr, GDN_ERR_UNSUPPORTED, "d_k and d_v must each be 32, 64 or 128 (or both 112)");
     // the bidirectional in-chunk scan exists on the frame-wise tensor-core path only (the paper's case, Alg. 1)
-    if ((c.flags & GDN_FLAG_BIDIR) && !(c.group > 1 && c.io_dtype == GDN_BF16 && c.d_k == c.d_v && (c.d_k == 64 || c.d_k == 128) &&
+    if ((c.flags & GDN_FLAG_BIDIR) && !(c.group > 1 && c.io_dtype == GDN_BF16 && c.d_k == c.d_v && (c.d_k == 64 || c.d_k == 112 || c.d_k == 128) &&
                                         !(c.flags & GDN_FLAG_FORCE_SIMT)))
         return fail(nullptr, GDN_ERR_UNSUPPORTED, "GDN_FLAG_BIDIR needs a frame-wise (group > 1) bf16 plan with d_k = d_v in {64,128}");
     const long long strides[4] = {c.q_token_stride, c.k_token_stride, c.v_token_stride, c.o_token_stride};

@@ -63,7 +63,10 @@ inline int tc_default_chunk(const gdn_config_t& c) { return c.chunk ? c.chunk : 
 // Does a tensor-core path exist for this config? Fills the resolved path / compute tile / launch count.
 inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, int* launches) {
     if (c.io_dtype != GDN_BF16) return false;
-    if (c.d_k != c.d_v || !(c.d_k == 64 || c.d_k == 128)) return false;
+    // head dim 112 (the paper's, PAPER.md L316 / Alg. 1 l.1) is computed as 128: the tensor maps zero-fill features 112..127
+    // on load and clip them on store, and zero features leave their rows / columns of every summary and state zero
+    if (c.d_k != c.d_v || !(c.d_k == 64 || c.d_k == 112 || c.d_k == 128)) return false;
+    if (c.d_k == 112 && c.group == 1 && (c.chunk == 64 || (c.flags & GDN_FLAG_UNFUSED))) return false;   // fused token kernel only
     if (c.group != 1) {                                               // frame-wise (the paper's variant)
         *path = GDN_PATH_TC_FRAME;
         *chunk = 0;
@@ -97,7 +100,7 @@ inline int frame_splits(int units, int tpf, int sms) {
 inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm_count, std::string* err) {
     tp.mode = GDN_PATH_TC_FRAME;
     tp.sm_count = sm_count;
-    tp.D = c.d_k; tp.C = 0; tp.BH = c.B * c.H;
+    tp.D = c.d_k == 112 ? 128 : c.d_k; tp.C = 0; tp.BH = c.B * c.H;
     tp.G = c.group; tp.F = c.T / c.group; tp.TPF = (c.group + 127) / 128;
     tp.NC = tp.F; tp.NSc = tp.F + 1; tp.NT = tp.F * tp.TPF;
     tp.NSPLIT = frame_splits(tp.BH * tp.F * (tp.D == 128 ? 2 : 1), tp.TPF, sm_count > 0 ? sm_count : 148);
@@ -169,7 +172,7 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     if (c.group != 1) return tc_plan_init_frame(tp, c, sm_count, err);
     tp.mode = GDN_PATH_TC_TOKEN;
     tp.sm_count = sm_count;
-    tp.D = c.d_k;
+    tp.D = c.d_k == 112 ? 128 : c.d_k;
     tp.C = tc_default_chunk(c);
     tp.BH = c.B * c.H;
     tp.NT = (c.T + 127) / 128;
@@ -411,7 +414,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
         TokParams cp{};
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
-        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dbg = nullptr;
+        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dr = c.d_k; cp.dbg = nullptr;
         cudaError_t e = cudaSuccess;
         cudaEvent_t den_ready = nullptr;
         if (na) {
@@ -451,7 +454,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     TokParams p{};
     p.alpha = alpha; p.beta = beta; p.S_in = S_in; p.S_out = S_out; p.out = out;
     p.Gw = tp.Gw; p.Nw = tp.Nw; p.gam = tp.gam; p.Qt = tp.Qt; p.Ol = tp.Ol; p.Sc = tp.Sc;
-    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC; p.NCa = tp.NC; p.NSc = tp.NSc;
+    p.B = c.B; p.H = c.H; p.T = c.T; p.NT = tp.NT; p.NC = tp.NC; p.NCa = tp.NC; p.NSc = tp.NSc; p.dr = c.d_k;
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;

@@ -234,10 +234,13 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
         for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
             const int bh = u / NCT, ct = u % NCT;
             const int col0 = ct * 64 + half * 32;
-            if (m_ok && p.S_in) {
-                const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * D + m) * D + col0);
+            if (m_ok && m < p.dr && p.S_in) {
+                const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * p.dr + m) * p.dr + col0);
 #pragma unroll
-                for (int i = 0; i < 8; ++i) { const float4 f = __ldcg(src + i); S[4 * i] = f.x; S[4 * i + 1] = f.y; S[4 * i + 2] = f.z; S[4 * i + 3] = f.w; }
+                for (int i = 0; i < 8; ++i) {
+                    const float4 f = (col0 + 4 * i < p.dr) ? __ldcg(src + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    S[4 * i] = f.x; S[4 * i + 1] = f.y; S[4 * i + 2] = f.z; S[4 * i + 3] = f.w;
+                }
             } else {
 #pragma unroll
                 for (int i = 0; i < 32; ++i) S[i] = 0.f;
@@ -294,10 +297,11 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 if (gs == 11 && tid == 0) GDN_STAMP_ANY(31);
                 if (tid == 0) GDN_TRACE(2 * gs + 1);
             }
-            if (m_ok) {
-                float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + col0);
+            if (m_ok && m < p.dr) {
+                float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * p.dr + m) * p.dr + col0);
 #pragma unroll
-                for (int i = 0; i < 8; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+                for (int i = 0; i < 8; ++i)
+                    if (col0 + 4 * i < p.dr) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
             }
         }
     } else if (warp < 12) {

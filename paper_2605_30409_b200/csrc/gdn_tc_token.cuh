@@ -42,6 +42,8 @@ struct TokParams {
     // frame path, Alg. 1 l.14-17: rev = 1 runs NC = NCa - 1 steps over the entries NCa-1, NCa-2, ..., 1 from a zero
     // state and stores the state BEFORE entry e is applied (= S<_e) in snapshot slot e; S_out may be NULL).
     int NCa, rev;
+    int dr;                      // real state dimension: D, or 112 when the head dim is zero-padded to D = 128 (Alg. 1 l.1); the
+                                 // user's state / z tensors are [dr][dr] / [dr], everything inside the library is [D][D]
     // chain kernel, normaliser z pass: the state is a vector living in column 0 of the matrix state.  z_vec_in [BH][D] (or
     // NULL = zeros) initialises it instead of S_in, z_vec_out [BH][D] receives it instead of S_out (either may be NULL).
     int zvec;
@@ -772,11 +774,14 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
     if (p.zvec) {
 #pragma unroll
         for (int i = 0; i < 64; ++i) S[i] = 0.f;
-        if (m_ok && ct == 0 && p.z_vec_in) S[0] = p.z_vec_in[(long long)bh * D + m];
-    } else if (m_ok && p.S_in) {
-        const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * D + m) * D + n0);
+        if (m_ok && m < p.dr && ct == 0 && p.z_vec_in) S[0] = p.z_vec_in[(long long)bh * p.dr + m];
+    } else if (m_ok && m < p.dr && p.S_in) {
+        const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * p.dr + m) * p.dr + n0);
 #pragma unroll
-        for (int i = 0; i < 16; ++i) { const float4 f = src[i]; S[4 * i] = f.x; S[4 * i + 1] = f.y; S[4 * i + 2] = f.z; S[4 * i + 3] = f.w; }
+        for (int i = 0; i < 16; ++i) {
+            const float4 f = (n0 + 4 * i < p.dr) ? src[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+            S[4 * i] = f.x; S[4 * i + 1] = f.y; S[4 * i + 2] = f.z; S[4 * i + 3] = f.w;
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < 64; ++i) S[i] = 0.f;
@@ -878,11 +883,12 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
             gamma_c = gamma_next;
         }
         if (p.zvec) {
-            if (m_ok && ct == 0 && p.z_vec_out) p.z_vec_out[(long long)bh * D + m] = S[0];
-        } else if (m_ok && p.S_out) {
-            float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * D + m) * D + n0);
+            if (m_ok && m < p.dr && ct == 0 && p.z_vec_out) p.z_vec_out[(long long)bh * p.dr + m] = S[0];
+        } else if (m_ok && m < p.dr && p.S_out) {
+            float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * p.dr + m) * p.dr + n0);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+            for (int i = 0; i < 16; ++i)
+                if (n0 + 4 * i < p.dr) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
         }
     }
     tc_fence_before();

@@ -149,7 +149,7 @@ def config(idx: int, *, T: Optional[int] = None, chunk: int = 0, frame: bool = F
     return wl
 
 
-def paper_shape(frames: int = 3) -> GdnWorkload:
+def paper_shape(frames: int = 3, d: int = 128) -> GdnWorkload:
     """The paper's production chunk: 22x40 = 880 tokens per frame, 20 heads, d padded to 128
     (PAPER.md L270, L316, L385); first chunk has 5 frames, later ones 3 (L460)."""
-    return GdnWorkload(f"paper_{frames}x880", 1, 20, frames * 880, 128, 128, group=880, seed=7000 + frames)
+    return GdnWorkload(f"paper_{frames}x880" + ("" if d == 128 else f"_d{d}"), 1, 20, frames * 880, d, d, group=880, seed=7000 + frames)

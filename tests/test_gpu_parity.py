@@ -302,6 +302,49 @@ def test_normalizer_tensor_core_zero_z_and_separate_output_and_errors():
     assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S_out.cpu(), S_ref) <= TOL_BF16 and rel_err(z_out.cpu(), z_ref) <= TOL_BF16
 
 
+# ---- head dim 112 (the paper's; "Pad head dimension to BLOCK_D = 128", Alg. 1 l.1, L316) -----------------
+@pytest.mark.parametrize("G,F,H", [(1, 1000, 3), (880, 3, 20), (352, 2, 4)])
+def test_head_dim_112_is_padded_inside_the_kernels(G, F, H):
+    """d_k = d_v = 112 tensors go in and come out unpadded: the tensor maps zero-fill / clip features 112..127 and the
+    state is [112][112]; token-wise (fused kernel) and frame-wise."""
+    T = F if G == 1 else G * F
+    wl = gin.GdnWorkload("d112", 1, H, T, 112, 112, group=G, seed=71)
+    inp = gin.make_inputs(wl)
+    out, S, info = run_cuda(inp)
+    assert gdn.PATH_NAMES[info[0]] in ("tc_token", "tc_frame")
+    o_ref, S_ref = run_oracle(inp)
+    assert out.shape[-1] == 112 and S.shape[-2:] == (112, 112)
+    assert rel_err(out, o_ref) <= TOL_BF16 and rel_err(S, S_ref) <= TOL_BF16
+
+
+def test_head_dim_112_full_operator_at_the_papers_shape():
+    import oracle
+    B, H, G, F, d = 1, 20, 880, 3, 112
+    wl = gin.GdnWorkload("d112_full", B, H, G * F, d, d, group=G, seed=72)
+    inp = gin.make_normalizer_inputs(wl)
+    ex = inp.extras
+    dev = torch.device("cuda:0")
+    out = torch.empty(B, G * F, H, d, device=dev, dtype=torch.bfloat16)
+    S_out = torch.empty(B, H, d, d, device=dev)
+    z = ex["z_in"].to(dev)
+    with gdn.GdnPlan(B=B, H=H, T=G * F, d_k=d, d_v=d, group=G, flags=gdn.GDN_FLAG_NORMALIZER | gdn.GDN_FLAG_BIDIR) as p:
+        p.forward_norm(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), ex["q_raw"].to(dev), ex["k_raw"].to(dev),
+                       inp.alpha.to(dev), inp.beta.to(dev), inp.state.to(dev), z, out, S_out, z)
+        torch.cuda.synchronize()
+    o_ref, S_ref, z_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=G, q_raw=ex["q_raw"],
+                                             k_raw=ex["k_raw"], z_in=ex["z_in"], normalizer=True, bidir=True)
+    assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S_out.cpu(), S_ref) <= TOL_BF16 and rel_err(z.cpu(), z_ref) <= TOL_BF16
+
+
+def test_head_dim_112_is_refused_without_a_tensor_core_path():
+    for kw in (dict(io_dtype=gdn.GDN_FP32), dict(chunk=64), dict(flags=gdn.GDN_FLAG_FORCE_SIMT), dict(d_v=128)):
+        args = dict(B=1, H=2, T=256, d_k=112, d_v=112)
+        args.update(kw)
+        with pytest.raises(gdn.GdnError) as ei:
+            gdn.GdnPlan(**args)
+        assert ei.value.status == gdn.GDN_ERR_UNSUPPORTED
+
+
 def test_bidirectional_flag_is_refused_where_it_has_no_path():
     for kw in (dict(group=1), dict(group=64, io_dtype=gdn.GDN_FP32), dict(group=64, d_k=32, d_v=32)):
         args = dict(B=1, H=2, T=256, d_k=64, d_v=64, flags=gdn.GDN_FLAG_BIDIR)
