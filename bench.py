@@ -373,6 +373,8 @@ def kernel_bytes(name, wl, by_call):
         "gdn_frm_summaries": th * ((wl.d_k + wl.d_v) * es + 4),
         "gdn_frm_readout": th * (wl.d_k + wl.d_v) * es,
     }
+    if name.startswith("gdn_tok_chain") or name == "gdn_frm_hist_add":
+        return 2 * st                              # the scans only carry the state in and out; their summaries are workspace
     return table.get(name, by_call)               # single-kernel paths: the whole call
 
 
