@@ -82,6 +82,7 @@ __device__ __forceinline__ void st_global_v4(void* p, uint32_t a, uint32_t b, ui
 // ---------------------------------------------------------------------------------------------------
 constexpr int kPrepassNH = 4;
 constexpr int kPrepassThreads = 128 * kPrepassNH;
+constexpr int kPrepassFlagTid = 128;   // lane 0 of a warp that idles during the diagonal-block inversion (FUSED: releases the ready flags)
 
 // 32x32 unit-lower-triangular inverse, one warp, no shuffles: lane c owns COLUMN c of X = (I + L)^-1.
 // Lt holds L TRANSPOSED (Lt[j*kLsStride + r] = L[r][j]) so that "column j of L" is a broadcast LDS.128
@@ -201,14 +202,8 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
 #pragma unroll
             for (int nb = 0; nb < NB; ++nb) tma_load_5d(sK + nb * kBlk, tmK, bar_kq, nb * 64, h, tile * 128, 0, b);
         }
-        // FUSED: the previous tile's stores are still draining. Its first group (Qt, Ol) was staged in sQ / sV.
-        if (FUSED) tma_store_wait_read_but1();
-        mbar_expect_tx(bar_q, TILE);
-#pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sQ + nb * kBlk, tmQ, bar_q, nb * 64, h, tile * 128, 0, b);
-        mbar_expect_tx(bar_v, TILE);
-#pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, tmV, bar_v, nb * 64, h, tile * 128, 0, b);
+        // Q and V are requested only after the diagonal-block inversions (below): tiles landing in shared memory while
+        // the inversions run slow their broadcast loads down by as much as the earlier start would gain.
     }
     // The three 128x128 operand buffers are never pre-zeroed: every phase that fills one writes whole rows
     // (data where the block structure has some, zeros elsewhere) -- see T2 (sA, sB) and the first X1 (sC).
@@ -268,14 +263,14 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
         // FUSED: G / N of the previous tile were staged in sA, sB, sC, which T2 overwrites once this commit
         // has been observed -- their reads must have ended first.
-        if (FUSED) tma_store_wait_read();
+        GDN_STAMP(23);
+        // FUSED: G / N of the previous tile were staged in sA, sB, sC, which T2 overwrites once this commit has been
+        // observed -- their reads must have ended first.  Waiting for the WRITES as well costs nothing more here (the
+        // stores were issued a scan and an MMA ago) and lets the commit below also stand for "the previous tile's
+        // summaries are complete in global memory", so that the ready flag can be released by another thread.
+        if (FUSED) tma_store_wait_all();
+        GDN_STAMP(24);
         umma_commit(bar_mma);
-        if (FUSED && prev_flag) {                  // the previous tile's summaries are complete in global memory
-            tma_store_wait_all();
-            asm volatile("fence.proxy.async;" ::: "memory");
-            __threadfence();
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(prev_flag), "r"(epoch) : "memory");
-        }
     }
     wait_mma();
 
@@ -303,6 +298,13 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     }
     GDN_STAMP(5);
+    if (FUSED && prev_flag && tid == kPrepassFlagTid) {
+        // The previous tile's ready flag.  A release at gpu scope takes ~800 cycles (and the fences that used to precede it
+        // another ~2000): on tid 0 that sat in front of the first diagonal-block inversion of every tile.  This thread's warp
+        // has nothing to do until the inversions are done.  The bulk stores were complete before the K K^T commit was issued
+        // (tid 0 above), this thread observed that commit's mbarrier phase, and the release is cumulative.
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(prev_flag), "r"(epoch) : "memory");
+    }
     float X[CW];                                   // this thread's columns of row `lane` of (I + Ld)^-1
     {
         // diagonal 32x32 block: ONE warp per quadrant reads it from TMEM (TMEM reads are the scarce
@@ -365,16 +367,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                     for (int s = 0; s < 2; ++s)
                         umma_bf16(c0 + 64 * i, desc_kmajor(aA + i * kBlk + s * 32), desc_mnmajor(aB + i * kBlk + (4 * i + s) * 2048, kBlk), id, s > 0);
                 umma_commit(bar_mma);
-                // Q K^T -> c1: not needed before the P mask, so it runs while the X1 round trip is under way
-                // (the next commit covers it)
-                mbar_wait(bar_q, par);
-                tc_fence_after();
-                const uint32_t idq = umma_idesc(128, 128, false, false);
-#pragma unroll
-                for (int s = 0; s < DS; ++s) {
-                    const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
-                    umma_bf16(c1, desc_kmajor(aQ + off), desc_kmajor(aK + off), idq, s > 0);
-                }
             } else {
                 const uint32_t id = umma_idesc(128, 64, false, true);
 #pragma unroll
@@ -419,10 +411,30 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                     umma_bf16(c0, desc_kmajor(aB + kBlk + s * 32), desc_mnmajor(aC + (4 + s) * 2048, kBlk), id, s > 0);
             }
             umma_commit(bar_mma);
+            if (level == (C == 128 ? 2 : 1)) {
+                // Q K^T -> c1: not needed before the P mask, so it runs in the shadow of the last doubling read-out
+                // (the next commit covers it); the Q tile was requested two round trips ago
+                mbar_wait(bar_q, par);
+                tc_fence_after();
+                const uint32_t idq = umma_idesc(128, 128, false, false);
+#pragma unroll
+                for (int s = 0; s < DS; ++s) {
+                    const uint32_t off = (s >> 2) * kBlk + (s & 3) * 32;
+                    umma_bf16(c1, desc_kmajor(aQ + off), desc_kmajor(aK + off), idq, s > 0);
+                }
+            }
         }
         wait_mma();
     };
 
+    if (tid == 64) {                               // sQ, sV are free: the previous tile's stores were complete before the K K^T commit
+        mbar_expect_tx(bar_q, TILE);
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sQ + nb * kBlk, tmQ, bar_q, nb * 64, h, tile * 128, 0, b);
+        mbar_expect_tx(bar_v, TILE);
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) tma_load_5d(sV + nb * kBlk, tmV, bar_v, nb * 64, h, tile * 128, 0, b);
+    }
     // ---- T3/T4: 32 -> 64 blocks: D' = D - mask(D L_off D) ------------------------------------------
     doubling_mmas(1);
     GDN_STAMP(7);
@@ -600,6 +612,9 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     };
     auto store_QO = [&](const uint8_t* odst) {                   // tid 0
+#ifdef GDN_DBG_NOSTORE
+        if (FUSED && (GDN_DBG_NOSTORE & 1)) return;
+#endif
         const int r0 = (int)(((long long)bh * p.NT + tile) * 128);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
@@ -609,6 +624,9 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     };
     auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
+#ifdef GDN_DBG_NOSTORE
+        if (FUSED && (GDN_DBG_NOSTORE & 2)) return;
+#endif
         const int z = bh * p.NC + chunk;
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
