@@ -84,21 +84,25 @@ constexpr int kPrepassNH = 4;
 constexpr int kPrepassThreads = 128 * kPrepassNH;
 constexpr int kPrepassFlagTid = 128;   // lane 0 of a warp that idles during the diagonal-block inversion (FUSED: releases the ready flags)
 
-// 32x32 unit-lower-triangular inverse, one warp, no shuffles: lane c owns COLUMN c of X = (I + L)^-1.
-// Lt holds L TRANSPOSED (Lt[j*kLsStride + r] = L[r][j]) so that "column j of L" is a broadcast LDS.128
-// row.  Right-looking forward substitution: once x_j is final every later row takes
-// x_r -= L[r][j] x_j (31-j independent FMAs): the serial depth is 31 FMAs, not 31 shuffle rounds.
+// The diagonal 32x32 blocks of I + L are inverted on CUDA cores, one warp per block, no shuffles.  Lt holds L TRANSPOSED
+// (Lt[j*kLsStride + r] = L[r][j]) so that "column j of L" is a row of 16-byte loads.  Blocked in 16s:
+// L = [[L11, 0], [L21, L22]]  ->  X = [[X11, 0], [-X22 L21 X11, X22]]; X11, X22 by right-looking forward substitution
+// (once x_j is final every later row takes x_r -= L[r][j] x_j: the serial depth is 15 FMAs), the off-diagonal block by
+// two register-tiled 16x16x16 products.
 constexpr int kLsStride = 36;                     // floats per row: 16-byte aligned, conflict-free
+// 16x16 unit-lower-triangular inverse: Lt[j*kLsStride + r] = L[r][j] (r, j < 16), the calling lane owns column `col` of
+// X = (I + L)^-1.  Two of these (the two diagonal 16-blocks of a 32-block) run in the two halves of one warp with
+// different base pointers.
 template <int J>
-__device__ __forceinline__ void inv32_load_row(const float* __restrict__ Lt, float4 (&l)[8]) {
+__device__ __forceinline__ void inv16_load_row(const float* __restrict__ Lt, float4 (&l)[4]) {
 #pragma unroll
-    for (int r4 = (J + 1) / 4; r4 < 8; ++r4) l[r4] = *reinterpret_cast<const float4*>(Lt + J * kLsStride + 4 * r4);
+    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) l[r4] = *reinterpret_cast<const float4*>(Lt + J * kLsStride + 4 * r4);
 }
 template <int J>
-__device__ __forceinline__ void inv32_apply_row(const float4 (&l)[8], float (&x)[32]) {
+__device__ __forceinline__ void inv16_apply_row(const float4 (&l)[4], float (&x)[16]) {
     const float xj = x[J];
 #pragma unroll
-    for (int r4 = (J + 1) / 4; r4 < 8; ++r4) {
+    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) {
         if (4 * r4 + 0 > J) x[4 * r4 + 0] = fmaf(-l[r4].x, xj, x[4 * r4 + 0]);
         if (4 * r4 + 1 > J) x[4 * r4 + 1] = fmaf(-l[r4].y, xj, x[4 * r4 + 1]);
         if (4 * r4 + 2 > J) x[4 * r4 + 2] = fmaf(-l[r4].z, xj, x[4 * r4 + 2]);
@@ -106,19 +110,19 @@ __device__ __forceinline__ void inv32_apply_row(const float4 (&l)[8], float (&x)
     }
 }
 template <int J>
-__device__ __forceinline__ void inv32_steps(const float* __restrict__ Lt, float4 (&cur)[8], float4 (&nxt)[8], float (&x)[32]) {
-    if constexpr (J < 31) {
-        if constexpr (J + 1 < 31) inv32_load_row<J + 1>(Lt, nxt);      // next row's loads fly during this row's FMAs
-        inv32_apply_row<J>(cur, x);
-        inv32_steps<J + 1>(Lt, nxt, cur, x);
+__device__ __forceinline__ void inv16_steps(const float* __restrict__ Lt, float4 (&cur)[4], float4 (&nxt)[4], float (&x)[16]) {
+    if constexpr (J < 15) {
+        if constexpr (J + 1 < 15) inv16_load_row<J + 1>(Lt, nxt);
+        inv16_apply_row<J>(cur, x);
+        inv16_steps<J + 1>(Lt, nxt, cur, x);
     }
 }
-__device__ __forceinline__ void inv32_columns(const float* __restrict__ Lt, int lane, float (&x)[32]) {
+__device__ __forceinline__ void inv16_columns(const float* __restrict__ Lt, int col, float (&x)[16]) {
 #pragma unroll
-    for (int r = 0; r < 32; ++r) x[r] = (r == lane) ? 1.f : 0.f;
-    float4 la[8], lb[8];
-    inv32_load_row<0>(Lt, la);
-    inv32_steps<0>(Lt, la, lb, x);
+    for (int r = 0; r < 16; ++r) x[r] = (r == col) ? 1.f : 0.f;
+    float4 la[4], lb[4];
+    inv16_load_row<0>(Lt, la);
+    inv16_steps<0>(Lt, la, lb, x);
 }
 
 // Shared-memory carve-up and barriers of one prepass CTA (set up once; a persistent CTA runs many tiles).
@@ -330,17 +334,60 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             for (int e = 0; e < 16; ++e) { Lq[e * kLsStride + lane] = v0[e]; Lq[(16 + e) * kLsStride + lane] = v1[e]; }
             __syncwarp();
             GDN_STAMP(16);
-            float xc[32];                          // column `lane` of the inverse
-            inv32_columns(Lq, lane, xc);
+            // Blocked: L = [[L11, 0], [L21, L22]] in 16-blocks, X = [[X11, 0], [-X22 L21 X11, X22]].
+            // Step 1 (this warp): lanes 0-15 invert I + L11, lanes 16-31 invert I + L22, each lane one column.
+            const int o = lane & 16, col = lane & 15;
+            float xc[16];
+            inv16_columns(Lq + o * kLsStride + o, col, xc);
             GDN_STAMP(18);
             __syncwarp();
-            GDN_STAMP(17);
-            // transpose through the same scratch: element (r, c = lane) -> Lq[r][c]
+            // X11 / X22 row-major over L11^T / L22^T (consumed): element (r, col) -> Lq[o + r][o + col]
 #pragma unroll
-            for (int r = 0; r < 32; ++r) Lq[r * kLsStride + lane] = xc[r];
+            for (int r = 0; r < 16; ++r) Lq[(o + r) * kLsStride + o + col] = xc[r];
+            __syncwarp();
+            // Steps 2a, 2b (same warp, lane = row r2 x 8 columns): M = L21 X11 into the free block Lq[16 + r][c] (L^T has
+            // nothing there), then X21 = -X22 M in its place, and zeros over L21^T (X's upper-right block).
+            const int r2 = lane >> 1, cc0 = (lane & 1) * 8;
+            float acc[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const float a = Lq[k * kLsStride + 16 + r2];                          // L21[r2][k] = L[16 + r2][k]
+                const float4 b0 = *reinterpret_cast<const float4*>(Lq + k * kLsStride + cc0);       // X11[k][cc0 ..]
+                const float4 b1 = *reinterpret_cast<const float4*>(Lq + k * kLsStride + cc0 + 4);
+                acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
+                acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
+            }
+            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0 + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
+            __syncwarp();
+            float xr[16];                                                             // X22[r2][0..15]
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4) {
+                const float4 f = *reinterpret_cast<const float4*>(Lq + (16 + r2) * kLsStride + 16 + 4 * k4);
+                xr[4 * k4] = f.x; xr[4 * k4 + 1] = f.y; xr[4 * k4 + 2] = f.z; xr[4 * k4 + 3] = f.w;
+            }
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const float4 b0 = *reinterpret_cast<const float4*>(Lq + (16 + k) * kLsStride + cc0);   // M[k][cc0 ..]
+                const float4 b1 = *reinterpret_cast<const float4*>(Lq + (16 + k) * kLsStride + cc0 + 4);
+                const float a = xr[k];
+                acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
+                acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
+            }
+            __syncwarp();                                                             // every M has been read
+            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0) = make_float4(-acc[0], -acc[1], -acc[2], -acc[3]);
+            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0 + 4) = make_float4(-acc[4], -acc[5], -acc[6], -acc[7]);
+            *reinterpret_cast<float4*>(Lq + r2 * kLsStride + 16 + cc0) = make_float4(0.f, 0.f, 0.f, 0.f);
+            *reinterpret_cast<float4*>(Lq + r2 * kLsStride + 16 + cc0 + 4) = make_float4(0.f, 0.f, 0.f, 0.f);
+            GDN_STAMP(17);
         }
+        const uint32_t qbar = 1 + wq, qthreads = 32 * NH;
         // all NH warps of the quadrant pick up their columns of row `lane`
-        asm volatile("bar.sync %0, %1;" ::"r"(1 + wq), "r"(32 * NH) : "memory");
+        asm volatile("bar.sync %0, %1;" ::"r"(qbar), "r"(qthreads) : "memory");
         ld_shared_fw(Lq + lane * kLsStride + cb, X);
     }
     store_roww_bf16(aB, kBlk, row, wq * 32 + cb, X);
