@@ -376,6 +376,7 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
     const int round_tiles = fp.HPR * NT;
     uint32_t it = 0, ph = 0;
     unsigned int* pending = nullptr;
+    float2 gates = make_float2(0.f, 0.f);          // this thread's alpha, beta of the next tile (prefetched a tile ahead)
     auto tile_of = [&](int i, int& bh, int& tile) {
         // chunk-major inside a head group, so the chain workers of the group can follow closely
         const int r = i / round_tiles, il = i - r * round_tiles;
@@ -388,7 +389,7 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
         if (i + nwp < fp.total_tiles) tile_of(i + nwp, nbh, ntile);
         if (tid == 0) GDN_TRACE(2 * it);
         // the previous tile's ready flag is published inside this tile, once its stores have completed
-        tok::prepass_tile<D, 128, true>(cx, tmQ, tmK, tmV, tmG, tmN, tmQt, tmOl, p, bh, tile, it, ph, pending, fp.epoch, nbh, ntile);
+        tok::prepass_tile<D, 128, true>(cx, tmQ, tmK, tmV, tmG, tmN, tmQt, tmOl, p, bh, tile, it, ph, pending, fp.epoch, nbh, ntile, &gates);
         if (tid == 0) GDN_TRACE(2 * it + 1);
         pending = fp.flags + (long long)bh * NT + tile;
     }

@@ -168,7 +168,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                                              const CUtensorMap* tmQt, const CUtensorMap* tmOl, const TokParams& p,
                                              int bh, int tile, uint32_t it, uint32_t& ph,
                                              unsigned int* prev_flag = nullptr, unsigned int epoch = 0,
-                                             int next_bh = -1, int next_tile = -1) {
+                                             int next_bh = -1, int next_tile = -1, float2* gates = nullptr) {
     static_assert(!FUSED || C == 128, "the fused path runs C = 128");
     constexpr int NH = kPrepassNH;
     constexpr int CW = 32 / NH;                   // columns of each 32-column chunk handled per thread
@@ -192,14 +192,16 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
 
     GDN_STAMP(0);
     // gates first: their global-load latency overlaps the barrier / TMEM / TMA set-up
-    const int t = tile * 128 + row;
-    float g = 0.f, beta_i = 0.f;
-    if (t < p.T) {
-        g = p.alpha[(long long)bh * p.T + t];
-        beta_i = p.beta[(long long)bh * p.T + t];
-    } else if (!p.log_alpha) {
-        g = 1.f;
-    }
+    // (a persistent CTA passes `gates`: this row's alpha, beta of this tile, fetched during the previous tile)
+    auto load_gates = [&](int gbh, int gtile) {
+        const int t = gtile * 128 + row;
+        float2 r = make_float2(p.log_alpha ? 0.f : 1.f, 0.f);                  // padding rows: alpha = 1, beta = 0
+        if (t < p.T) { r.x = p.alpha[(long long)gbh * p.T + t]; r.y = p.beta[(long long)gbh * p.T + t]; }
+        return r;
+    };
+    const float2 gb = (gates && it > 0) ? *gates : load_gates(bh, tile);
+    float g = gb.x;
+    const float beta_i = gb.y;
     if (tid == 0) {
         if (!FUSED || it == 0) {                   // FUSED, it > 0: the previous tile prefetched this tile's K
             mbar_expect_tx(bar_kq, TILE);
@@ -685,6 +687,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
 
     if (tid == 0) issue_summary(0);
+    if (gates && next_bh >= 0) *gates = load_gates(next_bh, next_tile);       // lands while the summary MMAs run
     wait_mma();
     GDN_STAMP(13);
     if (FUSED && tid == 0 && next_bh >= 0) {
