@@ -394,10 +394,8 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
         pending = fp.flags + (long long)bh * NT + tile;
     }
     if (tid == 0 && pending) {
-        tma_store_wait_all();                      // the last tile's summaries are complete in global memory
-        fence_proxy_async_all();
-        __threadfence();
-        st_release_gpu(pending, fp.epoch);
+        tma_store_wait_all();                      // the last tile's summaries are complete in global memory ...
+        st_release_gpu(pending, fp.epoch);         // ... and the release orders them (and this thread's gamma store) before the flag
     }
     tc_fence_before();
     __syncthreads();
