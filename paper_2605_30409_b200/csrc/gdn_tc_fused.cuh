@@ -82,7 +82,7 @@ constexpr uint32_t fused_smem_bytes() {
 
 // ---------------------------------------------------------------------------------------------------
 // chain worker.  warps 0-7: state rows (thread = row m x 32 columns); 8-11: output epilogue (thread = token
-// row); 12: MMA issuer (chain first, output behind it); 13: flag poller + TMA producer; 14-15: idle.
+// row); 12: chain MMA issuer; 13: flag poller + TMA producer; 14: output MMA issuer; 15: idle.
 // The chain (warps 0-7) and the output (warps 8-11) only meet at the bf16 state operand buffers: the output
 // of chunk c reads S_c while the chain is already up to NSB - 1 steps further on.
 // ---------------------------------------------------------------------------------------------------
@@ -107,6 +107,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
     uint64_t* out_free = out_full + 2;        // [2] output accumulator drained (4 warps)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(out_free + 2);
     float* sGamma = reinterpret_cast<float*>(smem + L::OFF_GAM);
+    volatile uint32_t* chain_issued = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_GAM + 64);   // chain MMAs issued so far
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
@@ -116,6 +117,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
         mbar_init(mma_chain, 1);
         for (int s = 0; s < 2; ++s) { mbar_init(&out_full[s], 1); mbar_init(&out_free[s], 4); }
         mbar_fence_init();
+        *chain_issued = 0;
     }
     if (warp == 0) tmem_alloc(tmem_slot, 256);
     tc_fence_before();
@@ -179,34 +181,14 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             }
         }
     } else if (warp == 12) {
-        // ===== MMA issuer.  chain: acc = G_c (A, K-major) * S_c (B, MN-major); output: acc_out = Qt_c (A) * S_c.
-        // The chain MMA of a step goes out the moment its operand is published; output MMAs follow in the
-        // shadow of the chain's TMEM -> register -> shared-memory round trip and may lag by up to NSB - 1 steps.
+        // ===== chain MMA issuer: acc = G_c (A, K-major) * S_c (B, MN-major), the moment the operand is published.
+        // Nothing else is issued by this thread: its commit covers the chain MMA only, and no output MMA's issue sits
+        // between a publication and the chain MMA that waits for it.
         if (lane == 0) {
             const uint32_t idc = umma_idesc(D, 64, false, true);
-            const uint32_t ido = umma_idesc(128, 64, false, true);
             const uint32_t total = (uint32_t)((nunits - (int)blockIdx.x + fp.NWC - 1) / fp.NWC) * (uint32_t)NT;   // steps of this CTA
-            uint32_t no = 0;                                         // next output MMA to issue
-            auto out_ready = [&](uint32_t o) {
-                return mbar_try_wait(&q_full[o % QST], (o / QST) & 1u) && (o < 2 || mbar_try_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u));
-            };
-            auto issue_out = [&](uint32_t o) {                       // S_o is published (o <= the chain step just issued)
-                const int qst = o % QST, sb = o % NSB;
-                mbar_wait(&q_full[qst], (o / QST) & 1u);
-                if (o >= 2) mbar_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u);
-                tc_fence_after();
-                const uint32_t aQ = smem_u32(sQ + qst * L::Q_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
-                const uint32_t acc_out = tmem + 64 + 64 * (o & 1);
-#pragma unroll
-                for (int s = 0; s < D / 16; ++s)
-                    umma_bf16(acc_out, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), ido, s > 0);
-                umma_commit(&out_full[o & 1]);
-                umma_commit(&s_free[sb]);
-            };
             for (uint32_t gs = 0; gs < total; ++gs) {
                 const int gst = gs % GST, sb = gs % NSB;
-                // publication gs reuses the buffer of step gs - NSB: its output MMA must be out before we block on s_ready
-                while (no + NSB <= gs) issue_out(no++);
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
                 if (gs == 12) GDN_STAMP_ANY(40);
                 mbar_wait(&s_ready[sb], (gs / NSB) & 1u);
@@ -218,10 +200,31 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     umma_bf16(acc_chain, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), idc, s > 0);
                 umma_commit(mma_chain);
                 umma_commit(&g_empty[gst]);
+                *chain_issued = gs + 1;                              // the output issuer lets the chain MMA of a step go first
                 if (gs == 12) GDN_STAMP_ANY(42);
-                while (no <= gs && out_ready(no)) issue_out(no++);
             }
-            while (no < total) issue_out(no++);
+        }
+    } else if (warp == 14) {
+        // ===== output MMA issuer: acc_out = Qt_c (A) * S_c (B), in the shadow of the chain's TMEM -> register ->
+        // shared-memory round trip; may lag the chain by up to NSB - 1 steps (s_free gates the reuse of an operand buffer).
+        if (lane == 0) {
+            const uint32_t ido = umma_idesc(128, 64, false, true);
+            const uint32_t total = (uint32_t)((nunits - (int)blockIdx.x + fp.NWC - 1) / fp.NWC) * (uint32_t)NT;
+            for (uint32_t o = 0; o < total; ++o) {
+                const int qst = o % QST, sb = o % NSB;
+                mbar_wait(&s_ready[sb], (o / NSB) & 1u);             // S_o is published
+                mbar_wait(&q_full[qst], (o / QST) & 1u);
+                if (o >= 2) mbar_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u);
+                while (*chain_issued <= o) {}
+                tc_fence_after();
+                const uint32_t aQ = smem_u32(sQ + qst * L::Q_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
+                const uint32_t acc_out = tmem + 64 + 64 * (o & 1);
+#pragma unroll
+                for (int s = 0; s < D / 16; ++s)
+                    umma_bf16(acc_out, desc_kmajor(aQ + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), ido, s > 0);
+                umma_commit(&out_full[o & 1]);
+                umma_commit(&s_free[sb]);
+            }
         }
     } else if (warp < 8) {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
