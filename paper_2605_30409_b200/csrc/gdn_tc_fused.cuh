@@ -183,8 +183,10 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
     } else if (warp == 12) {
         // ===== chain MMA issuer: acc = G_c (A, K-major) * S_c (B, MN-major), the moment the operand is published.
         // Nothing else is issued by this thread: its commit covers the chain MMA only, and no output MMA's issue sits
-        // between a publication and the chain MMA that waits for it.
-        if (lane == 0) {
+        // between a publication and the chain MMA that waits for it.  Issued under elect.sync: with a plain `lane == 0`
+        // every tcgen05.mma sits in a ~70-cycle "waterfall" loop (ELECT / R2UR / BRA.U.ANY) because ptxas cannot keep
+        // its operands in uniform registers -- on this serial chain that is exposed latency (~450 cycles per step).
+        if (elect_one()) {
             const uint32_t idc = umma_idesc(D, 64, false, true);
             const uint32_t total = (uint32_t)((nunits - (int)blockIdx.x + fp.NWC - 1) / fp.NWC) * (uint32_t)NT;   // steps of this CTA
             for (uint32_t gs = 0; gs < total; ++gs) {
