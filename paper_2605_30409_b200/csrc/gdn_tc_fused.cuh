@@ -82,7 +82,8 @@ constexpr uint32_t fused_smem_bytes() {
 
 // ---------------------------------------------------------------------------------------------------
 // chain worker.  warps 0-7: state rows (thread = row m x 32 columns); 8-11: output epilogue (thread = token
-// row); 12: chain MMA issuer; 13: flag poller + TMA producer; 14: output MMA issuer; 15: idle.
+// row); 12: chain MMA issuer; 13: flag poller + TMA producer of the chain's operands; 14: output MMA issuer; 15: flag
+// poller + TMA producer of the output's Qt tiles.
 // The chain (warps 0-7) and the output (warps 8-11) only meet at the bf16 state operand buffers: the output
 // of chunk c reads S_c while the chain is already up to NSB - 1 steps further on.
 // ---------------------------------------------------------------------------------------------------
@@ -128,10 +129,13 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
     const int NT = p.NT;
     const int nunits = p.B * p.H * NCT;
 
-    if (warp == 13) {
-        // ===== flag poller + TMA producer =====
+    if (warp == 13 || warp == 15) {
+        // ===== flag pollers + TMA producers: warp 13 feeds the chain (G_c, N_c, gamma_c), warp 15 the output (Qt).  Two
+        // producers, because the Qt ring also stages the outgoing tiles and recycles at the pace of the output path: in one
+        // in-order producer a late q_empty held back the NEXT chunk's G / N and with it the serial chain.
         // The 32 lanes poll the flags of the next 32 chunks together (one L2 round trip for all of them);
-        // lane 0 issues the loads of every chunk in the ready prefix.
+        // the elected lane issues the loads of every chunk in the ready prefix.
+        const bool feed_chain = warp == 13;
         uint32_t gs = 0;
         for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
             const int bh = u / NCT, ct = u % NCT;
@@ -144,7 +148,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     const bool ok = idx < NT && ld_acquire_gpu(fp.flags + (long long)bh * NT + idx) >= fp.epoch;
                     const uint32_t m = __ballot_sync(0xffffffffu, ok);
                     ready += (m == 0xffffffffu) ? 32 : (__ffs(~m) - 1);      // length of the ready prefix
-                    if (idx < ready) {                       // accepted exactly once per chunk
+                    if (feed_chain && idx < ready) {         // accepted exactly once per chunk
                         gam_l = __ldcg(p.gam + (long long)bh * p.NC + idx);
                         if (GST < 3) {                       // shallow ring: have the summaries waiting in L2
                             fence_proxy_async_all();
@@ -159,23 +163,27 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 }
                 const float gam_c = __shfl_sync(0xffffffffu, gam_l, c - base);
                 if (lane == 0) {
-                    GDN_TRACE(2 * gs);
                     fence_proxy_async_all();
-                    const int gst = gs % GST, qst = gs % QST;
-                    if (gs >= (uint32_t)GST) mbar_wait(&g_empty[gst], ((gs / GST) - 1) & 1u);
-                    sGamma[gst] = gam_c;                     // visible to the waiters of g_full through the arrive below
-                    mbar_expect_tx(&g_full[gst], L::GN_BYTES);
-                    uint8_t* gb = sG + gst * L::GN_BYTES;
-                    const int z = bh * p.NC + c;
+                    if (feed_chain) {
+                        GDN_TRACE(2 * gs);
+                        const int gst = gs % GST;
+                        if (gs >= (uint32_t)GST) mbar_wait(&g_empty[gst], ((gs / GST) - 1) & 1u);
+                        sGamma[gst] = gam_c;                 // visible to the waiters of g_full through the arrive below
+                        mbar_expect_tx(&g_full[gst], L::GN_BYTES);
+                        uint8_t* gb = sG + gst * L::GN_BYTES;
+                        const int z = bh * p.NC + c;
 #pragma unroll
-                    for (int nb = 0; nb < NB; ++nb) tma_load_3d(gb + nb * (D * 128), tmG, &g_full[gst], nb * 64, 0, z);
-                    tma_load_3d(gb + L::G_BYTES, tmN, &g_full[gst], ct * 64, 0, z);
-                    tma_load_3d(gb + L::G_BYTES + D * 128, tmN, &g_full[gst], ct * 64 + 32, 0, z);
-                    if (gs >= (uint32_t)QST) mbar_wait(&q_empty[qst], ((gs / QST) - 1) & 1u);
-                    mbar_expect_tx(&q_full[qst], L::Q_BYTES);
-                    uint8_t* qb = sQ + qst * L::Q_BYTES;
+                        for (int nb = 0; nb < NB; ++nb) tma_load_3d(gb + nb * (D * 128), tmG, &g_full[gst], nb * 64, 0, z);
+                        tma_load_3d(gb + L::G_BYTES, tmN, &g_full[gst], ct * 64, 0, z);
+                        tma_load_3d(gb + L::G_BYTES + D * 128, tmN, &g_full[gst], ct * 64 + 32, 0, z);
+                    } else {
+                        const int qst = gs % QST;
+                        if (gs >= (uint32_t)QST) mbar_wait(&q_empty[qst], ((gs / QST) - 1) & 1u);
+                        mbar_expect_tx(&q_full[qst], L::Q_BYTES);
+                        uint8_t* qb = sQ + qst * L::Q_BYTES;
 #pragma unroll
-                    for (int nb = 0; nb < NB; ++nb) tma_load_2d(qb + nb * kBlk, tmQt, &q_full[qst], nb * 64, (bh * NT + c) * 128);
+                        for (int nb = 0; nb < NB; ++nb) tma_load_2d(qb + nb * kBlk, tmQt, &q_full[qst], nb * 64, (bh * NT + c) * 128);
+                    }
                 }
                 __syncwarp();
             }
