@@ -661,9 +661,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     };
     auto store_QO = [&](const uint8_t* odst) {                   // tid 0
-#ifdef GDN_DBG_NOSTORE
-        if (FUSED && (GDN_DBG_NOSTORE & 1)) return;
-#endif
         const int r0 = (int)(((long long)bh * p.NT + tile) * 128);
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) {
@@ -673,9 +670,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     };
     auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
-#ifdef GDN_DBG_NOSTORE
-        if (FUSED && (GDN_DBG_NOSTORE & 2)) return;
-#endif
         const int z = bh * p.NC + chunk;
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
