@@ -360,6 +360,23 @@ def ncu_traffic(kernel, wl):
     return best
 
 
+def ncu_counters(kernel, wl):
+    """Tensor-pipe utilisation and DRAM throughput of `kernel` on this workload from the same committed ncu capture
+    (north_star: "tensor-pipe utilisation and achieved HBM GB/s from ncu"); None when it was not captured."""
+    f = ROOT / "profiles" / "ncu_traffic.csv"
+    if not f.exists():
+        return None
+    key = (kernel, wl.name, "token" if wl.group == 1 else "frame")
+    best = None
+    for line in f.read_text().splitlines():
+        c = [x.strip() for x in line.split(",")]
+        if len(c) >= 9 and not line.startswith("#") and (c[0], c[1], c[2]) == key:
+            us = float(c[6])
+            best = {"source": "profiles/" + c[5], "gpu_time_us": us, "tensor_pipe_pct_of_active": float(c[7]),
+                    "dram_pct_of_peak": float(c[8]), "dram_gbs": (float(c[3]) + float(c[4])) / (us * 1e-6) / 1e9}
+    return best
+
+
 def kernel_bytes(name, wl, by_call):
     """Algorithmic HBM bytes of ONE launch of kernel `name`: the user tensors that launch must
     read or write once; workspace traffic is not algorithmic."""
@@ -388,7 +405,7 @@ def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
     achieved = kb / (dur_ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
             "frac": achieved / pk["hbm_gbs"], "traffic": ncu_traffic(name, wl), "peak_source": pk_src,
-            "algorithmic_bytes": kb, "kernel_avg_us": dur_ms * 1e3,
+            "algorithmic_bytes": kb, "kernel_avg_us": dur_ms * 1e3, "ncu": ncu_counters(name, wl),
             "whole_call": {"algorithmic_bytes": by, "achieved": by / (ms_per_step * 1e-3) / 1e9,
                            "frac": by / (ms_per_step * 1e-3) / 1e9 / pk["hbm_gbs"]}}
 
