@@ -406,6 +406,8 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
         if (tid == 0) GDN_TRACE(2 * it + 1);
         pending = fp.flags + (long long)bh * NT + tile;
     }
+    if (D == 128 && tid == tok::kPrepassFlagTid && pending) tma_store_wait_all();      // this thread's share of the last tile's stores
+    __syncthreads();
     if (tid == 0 && pending) {
         tma_store_wait_all();                      // the last tile's summaries are complete in global memory ...
         st_release_gpu(pending, fp.epoch);         // ... and the release orders them (and this thread's gamma store) before the flag

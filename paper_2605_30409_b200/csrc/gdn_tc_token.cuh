@@ -304,6 +304,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     }
     GDN_STAMP(5);
+    if (FUSED && D == 128 && it > 0 && tid == kPrepassFlagTid) tma_store_wait_all();     // this thread's share of the previous tile's stores (sC is not reused before the next CTA barrier)
     if (FUSED && prev_flag && tid == kPrepassFlagTid) {
         // The previous tile's ready flag.  A release at gpu scope takes ~800 cycles (and the fences that used to precede it
         // another ~2000): on tid 0 that sat in front of the first diagonal-block inversion of every tile.  This thread's warp
@@ -669,14 +670,15 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             else tma_store_2d(tmOl, odst + nb * kBlk, nb * 64, r0);
         }
     };
-    auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk) {   // tid 0
+    // j_lo .. j_hi: which [D][32] blocks of N go with this call (FUSED, d = 128: the last two, staged in sC, are stored
+    // by the flag thread as a group of its own, so that tid 0's wait in front of the next K K^T commit is shorter)
+    auto store_NG = [&](const uint8_t* gsrc, const uint8_t* nsrc, int chunk, int j_lo = 0, int j_hi = D / 32, bool with_g = true) {
         const int z = bh * p.NC + chunk;
+        if (with_g) {
 #pragma unroll
-        for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) {
-            tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
+            for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
         }
+        for (int j = j_lo; j < j_hi; ++j) tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
     };
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
 
@@ -706,9 +708,14 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         if (tid == 0) {
             if (!(FUSED && D == 128)) store_QO(sV);
             if (FUSED) tma_store_commit();         // group 1: Qt, Ol (sQ, sV); group 2: G, N (sA, sB, sC)
-            store_NG(sA, sB, tile);
+            if (FUSED && D == 128) store_NG(sA, sB, tile, 0, 2);
+            else store_NG(sA, sB, tile);
             tma_store_commit();
             if (!FUSED) tma_store_wait_read();     // FUSED: the next tile waits where it reuses the staging
+        }
+        if (FUSED && D == 128 && tid == kPrepassFlagTid) {      // N blocks 2, 3 (sC): awaited by this thread before it releases the flag
+            store_NG(sA, sB, tile, 2, 4, false);
+            tma_store_commit();
         }
     } else {
         // first half: drain [PUt | PW] (c2), send Qt / Ol off, then reuse c2 for the second chunk's [N | G]
