@@ -376,7 +376,7 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
     tok::prepass_carve<D>(smem, cx, &tmem_slot);
     const int tid = threadIdx.x;
     if (tid == 0) {
-        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
+        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1); mbar_init(cx.bar_mma2, 1);
         mbar_fence_init();
     }
     if (tid < 32) tmem_alloc(tmem_slot, 512);

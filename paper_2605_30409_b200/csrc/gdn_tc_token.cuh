@@ -130,6 +130,7 @@ struct PrepassCtx {
     uint8_t *sK, *sQ, *sV, *sA, *sB, *sC;
     float *sGam, *sBeta, *sBG, *sCF, *sWarp, *sL;
     uint64_t *bar_kq, *bar_q, *bar_v, *bar_mma;    // bar_kq: K tile landed; bar_q: Q tile; bar_v: V tile
+    uint64_t* bar_mma2;                           // C = 128: the [N | G] summary MMAs (committed behind [P Ut | P W], which bar_mma covers)
     uint32_t tmem;                                // 512 TMEM columns
 };
 template <int D>
@@ -151,8 +152,8 @@ __device__ __forceinline__ void prepass_carve(uint8_t* smem, PrepassCtx& cx, uin
     cx.sCF = cx.sBG + 128;                        // [128] e^{Gam_ref(j) - Gam_j}, ref = last row of j's 32-chunk
     cx.sWarp = cx.sCF + 128;                      // [4] per-warp sums of log alpha
     uint64_t* bars = reinterpret_cast<uint64_t*>(cx.sWarp + 4);
-    cx.bar_kq = &bars[0]; cx.bar_v = &bars[1]; cx.bar_mma = &bars[2]; cx.bar_q = &bars[3];
-    *tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
+    cx.bar_kq = &bars[0]; cx.bar_v = &bars[1]; cx.bar_mma = &bars[2]; cx.bar_q = &bars[3]; cx.bar_mma2 = &bars[4];
+    *tmem_slot = reinterpret_cast<uint32_t*>(bars + 5);
 }
 
 // One 128-token tile of one (b,h) stream.  `it` = how many tiles this CTA has run before (barrier parity),
@@ -682,10 +683,37 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     };
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
 
-    if (tid == 0) issue_summary(0);
+    if (C == 128) {
+        // [P Ut | P W] first with a commit of its own: Qt / Ol are staged (and, d = 128, sent off) while [N | G] still runs
+        if (tid == 0) {
+            tc_fence_after();
+            const uint32_t idp = umma_idesc(128, 2 * D, false, true), idg = umma_idesc(D, 2 * D, true, true);
+#pragma unroll
+            for (int s = 0; s < KS; ++s)
+                umma_bf16(c2, desc_kmajor(aC + (s >> 2) * kBlk + (s & 3) * 32), desc_mnmajor(aA + s * 2048, LBO2), idp, s > 0);
+            umma_commit(bar_mma);
+#pragma unroll
+            for (int s = 0; s < KS; ++s)
+                umma_bf16(c0, desc_mnmajor(aK + s * 2048, kBlk), desc_mnmajor(aA + s * 2048, LBO2), idg, s > 0);
+            umma_commit(cx.bar_mma2);
+        }
+    } else {
+        if (tid == 0) issue_summary(0);
+    }
     if (gates && next_bh >= 0) *gates = load_gates(next_bh, next_tile);       // lands while the summary MMAs run
     wait_mma();
     GDN_STAMP(13);
+    if (C == 128) {
+        stage_QO(c2, aV);                          // Qt in place in sQ, Ol -> sV: neither is an operand of [N | G]
+        if (FUSED && D == 128) {
+            // d = 128 leaves 160 KB per tile and the next tile's K K^T commit waits for these stores: Qt / Ol (64 KB) set
+            // off while G / N are still being computed and staged
+            publish_staging();
+            if (tid == 0) { store_QO(sV); tma_store_commit(); }
+        }
+        mbar_wait(cx.bar_mma2, par);
+        tc_fence_after();
+    }
     if (FUSED && tid == 0 && next_bh >= 0) {
         // sK is free (the summary MMAs were its last readers): fetch the next tile's K ahead of this tile's
         // stores, so the next K K^T does not queue behind them
@@ -695,13 +723,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     if (C == 128) {
         // everything is free now: Qt in place, Ol -> sV, G -> sA, N -> sB (+ sC)
-        stage_QO(c2, aV);
-        if (FUSED && D == 128) {
-            // d = 128 leaves 160 KB per tile and the next tile's K K^T commit waits for these stores: Qt / Ol (64 KB) set
-            // off while G / N are still being staged, one barrier more, ~1.3 k cycles of drain earlier
-            publish_staging();
-            if (tid == 0) { store_QO(sV); tma_store_commit(); }
-        }
         stage_NG(c0, aA, aB);
         if (tid == 0) p.gam[(long long)bh * p.NC + tile] = fast_exp(gam_end);
         publish_staging();
@@ -759,7 +780,7 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t* tmem_slot;
     prepass_carve<D>(smem, cx, &tmem_slot);
     if (threadIdx.x == 0) {
-        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1);
+        mbar_init(cx.bar_kq, 1); mbar_init(cx.bar_q, 1); mbar_init(cx.bar_v, 1); mbar_init(cx.bar_mma, 1); mbar_init(cx.bar_mma2, 1);
         mbar_fence_init();
     }
     if (threadIdx.x < 32) tmem_alloc(tmem_slot, 512);
