@@ -94,9 +94,9 @@ constexpr int kLsStride = 36;                     // floats per row: 16-byte ali
 // X = (I + L)^-1.  Two of these (the two diagonal 16-blocks of a 32-block) run in the two halves of one warp with
 // different base pointers.
 template <int J>
-__device__ __forceinline__ void inv16_load_row(const float* __restrict__ Lt, float4 (&l)[4]) {
+__device__ __forceinline__ void inv16_load_row(uint32_t Lt, float4 (&l)[4]) {
 #pragma unroll
-    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) l[r4] = *reinterpret_cast<const float4*>(Lt + J * kLsStride + 4 * r4);
+    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) l[r4] = lds_f4(Lt + (J * kLsStride + 4 * r4) * 4);
 }
 template <int J>
 __device__ __forceinline__ void inv16_apply_row(const float4 (&l)[4], float (&x)[16]) {
@@ -110,14 +110,15 @@ __device__ __forceinline__ void inv16_apply_row(const float4 (&l)[4], float (&x)
     }
 }
 template <int J>
-__device__ __forceinline__ void inv16_steps(const float* __restrict__ Lt, float4 (&cur)[4], float4 (&nxt)[4], float (&x)[16]) {
+__device__ __forceinline__ void inv16_steps(uint32_t Lt, float4 (&cur)[4], float4 (&nxt)[4], float (&x)[16]) {
     if constexpr (J < 15) {
         if constexpr (J + 1 < 15) inv16_load_row<J + 1>(Lt, nxt);
         inv16_apply_row<J>(cur, x);
         inv16_steps<J + 1>(Lt, nxt, cur, x);
     }
 }
-__device__ __forceinline__ void inv16_columns(const float* __restrict__ Lt, int col, float (&x)[16]) {
+// Lt = shared-space byte address of the block's L^T
+__device__ __forceinline__ void inv16_columns(uint32_t Lt, int col, float (&x)[16]) {
 #pragma unroll
     for (int r = 0; r < 16; ++r) x[r] = (r == col) ? 1.f : 0.f;
     float4 la[4], lb[4];
@@ -224,13 +225,14 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         const float y = __shfl_up_sync(0xffffffffu, x, o);
         if (lane >= o) x += y;
     }
-    if (hh == 0 && lane == 31) sWarp[wq] = x;
+    if (hh == 0 && lane == 31) sts_f32(smem_u32(sWarp) + wq * 4, x);
     __syncthreads();
     const uint32_t tmem = cx.tmem;
     const uint32_t c0 = tmem, c1 = tmem + 128, c2 = tmem + 256, c3 = tmem + 384;
     float gam_i, gam_end;            // Gam_i and Gam at the end of this row's chunk
     {
-        const float w0 = sWarp[0], w1 = sWarp[1], w2 = sWarp[2], w3 = sWarp[3];
+        const float4 w4 = lds_f4(smem_u32(sWarp));
+        const float w0 = w4.x, w1 = w4.y, w2 = w4.z, w3 = w4.w;
         if (C == 128) {
             gam_i = x + (wq > 0 ? w0 : 0.f) + (wq > 1 ? w1 : 0.f) + (wq > 2 ? w2 : 0.f);
             gam_end = w0 + w1 + w2 + w3;
@@ -241,17 +243,17 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     const float gam_ref = __shfl_sync(0xffffffffu, gam_i, 31);     // Gam at the last row of this 32-chunk
     if (hh == 0) {
-        sGam[row] = gam_i;
-        sBeta[row] = beta_i;
-        sBG[row] = beta_i * fast_exp(gam_i);
-        sCF[row] = fast_exp(gam_ref - gam_i);
+        sts_f32(smem_u32(sGam) + row * 4, gam_i);
+        sts_f32(smem_u32(sBeta) + row * 4, beta_i);
+        sts_f32(smem_u32(sBG) + row * 4, beta_i * fast_exp(gam_i));
+        sts_f32(smem_u32(sCF) + row * 4, fast_exp(gam_ref - gam_i));
     }
     __syncthreads();
     const int half_lo = (C == 128) ? 0 : (wq >> 1) * 2;      // first 32-column chunk of this row's chunk
     // decay factors: e^{Gam_i - Gam_j} = rf[cc] * sCF[j] for j in an earlier 32-chunk cc (both factors <= 1)
     float rf[3];
 #pragma unroll
-    for (int cc = 0; cc < 3; ++cc) rf[cc] = (cc < wq && cc >= half_lo) ? fast_exp(gam_i - sGam[cc * 32 + 31]) : 0.f;
+    for (int cc = 0; cc < 3; ++cc) rf[cc] = (cc < wq && cc >= half_lo) ? fast_exp(gam_i - lds_f32(smem_u32(sGam) + (cc * 32 + 31) * 4)) : 0.f;
 
     auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
@@ -333,21 +335,23 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                 v1[e] *= m1 * fast_exp(fminf(gam_i - g1[e], 0.f));
             }
             GDN_STAMP(21);
-            // L^T into the scratch: element (r = lane, j) -> Lq[j][r]
+            // L^T into the scratch: element (r = lane, j) -> Lq[j][r]   (aL: shared-space byte address of Lq, S = row stride)
+            const uint32_t aL = smem_u32(Lq);
+            constexpr uint32_t S = kLsStride * 4;
 #pragma unroll
-            for (int e = 0; e < 16; ++e) { Lq[e * kLsStride + lane] = v0[e]; Lq[(16 + e) * kLsStride + lane] = v1[e]; }
+            for (int e = 0; e < 16; ++e) { sts_f32(aL + e * S + lane * 4, v0[e]); sts_f32(aL + (16 + e) * S + lane * 4, v1[e]); }
             __syncwarp();
             GDN_STAMP(16);
             // Blocked: L = [[L11, 0], [L21, L22]] in 16-blocks, X = [[X11, 0], [-X22 L21 X11, X22]].
             // Step 1 (this warp): lanes 0-15 invert I + L11, lanes 16-31 invert I + L22, each lane one column.
             const int o = lane & 16, col = lane & 15;
             float xc[16];
-            inv16_columns(Lq + o * kLsStride + o, col, xc);
+            inv16_columns(aL + o * S + o * 4, col, xc);
             GDN_STAMP(18);
             __syncwarp();
             // X11 / X22 row-major over L11^T / L22^T (consumed): element (r, col) -> Lq[o + r][o + col]
 #pragma unroll
-            for (int r = 0; r < 16; ++r) Lq[(o + r) * kLsStride + o + col] = xc[r];
+            for (int r = 0; r < 16; ++r) sts_f32(aL + (o + r) * S + (o + col) * 4, xc[r]);
             __syncwarp();
             // Steps 2a, 2b (same warp, lane = row r2 x 8 columns): M = L21 X11 into the free block Lq[16 + r][c] (L^T has
             // nothing there), then X21 = -X22 M in its place, and zeros over L21^T (X's upper-right block).
@@ -357,36 +361,36 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             for (int e = 0; e < 8; ++e) acc[e] = 0.f;
 #pragma unroll
             for (int k = 0; k < 16; ++k) {
-                const float a = Lq[k * kLsStride + 16 + r2];                          // L21[r2][k] = L[16 + r2][k]
-                const float4 b0 = *reinterpret_cast<const float4*>(Lq + k * kLsStride + cc0);       // X11[k][cc0 ..]
-                const float4 b1 = *reinterpret_cast<const float4*>(Lq + k * kLsStride + cc0 + 4);
+                const float a = lds_f32(aL + k * S + (16 + r2) * 4);                  // L21[r2][k] = L[16 + r2][k]
+                const float4 b0 = lds_f4(aL + k * S + cc0 * 4);                       // X11[k][cc0 ..]
+                const float4 b1 = lds_f4(aL + k * S + (cc0 + 4) * 4);
                 acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
                 acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
             }
-            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0) = make_float4(acc[0], acc[1], acc[2], acc[3]);
-            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0 + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
+            sts_f4(aL + (16 + r2) * S + cc0 * 4, make_float4(acc[0], acc[1], acc[2], acc[3]));
+            sts_f4(aL + (16 + r2) * S + (cc0 + 4) * 4, make_float4(acc[4], acc[5], acc[6], acc[7]));
             __syncwarp();
             float xr[16];                                                             // X22[r2][0..15]
 #pragma unroll
             for (int k4 = 0; k4 < 4; ++k4) {
-                const float4 f = *reinterpret_cast<const float4*>(Lq + (16 + r2) * kLsStride + 16 + 4 * k4);
+                const float4 f = lds_f4(aL + (16 + r2) * S + (16 + 4 * k4) * 4);
                 xr[4 * k4] = f.x; xr[4 * k4 + 1] = f.y; xr[4 * k4 + 2] = f.z; xr[4 * k4 + 3] = f.w;
             }
 #pragma unroll
             for (int e = 0; e < 8; ++e) acc[e] = 0.f;
 #pragma unroll
             for (int k = 0; k < 16; ++k) {
-                const float4 b0 = *reinterpret_cast<const float4*>(Lq + (16 + k) * kLsStride + cc0);   // M[k][cc0 ..]
-                const float4 b1 = *reinterpret_cast<const float4*>(Lq + (16 + k) * kLsStride + cc0 + 4);
+                const float4 b0 = lds_f4(aL + (16 + k) * S + cc0 * 4);                // M[k][cc0 ..]
+                const float4 b1 = lds_f4(aL + (16 + k) * S + (cc0 + 4) * 4);
                 const float a = xr[k];
                 acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
                 acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
             }
             __syncwarp();                                                             // every M has been read
-            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0) = make_float4(-acc[0], -acc[1], -acc[2], -acc[3]);
-            *reinterpret_cast<float4*>(Lq + (16 + r2) * kLsStride + cc0 + 4) = make_float4(-acc[4], -acc[5], -acc[6], -acc[7]);
-            *reinterpret_cast<float4*>(Lq + r2 * kLsStride + 16 + cc0) = make_float4(0.f, 0.f, 0.f, 0.f);
-            *reinterpret_cast<float4*>(Lq + r2 * kLsStride + 16 + cc0 + 4) = make_float4(0.f, 0.f, 0.f, 0.f);
+            sts_f4(aL + (16 + r2) * S + cc0 * 4, make_float4(-acc[0], -acc[1], -acc[2], -acc[3]));
+            sts_f4(aL + (16 + r2) * S + (cc0 + 4) * 4, make_float4(-acc[4], -acc[5], -acc[6], -acc[7]));
+            sts_f4(aL + r2 * S + (16 + cc0) * 4, make_float4(0.f, 0.f, 0.f, 0.f));
+            sts_f4(aL + r2 * S + (16 + cc0 + 4) * 4, make_float4(0.f, 0.f, 0.f, 0.f));
             GDN_STAMP(17);
         }
         const uint32_t qbar = 1 + wq, qthreads = 32 * NH;

@@ -305,6 +305,18 @@ __device__ __forceinline__ void store_row8_bf16(uint32_t tile_saddr, uint32_t bl
 }
 __device__ __forceinline__ void store_roww_bf16(uint32_t a, uint32_t bs, int row, int col0, const float (&v)[8]) { store_row8_bf16(a, bs, row, col0, v); }
 __device__ __forceinline__ void store_roww_bf16(uint32_t a, uint32_t bs, int row, int col0, const float (&v)[16]) { store_row16_bf16(a, bs, row, col0, v); }
+// Explicit shared-space accesses by 32-bit address.  A C++ dereference of a pointer that ptxas cannot prove to be shared
+// (e.g. one carried in a struct) becomes a GENERIC LD.E / ST.E, which is noticeably slower on latency-bound code.
+__device__ __forceinline__ float lds_f32(uint32_t a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ float4 lds_f4(uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f4(uint32_t a, float4 v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 __device__ __forceinline__ float4 ld_shared_f4(const float* p) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)) : "memory");
