@@ -168,7 +168,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                         GDN_TRACE(2 * gs);
                         const int gst = gs % GST;
                         if (gs >= (uint32_t)GST) mbar_wait(&g_empty[gst], ((gs / GST) - 1) & 1u);
-                        sGamma[gst] = gam_c;                 // visible to the waiters of g_full through the arrive below
+                        sts_f32(smem_u32(sGamma) + gst * 4, gam_c);      // visible to the waiters of g_full through the arrive below
                         mbar_expect_tx(&g_full[gst], L::GN_BYTES);
                         uint8_t* gb = sG + gst * L::GN_BYTES;
                         const int z = bh * p.NC + c;
@@ -278,7 +278,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 const int gst = gs % GST;
                 if (gs == 12 && tid == 0) GDN_STAMP_ANY(32);
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
-                const float gamma_c = sGamma[gst];
+                const float gamma_c = lds_f32(smem_u32(sGamma) + gst * 4);
                 if (gs == 12 && tid == 0) GDN_STAMP_ANY(33);
                 {   // state-independent half, while the MMA runs: S <- gamma_c S + N_c
                     const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES + half * (D * 128));
