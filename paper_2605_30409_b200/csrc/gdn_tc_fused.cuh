@@ -108,7 +108,9 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
     uint64_t* out_free = out_full + 2;        // [2] output accumulator drained (4 warps)
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(out_free + 2);
     float* sGamma = reinterpret_cast<float*>(smem + L::OFF_GAM);
-    volatile uint32_t* chain_issued = reinterpret_cast<volatile uint32_t*>(smem + L::OFF_GAM + 64);   // chain MMAs issued so far
+    const uint32_t a_issued = smem_u32(smem + L::OFF_GAM + 64);       // chain MMAs issued so far (shared-space word)
+    auto issued_ld = [&]() { uint32_t v; asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a_issued) : "memory"); return v; };
+    auto issued_st = [&](uint32_t v) { asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(a_issued), "r"(v) : "memory"); };
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
@@ -118,7 +120,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
         mbar_init(mma_chain, 1);
         for (int s = 0; s < 2; ++s) { mbar_init(&out_full[s], 1); mbar_init(&out_free[s], 4); }
         mbar_fence_init();
-        *chain_issued = 0;
+        issued_st(0u);
     }
     if (warp == 0) tmem_alloc(tmem_slot, 256);
     tc_fence_before();
@@ -210,7 +212,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     umma_bf16(acc_chain, desc_kmajor(aG + (s >> 2) * (D * 128) + (s & 3) * 32), desc_mnmajor(aS + s * 2048, 0), idc, s > 0);
                 umma_commit(mma_chain);
                 umma_commit(&g_empty[gst]);
-                *chain_issued = gs + 1;                              // the output issuer lets the chain MMA of a step go first
+                issued_st(gs + 1);                                   // the output issuer lets the chain MMA of a step go first
                 if (gs == 12) GDN_STAMP_ANY(42);
             }
         }
@@ -225,7 +227,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 mbar_wait(&s_ready[sb], (o / NSB) & 1u);             // S_o is published
                 mbar_wait(&q_full[qst], (o / QST) & 1u);
                 if (o >= 2) mbar_wait(&out_free[o & 1], ((o >> 1) - 1) & 1u);
-                while (*chain_issued <= o) {}
+                while (issued_ld() <= o) {}
                 tc_fence_after();
                 const uint32_t aQ = smem_u32(sQ + qst * L::Q_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
                 const uint32_t acc_out = tmem + 64 + 64 * (o & 1);
