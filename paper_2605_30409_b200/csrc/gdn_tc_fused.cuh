@@ -48,6 +48,8 @@ __device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) 
 }
 // orders async-proxy accesses (TMA) of any state space with this thread's generic-proxy accesses
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// the same for global memory only: the flag acquire (generic proxy) before the TMA loads of what the flag guards
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 #ifdef GDN_PHASE_TIMING
 __device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
@@ -153,7 +155,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     if (feed_chain && idx < ready) {         // accepted exactly once per chunk
                         gam_l = __ldcg(p.gam + (long long)bh * p.NC + idx);
                         if (GST < 3) {                       // shallow ring: have the summaries waiting in L2
-                            fence_proxy_async_all();
+                            fence_proxy_async_global();
                             const int z = bh * p.NC + idx;
 #pragma unroll
                             for (int nb = 0; nb < NB; ++nb) tma_prefetch_3d(tmG, nb * 64, 0, z);
@@ -165,7 +167,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 }
                 const float gam_c = __shfl_sync(0xffffffffu, gam_l, c - base);
                 if (lane == 0) {
-                    fence_proxy_async_all();
+                    fence_proxy_async_global();
                     if (feed_chain) {
                         GDN_TRACE(2 * gs);
                         const int gst = gs % GST;
