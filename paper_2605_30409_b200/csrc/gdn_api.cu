@@ -39,6 +39,30 @@ struct Staging {
 
 }  // namespace
 
+namespace {
+// release everything the host entry point set up (also after a partial set-up, so that a retry starts clean)
+void staging_free(Staging& h) {
+    void* bufs[] = {h.q, h.k, h.v, h.out, h.alpha, h.beta, h.state};
+    for (void* b : bufs) if (b) cudaFree(b);
+    h.q = h.k = h.v = h.out = nullptr; h.alpha = h.beta = h.state = nullptr;
+    if (h.seg_plan) gdn_destroy(h.seg_plan);
+    if (h.tail_plan) gdn_destroy(h.tail_plan);
+    h.seg_plan = h.tail_plan = nullptr;
+    if (h.s_in) cudaStreamDestroy(h.s_in);
+    if (h.s_out) cudaStreamDestroy(h.s_out);
+    h.s_in = h.s_out = nullptr;
+    if (h.ev_start) cudaEventDestroy(h.ev_start);
+    if (h.ev_out) cudaEventDestroy(h.ev_out);
+    h.ev_start = h.ev_out = nullptr;
+    for (int i = 0; i < kMaxSeg; ++i) {
+        if (h.ev_in[i]) cudaEventDestroy(h.ev_in[i]);
+        if (h.ev_comp[i]) cudaEventDestroy(h.ev_comp[i]);
+        h.ev_in[i] = h.ev_comp[i] = nullptr;
+    }
+    h.ready = false;
+}
+}  // namespace
+
 struct gdn_plan {
     gdn_config_t cfg;
     int device = -1;
@@ -126,6 +150,11 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
     if (out == q || out == k || out == v) return fail(p, GDN_ERR_INVALID_ARG, "out must not alias an input");
     gdn_status_t ds = check_device(p);
     if (ds != GDN_OK) return ds;
+    {   // a plan is bound to the device it was created on (workspace, tensor maps, kernel attributes)
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device)
+            return fail(p, GDN_ERR_INVALID_ARG, "the current device is not the one the plan was created on (device " + std::to_string(p->device) + ")");
+    }
 
     if (p->path != GDN_PATH_SIMT_FP32) {
         std::string msg;
@@ -225,7 +254,7 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
         if (gdn::tc_supported(c, &path, &chunk, &launches)) {
             if (p->device >= 0 && p->cc_major == 10 && p->cc_minor == 0) {
                 gdn_status_t ts = gdn::tc_plan_init(p->tc, c, p->sm_count, &msg);
-                if (ts != GDN_OK) { delete p; return fail(nullptr, ts, msg); }
+                if (ts != GDN_OK) { gdn::tc_plan_free(p->tc); delete p; return fail(nullptr, ts, msg); }
             }
             // frame path: + S^hist kernel with the bidirectional scan (F > 1); the normaliser runs all of it twice
             if (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_BIDIR) && c.T / c.group > 1) launches += 1;
@@ -290,6 +319,8 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
         const int unit = c.group == 1 ? 128 : c.group;
         const int units = (c.T + unit - 1) / unit;
         int nseg = (int)((2 * nq + nv + na + nb) / (16u << 20));
+        // the reverse scan of Alg. 1 l.14-17 runs over ALL frames of the call: a token split is only exact for the forward scan
+        if (c.flags & GDN_FLAG_BIDIR) nseg = 1;
         if (nseg > kMaxSeg) nseg = kMaxSeg;
         if (nseg > units) nseg = units;
         if (nseg < 1) nseg = 1;
@@ -300,15 +331,15 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
         cudaError_t e = cudaSuccess;
         auto alloc = [&](void** ptr, size_t n) { if (e == cudaSuccess) e = cudaMalloc(ptr, n ? n : 16); };
         alloc(&h.q, nq); alloc(&h.k, nq); alloc(&h.v, nv); alloc(&h.out, nv);
-        alloc((void**)&h.alpha, na); alloc((void**)&h.beta, nb); alloc((void**)&h.state, ns);
-        if (e != cudaSuccess) { cudaGetLastError(); return fail(p, GDN_ERR_NOMEM, "host-path staging allocation failed"); }
+        alloc((void**)&h.alpha, na + 16 * kMaxSeg); alloc((void**)&h.beta, nb + 16 * kMaxSeg); alloc((void**)&h.state, ns);
+        if (e != cudaSuccess) { cudaGetLastError(); staging_free(h); return fail(p, GDN_ERR_NOMEM, "host-path staging allocation failed"); }
         if (h.nseg > 1) {
             gdn_config_t sc = c;
             sc.T = h.Tseg;
-            if (gdn_plan(&sc, &h.seg_plan) != GDN_OK) return fail(p, GDN_ERR_NOMEM, std::string("segment plan: ") + g_plan_error);
+            if (gdn_plan(&sc, &h.seg_plan) != GDN_OK) { staging_free(h); return fail(p, GDN_ERR_NOMEM, std::string("segment plan: ") + g_plan_error); }
             if (h.Ttail != h.Tseg) {
                 sc.T = h.Ttail;
-                if (gdn_plan(&sc, &h.tail_plan) != GDN_OK) return fail(p, GDN_ERR_NOMEM, std::string("tail segment plan: ") + g_plan_error);
+                if (gdn_plan(&sc, &h.tail_plan) != GDN_OK) { staging_free(h); return fail(p, GDN_ERR_NOMEM, std::string("tail segment plan: ") + g_plan_error); }
             }
             if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h.s_in, cudaStreamNonBlocking);
             if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h.s_out, cudaStreamNonBlocking);
@@ -318,7 +349,7 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
                 e = cudaEventCreateWithFlags(&h.ev_in[i], cudaEventDisableTiming);
                 if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h.ev_comp[i], cudaEventDisableTiming);
             }
-            if (e != cudaSuccess) return cuda_fail(p, e, "host-path pipeline set-up");
+            if (e != cudaSuccess) { staging_free(h); return cuda_fail(p, e, "host-path pipeline set-up"); }
         }
         h.ready = true;
         p->workspace_bytes += 2 * nq + 2 * nv + na + nb + ns;
@@ -369,7 +400,9 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
         ck(cudaEventRecord(h.ev_comp[sgi], st));
         ck(cudaStreamWaitEvent(h.s_out, h.ev_comp[sgi], 0));
         ck(cudaMemcpy2DAsync((uint8_t*)out_host + t0 * rowv, c.T * rowv, dout, Ts * rowv, Ts * rowv, c.B, cudaMemcpyDeviceToHost, h.s_out));
-        oq += (size_t)c.B * Ts * rowq; ov += (size_t)c.B * Ts * rowv; oa += (size_t)BH * Fs * 4; ob += (size_t)BH * Ts * 4;
+        oq += (size_t)c.B * Ts * rowq; ov += (size_t)c.B * Ts * rowv;
+        oa = (oa + (size_t)BH * Fs * 4 + 15) & ~(size_t)15;     // every segment's gates start 16-byte aligned (forward_impl checks it)
+        ob = (ob + (size_t)BH * Ts * 4 + 15) & ~(size_t)15;
     }
     ck(cudaMemcpyAsync(state_out_host, h.state, ns, cudaMemcpyDeviceToHost, st));
     ck(cudaEventRecord(h.ev_out, h.s_out));
@@ -383,16 +416,7 @@ gdn_status_t gdn_destroy(gdn_plan_t* plan) {
     gdn::tc_plan_free(plan->tc);
     plan->prof.set_enabled(false);
     if (plan->z_stage) cudaFree(plan->z_stage);
-    Staging& h = plan->host;
-    void* bufs[] = {h.q, h.k, h.v, h.out, h.alpha, h.beta, h.state};
-    for (void* b : bufs) if (b) cudaFree(b);
-    if (h.seg_plan) gdn_destroy(h.seg_plan);
-    if (h.tail_plan) gdn_destroy(h.tail_plan);
-    if (h.s_in) cudaStreamDestroy(h.s_in);
-    if (h.s_out) cudaStreamDestroy(h.s_out);
-    if (h.ev_start) cudaEventDestroy(h.ev_start);
-    if (h.ev_out) cudaEventDestroy(h.ev_out);
-    for (int i = 0; i < kMaxSeg; ++i) { if (h.ev_in[i]) cudaEventDestroy(h.ev_in[i]); if (h.ev_comp[i]) cudaEventDestroy(h.ev_comp[i]); }
+    staging_free(plan->host);
     delete plan;
     return GDN_OK;
 }
