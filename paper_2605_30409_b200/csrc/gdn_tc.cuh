@@ -15,6 +15,7 @@
 #include "gdn_tc_token.cuh"
 #include "gdn_tc_frame.cuh"
 #include "gdn_tc_fused.cuh"
+#include "gdn_tc_tile64.cuh"
 #include "tc_tmap.cuh"
 
 namespace gdn {
@@ -31,6 +32,8 @@ struct TcPlan {
     __nv_bfloat16 *Gw = nullptr, *Qt = nullptr, *Ol = nullptr, *Sc = nullptr;
     float *Nw = nullptr, *gam = nullptr, *part = nullptr;
     CUtensorMap tmG, tmN, tmQt, tmOl, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
+    CUtensorMap tmQt64, tmOl64;                      // the same rows with a 64-row box (light 64-token tile workers, d = 64)
+    bool tile64 = false;                             // d = 64, C = 64: summaries by gdn_tok_tile64 (activation boxes of 64 tokens)
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr, *co = nullptr;
     CUtensorMap tmQ, tmK, tmV, tmO;
@@ -255,7 +258,11 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         const uint32_t box[2] = {64, 128};
         ok = ok && tc::make_tmap(&tp.tmQt, tp.Qt, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
         ok = ok && tc::make_tmap(&tp.tmOl, tp.Ol, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        const uint32_t box64[2] = {64, 64};
+        ok = ok && tc::make_tmap(&tp.tmQt64, tp.Qt, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box64, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        ok = ok && tc::make_tmap(&tp.tmOl64, tp.Ol, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims, str, box64, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
+    tp.tile64 = tp.D == 64 && tp.C == 64;
     if (!ok) { cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
     tp.ready = true;
     return GDN_OK;
@@ -305,8 +312,19 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
         attr_done = true;
     }
     if (prof) prof->begin(st);
-    gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmOl, p);
-    if (prof) prof->mark(st, "gdn_tok_prepass");
+    if (D == 64 && C == 64) {
+        static bool attr64 = false;
+        if (!attr64) {
+            cudaError_t e = set_smem(t64::gdn_tok_tile64, t64::SMEM_BYTES);
+            if (e != cudaSuccess) return e;
+            attr64 = true;
+        }
+        t64::gdn_tok_tile64<<<tp.BH * tp.NC, t64::kThreads, t64::SMEM_BYTES, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt64, tp.tmOl64, p);
+        if (prof) prof->mark(st, "gdn_tok_tile64");
+    } else {
+        gdn_tok_prepass<D, C><<<tp.BH * tp.NT, kPrepassThreads, smem1, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmOl, p);
+        if (prof) prof->mark(st, "gdn_tok_prepass");
+    }
     cudaError_t le = launch_pdl(gdn_tok_chain<D>, dim3(tp.BH * (D / 64)), dim3(kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, p);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_chain");
@@ -393,9 +411,10 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     auto ts = [&](long long s, int d) { return s ? s : (long long)c.H * d; };
     if (q != tp.cq || k != tp.ck || v != tp.cv) {
         const int Gm = (tp.mode == GDN_PATH_TC_FRAME) ? c.group : c.T;      // token-wise: one "frame" of T tokens
-        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, Gm, ts(c.q_token_stride, c.d_k), 128, err) &&
-                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, Gm, ts(c.k_token_stride, c.d_k), 128, err) &&
-                  tc::make_act_tmap(&tp.tmV, v, c.B, c.T, c.H, c.d_v, Gm, ts(c.v_token_stride, c.d_v), 128, err);
+        const int rows = tp.tile64 ? 64 : 128;
+        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, Gm, ts(c.q_token_stride, c.d_k), rows, err) &&
+                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, Gm, ts(c.k_token_stride, c.d_k), rows, err) &&
+                  tc::make_act_tmap(&tp.tmV, v, c.B, c.T, c.H, c.d_v, Gm, ts(c.v_token_stride, c.d_v), rows, err);
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
     }

@@ -93,10 +93,10 @@ constexpr int kLsStride = 36;                     // floats per row: 16-byte ali
 // 16x16 unit-lower-triangular inverse: Lt[j*kLsStride + r] = L[r][j] (r, j < 16), the calling lane owns column `col` of
 // X = (I + L)^-1.  Two of these (the two diagonal 16-blocks of a 32-block) run in the two halves of one warp with
 // different base pointers.
-template <int J>
+template <int J, int LS>
 __device__ __forceinline__ void inv16_load_row(uint32_t Lt, float4 (&l)[4]) {
 #pragma unroll
-    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) l[r4] = lds_f4(Lt + (J * kLsStride + 4 * r4) * 4);
+    for (int r4 = (J + 1) / 4; r4 < 4; ++r4) l[r4] = lds_f4(Lt + (J * LS + 4 * r4) * 4);
 }
 template <int J>
 __device__ __forceinline__ void inv16_apply_row(const float4 (&l)[4], float (&x)[16]) {
@@ -109,21 +109,22 @@ __device__ __forceinline__ void inv16_apply_row(const float4 (&l)[4], float (&x)
         if (4 * r4 + 3 > J) x[4 * r4 + 3] = fmaf(-l[r4].w, xj, x[4 * r4 + 3]);
     }
 }
-template <int J>
+template <int J, int LS>
 __device__ __forceinline__ void inv16_steps(uint32_t Lt, float4 (&cur)[4], float4 (&nxt)[4], float (&x)[16]) {
     if constexpr (J < 15) {
-        if constexpr (J + 1 < 15) inv16_load_row<J + 1>(Lt, nxt);
+        if constexpr (J + 1 < 15) inv16_load_row<J + 1, LS>(Lt, nxt);
         inv16_apply_row<J>(cur, x);
-        inv16_steps<J + 1>(Lt, nxt, cur, x);
+        inv16_steps<J + 1, LS>(Lt, nxt, cur, x);
     }
 }
-// Lt = shared-space byte address of the block's L^T
+// Lt = shared-space byte address of the block's L^T, LS = floats per scratch row
+template <int LS = kLsStride>
 __device__ __forceinline__ void inv16_columns(uint32_t Lt, int col, float (&x)[16]) {
 #pragma unroll
     for (int r = 0; r < 16; ++r) x[r] = (r == col) ? 1.f : 0.f;
     float4 la[4], lb[4];
-    inv16_load_row<0>(Lt, la);
-    inv16_steps<0>(Lt, la, lb, x);
+    inv16_load_row<0, LS>(Lt, la);
+    inv16_steps<0, LS>(Lt, la, lb, x);
 }
 
 // Shared-memory carve-up and barriers of one prepass CTA (set up once; a persistent CTA runs many tiles).
