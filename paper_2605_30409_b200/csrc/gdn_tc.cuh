@@ -501,6 +501,9 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fprintf(stderr, " [5->19:%lld 19->20:%lld 20->21:%lld 21->16:%lld 16->18:%lld 18->17:%lld 17->6:%lld]", hst[19] - hst[5], hst[20] - hst[19], hst[21] - hst[20], hst[16] - hst[21], hst[18] - hst[16], hst[17] - hst[18], hst[6] - hst[17]);
         fprintf(stderr, " [T1: 3->23 issue:%lld wait_all:%lld 24->4:%lld]", hst[23] - hst[3], hst[24] - hst[23], hst[4] - hst[24]);
         fprintf(stderr, " tile(0->14):%lld total:%lld\n", hst[14] - hst[0], hst[15] - hst[0]);
+        fprintf(stderr, "[t64 tid64]");
+        for (int i = 1; i < 15; ++i) fprintf(stderr, " %d:%lld", i, hst[32 + i] - hst[32 + i - 1]);
+        fprintf(stderr, "\n");
         fprintf(stderr, "[gdn chain step cycles] snapshot:%lld premath:%lld wait_mma:%lld ld+sub:%lld publish:%lld fence+sync:%lld total:%lld\n",
                 hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36], hst[38] - hst[37], hst[38] - hst[32]);
         fprintf(stderr, "[gdn fused chain step 12] prev-publish->top:%lld gfull+gam:%lld Nfma:%lld wait_mma:%lld ld+sub:%lld publish:%lld | mma warp: sready-seen@%lld commit@%lld (rel. to top) state-mma-done@%lld\n",

@@ -30,15 +30,15 @@ namespace t64 {
 using namespace tc;
 
 constexpr int kThreads = 128;
-constexpr int kLS = 68;                               // floats per row of the fp32 inversion scratch (16-byte aligned rows)
 constexpr uint32_t kTile = 8192;                      // one [64][64] bf16 tile (128-byte rows, 128-byte swizzle)
 constexpr uint32_t OFF_K = 0;                         // K tile  } the stacked K-major A operand of S1; K alone is its B operand
 constexpr uint32_t OFF_Q = 8192;                      // Q tile  }   later: Kt in place / Qt in place
 constexpr uint32_t OFF_V = 16384;                     // V tile; later Ol
 constexpr uint32_t OFF_PT = 24576;                    // P^T [j][i] bf16; later the staging of G
-constexpr uint32_t OFF_X = 32768;                     // fp32 scratch [64][kLS] -> [Tm diag(beta gamma) ; Tm diag(beta)] bf16 [128][64]
+constexpr uint32_t OFF_X = 32768;                     // L_bf | D_bf (bf16 [64][64] each) | fp32 diagonal 16-blocks (4 KB)
+                                                      //   -> [Tm diag(beta gamma) ; Tm diag(beta)] bf16 [128][64]
                                                       //   -> [W | Ut] bf16 2 x [64][64] -> staging of N
-constexpr uint32_t X_BYTES = 64u * kLS * 4u;          // 17408
+constexpr uint32_t X_BYTES = 2 * kTile + 4096;
 constexpr uint32_t OFF_VEC = OFF_X + X_BYTES;         // Gam[64], Beta[64], BG[64], KS[64], CF[32]
 constexpr uint32_t OFF_BAR = OFF_VEC + 1280;
 constexpr uint32_t SMEM_BYTES = OFF_BAR + 64 + 1024;  // + slack for the 1024-byte alignment of the dynamic base
@@ -49,7 +49,27 @@ struct Tile64Maps {
     const CUtensorMap *tmQt, *tmOl;                   // workspace rows, box {64, 64}
 };
 
+#ifdef GDN_PHASE_TIMING
+#define T64_STAMP(n) do { if (p.dbg && blockIdx.x == p.dbg_cta && (tid & 63) == 0) p.dbg[(n) + (tid >> 6) * 32] = clock64(); } while (0)
+#else
+#define T64_STAMP(n) do { } while (0)
+#endif
+
 __device__ __forceinline__ void sts_b16(uint32_t a, unsigned short v) { asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
+
+__device__ __forceinline__ void sts_b32(uint32_t a, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+// warp-level matrix loads / MMA for the small blocks of the triangular inverse (see tile64)
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t a) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t (&r)[4], uint32_t a) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(a) : "memory");
+}
+// d += a (16x16, row) * b (16x8, col), bf16 operands, fp32 accumulate
+__device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
 
 // One 64-token chunk `chunk` of stream `bh`.  smem: 1024-byte aligned base; tmem: 128 columns; bars: 4 mbarriers
 // (K+Q landed, V landed, MMA complete, spare) initialised to count 1; `use` = how many chunks this CTA has run before.
@@ -67,6 +87,7 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     const int i = tid & 63;                           // token row inside the chunk (both halves of the CTA)
     const uint32_t lane_base = (uint32_t)(warp * 32);
 
+    T64_STAMP(0);
     if (tid == 0) {
         mbar_expect_tx(bar_kq, 2 * kTile);
         tma_load_5d(smem + OFF_K, mp.tmK, bar_kq, 0, h, chunk * 64, 0, b);
@@ -104,8 +125,10 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
 
+    T64_STAMP(1);
     // ---- S1: [K ; Q] K^T -> TMEM columns 0..63 ----
     mbar_wait(bar_kq, par);
+    T64_STAMP(2);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, 64, false, false);
@@ -114,11 +137,13 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         umma_commit(bar_mma);
     }
     wait_mma();
+    T64_STAMP(3);
 
-    // ---- S1 epilogue.  warps 0-1 (row i of K K^T): L_ij = beta_i e^{Gam_i-Gam_j} k_i.k_j (j < i), stored TRANSPOSED in
-    //      the fp32 scratch M (M[j][i] = L[i][j]: "column j of L" is then a row of 16-byte loads); warps 2-3 (row i of
-    //      Q K^T): P_ij = e^{Gam_i-Gam_j} q_i.k_j (j <= i) -> bf16 P^T[j][i].  Inside a 32-column block the exponent is
-    //      taken directly; across blocks e^{Gam_i-Gam_j} = e^{Gam_i-Gam_31} e^{Gam_31-Gam_j} (both factors <= 1).
+    // ---- S1 epilogue.  warps 0-1 (row i of K K^T): L_ij = beta_i e^{Gam_i-Gam_j} k_i.k_j (j < i) -> bf16 row of L_bf, and
+    //      its diagonal 16-block TRANSPOSED in fp32 -> scratch (for the forward substitution); warps 2-3 (row i of Q K^T):
+    //      P_ij = e^{Gam_i-Gam_j} q_i.k_j (j <= i) -> bf16 P^T[j][i].  Inside a 32-column block the exponent is taken
+    //      directly; across blocks e^{Gam_i-Gam_j} = e^{Gam_i-Gam_31} e^{Gam_31-Gam_j} (both factors <= 1).
+    const uint32_t aLB = aX, aDB = aX + kTile, aSC = aX + 2 * kTile;
     {
         const int ci = warp & 1;                      // 32-block of this row
         const bool is_l = warp < 2;
@@ -149,13 +174,19 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
                     }
                 }
             } else {
-                if (is_l) continue;                   // M[j >= 32][i < 32] is the lower-left block: written by the inversion
+                if (is_l) continue;                   // L above the diagonal blocks is never read
 #pragma unroll
                 for (int j = 0; j < 32; ++j) v[j] = 0.f;
             }
             if (is_l) {
+                store_row32_bf16(aLB, 0, i, 32 * hc, v);
+                if (hc == ci) {
+                    // diagonal 16-block (i >> 4): Lt[jl][i & 15] = L[i][16 (i >> 4) + jl]
+                    const uint32_t dst = aSC + (uint32_t)(i >> 4) * 1024u + (uint32_t)(i & 15) * 4u;
+                    const bool hi = (lane & 16) != 0;
 #pragma unroll
-                for (int j = 0; j < 32; ++j) sts_f32(aX + ((hc * 32 + j) * kLS + i) * 4, v[j]);
+                    for (int jl = 0; jl < 16; ++jl) sts_f32(dst + jl * 64, hi ? v[16 + jl] : v[jl]);
+                }
             } else {
                 const uint32_t colb = aPT + (uint32_t)((i & 7) * 2);
 #pragma unroll
@@ -166,117 +197,124 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             }
         }
     }
+    T64_STAMP(4);
 
-    // ---- (I + L)^-1 in fp32, in place in M.  After each stage the finished diagonal blocks hold X row-major (zeros
-    //      above the diagonal) and the blocks above them still hold L^T.
-    constexpr uint32_t S = kLS * 4;
+    // ---- Tm = (I + L)^-1 -> D_bf (bf16, swizzled rows).  Diagonal 16-blocks: fp32 forward substitution on CUDA cores
+    //      (tok::inv16_columns, one column per lane).  16 -> 32 -> 64: X21 = -X22 (L21 X11) with warp-level mma.sync on
+    //      the bf16 blocks: these products are 16^3 / 32^3, far below the M >= 64 tile of tcgen05.mma and not worth an
+    //      asynchronous TMEM round trip each; the transposed first product (L21 X11)^T = X11^T L21^T leaves its fp32
+    //      accumulator fragments in exactly the layout of the second product's B fragments, so nothing goes through memory.
+    const int qm = lane >> 3, rr = lane & 7;          // ldmatrix: this lane addresses row rr of matrix qm
+    const int g8 = lane >> 2, c2 = (lane & 3) * 2;    // mma fragments: row g8, column pair c2
+    auto tile_addr = [](uint32_t base, int r, int chunk) { return base + (uint32_t)r * 128u + (uint32_t)((chunk ^ (r & 7)) << 4); };
     if (warp < 2) {
-        // 16-blocks: the two halves of warp w invert the two diagonal 16-blocks of 32-block w, one column per lane
-        // (right-looking forward substitution, tok::inv16_columns); then X21 = -X22 (L21 X11) of the 32-block.
         __syncwarp();
-        const uint32_t aL = aX + (uint32_t)(32 * warp * kLS + 32 * warp) * 4;
-        const int o = lane & 16, col = lane & 15;
-        float xc[16];
-        tok::inv16_columns<kLS>(aL + o * S + o * 4, col, xc);
-        __syncwarp();
+        {
+            const int bi = 2 * warp + (lane >> 4), col = lane & 15;
+            float xc[16];
+            tok::inv16_columns<16>(aSC + (uint32_t)bi * 1024u, col, xc);
+            const int cg = 16 * bi + col;             // column of D_bf
 #pragma unroll
-        for (int r = 0; r < 16; ++r) sts_f32(aL + (o + r) * S + (o + col) * 4, xc[r]);
-        __syncwarp();
-        const int r2 = lane >> 1, cc0 = (lane & 1) * 8;
-        float acc[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const float a = lds_f32(aL + k * S + (16 + r2) * 4);                  // L21[r2][k]
-            const float4 b0 = lds_f4(aL + k * S + cc0 * 4);                       // X11[k][cc0 ..]
-            const float4 b1 = lds_f4(aL + k * S + (cc0 + 4) * 4);
-            acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
-            acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
+            for (int r = 0; r < 16; ++r) {
+                const int R = 16 * bi + r;
+                sts_b16(tile_addr(aDB, R, cg >> 3) + (uint32_t)(cg & 7) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(xc[r])));
+            }
+            // zeros above the 16-blocks inside this warp's 32-block: rows 32w .. 32w+15, columns 32w+16 .. 32w+31
+            st_shared_v4(tile_addr(aDB, 32 * warp + (lane >> 1), 4 * warp + 2 + (lane & 1)), 0u, 0u, 0u, 0u);
         }
-        sts_f4(aL + (16 + r2) * S + cc0 * 4, make_float4(acc[0], acc[1], acc[2], acc[3]));          // M1 into the free lower-left block
-        sts_f4(aL + (16 + r2) * S + (cc0 + 4) * 4, make_float4(acc[4], acc[5], acc[6], acc[7]));
         __syncwarp();
-        float xr[16];                                                             // X22[r2][0..15]
+        const int b0 = 32 * warp;
+        uint32_t a[4], bb[4], a2[4];
+        ldsm_x4_trans(a, tile_addr(aDB, b0 + (qm >> 1) * 8 + rr, 4 * warp + (qm & 1)));              // X00^T
+        ldsm_x4(bb, tile_addr(aLB, b0 + 16 + (qm >> 1) * 8 + rr, 4 * warp + (qm & 1)));              // L10^T as [n][k]
+        ldsm_x4(a2, tile_addr(aDB, b0 + 16 + (qm & 1) * 8 + rr, 4 * warp + 2 + (qm >> 1)));          // X11
+        float t0[4] = {0.f, 0.f, 0.f, 0.f}, t1[4] = {0.f, 0.f, 0.f, 0.f};
+        mma_bf16_16816(t0, a, bb[0], bb[1]);
+        mma_bf16_16816(t1, a, bb[2], bb[3]);
+        float y0[4] = {0.f, 0.f, 0.f, 0.f}, y1[4] = {0.f, 0.f, 0.f, 0.f};
+        mma_bf16_16816(y0, a2, pack_bf16(t0[0], t0[1]), pack_bf16(t1[0], t1[1]));
+        mma_bf16_16816(y1, a2, pack_bf16(t0[2], t0[3]), pack_bf16(t1[2], t1[3]));
+        // X10 = -Y: rows b0+16+g8 (+8), columns b0 + 8 j2 + c2
 #pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-            const float4 f = lds_f4(aL + (16 + r2) * S + (16 + 4 * k4) * 4);
-            xr[4 * k4] = f.x; xr[4 * k4 + 1] = f.y; xr[4 * k4 + 2] = f.z; xr[4 * k4 + 3] = f.w;
+        for (int j2 = 0; j2 < 2; ++j2) {
+            const float* y = j2 ? y1 : y0;
+            const int C = b0 + 8 * j2 + c2;
+            const int R0 = b0 + 16 + g8, R1 = R0 + 8;
+            sts_b32(tile_addr(aDB, R0, C >> 3) + (uint32_t)(C & 7) * 2u, pack_bf16(-y[0], -y[1]));
+            sts_b32(tile_addr(aDB, R1, C >> 3) + (uint32_t)(C & 7) * 2u, pack_bf16(-y[2], -y[3]));
         }
-#pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const float4 b0 = lds_f4(aL + (16 + k) * S + cc0 * 4);                // M1[k][cc0 ..]
-            const float4 b1 = lds_f4(aL + (16 + k) * S + (cc0 + 4) * 4);
-            const float a = xr[k];
-            acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
-            acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
-        }
-        __syncwarp();                                                             // every M1 has been read
-        sts_f4(aL + (16 + r2) * S + cc0 * 4, make_float4(-acc[0], -acc[1], -acc[2], -acc[3]));
-        sts_f4(aL + (16 + r2) * S + (cc0 + 4) * 4, make_float4(-acc[4], -acc[5], -acc[6], -acc[7]));
-        sts_f4(aL + r2 * S + (16 + cc0) * 4, make_float4(0.f, 0.f, 0.f, 0.f));    // zeros over L21^T
-        sts_f4(aL + r2 * S + (16 + cc0 + 4) * 4, make_float4(0.f, 0.f, 0.f, 0.f));
     }
+    T64_STAMP(5);
     __syncthreads();
+    T64_STAMP(6);
     {
-        // 32 -> 64, all four warps: Y21 = -Y22 (L21 Y11), Y11 = M[0:32][0:32], Y22 = M[32:64][32:64] (both clean
-        // lower-triangular), L21^T = M[0:32][32:64].  Thread (r, c8): row r of the block, eight columns.
-        const int r = tid >> 2, c8 = (tid & 3) * 8;
-        float acc[8];
+        // 32 -> 64, all four warps: warp (mt, m2) = (warp & 1, warp >> 1) produces Y21[16 m2 .. +15][16 mt .. +15],
+        // Y21 = -Y22 (L21 Y11), Y11 = D_bf[0:32][0:32], Y22 = D_bf[32:64][32:64], L21 = L_bf[32:64][0:32].
+        const int mt = warp & 1, m2 = warp >> 1;
+        float t[4][4];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-#pragma unroll 8
-        for (int k = 0; k < 32; ++k) {
-            const float a = lds_f32(aX + (k * kLS + 32 + r) * 4);                 // L[32 + r][k]
-            const float4 b0 = lds_f4(aX + (k * kLS + c8) * 4);                    // Y11[k][c8 ..] (zero for k < column)
-            const float4 b1 = lds_f4(aX + (k * kLS + c8 + 4) * 4);
-            acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
-            acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
+        for (int n = 0; n < 4; ++n)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) t[n][e] = 0.f;
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks) {
+            uint32_t a[4];
+            ldsm_x4_trans(a, tile_addr(aDB, 16 * ks + (qm >> 1) * 8 + rr, 2 * mt + (qm & 1)));       // Y11^T, rows c of tile mt
+#pragma unroll
+            for (int np = 0; np < 2; ++np) {
+                uint32_t bb[4];
+                ldsm_x4(bb, tile_addr(aLB, 32 + 16 * np + (qm >> 1) * 8 + rr, 2 * ks + (qm & 1)));   // L21^T as [n = r][k]
+                mma_bf16_16816(t[2 * np], a, bb[0], bb[1]);
+                mma_bf16_16816(t[2 * np + 1], a, bb[2], bb[3]);
+            }
         }
-        sts_f4(aX + ((32 + r) * kLS + c8) * 4, make_float4(acc[0], acc[1], acc[2], acc[3]));        // M1 -> lower-left block
-        sts_f4(aX + ((32 + r) * kLS + c8 + 4) * 4, make_float4(acc[4], acc[5], acc[6], acc[7]));
-        float yr[32];                                                             // Y22[r][0..31] (zero beyond the diagonal)
+        float y[2][4];
 #pragma unroll
-        for (int k4 = 0; k4 < 8; ++k4) {
-            const float4 f = lds_f4(aX + ((32 + r) * kLS + 32 + 4 * k4) * 4);
-            yr[4 * k4] = f.x; yr[4 * k4 + 1] = f.y; yr[4 * k4 + 2] = f.z; yr[4 * k4 + 3] = f.w;
+        for (int j2 = 0; j2 < 2; ++j2)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) y[j2][e] = 0.f;
+#pragma unroll
+        for (int ks2 = 0; ks2 < 2; ++ks2) {
+            uint32_t a2[4];
+            ldsm_x4(a2, tile_addr(aDB, 32 + 16 * m2 + (qm & 1) * 8 + rr, 4 + 2 * ks2 + (qm >> 1)));  // Y22 rows of tile m2
+            mma_bf16_16816(y[0], a2, pack_bf16(t[2 * ks2][0], t[2 * ks2][1]), pack_bf16(t[2 * ks2 + 1][0], t[2 * ks2 + 1][1]));
+            mma_bf16_16816(y[1], a2, pack_bf16(t[2 * ks2][2], t[2 * ks2][3]), pack_bf16(t[2 * ks2 + 1][2], t[2 * ks2 + 1][3]));
         }
-        __syncthreads();
 #pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-#pragma unroll
-        for (int k = 0; k < 32; ++k) {
-            const float4 b0 = lds_f4(aX + ((32 + k) * kLS + c8) * 4);             // M1[k][c8 ..]
-            const float4 b1 = lds_f4(aX + ((32 + k) * kLS + c8 + 4) * 4);
-            const float a = yr[k];
-            acc[0] = fmaf(a, b0.x, acc[0]); acc[1] = fmaf(a, b0.y, acc[1]); acc[2] = fmaf(a, b0.z, acc[2]); acc[3] = fmaf(a, b0.w, acc[3]);
-            acc[4] = fmaf(a, b1.x, acc[4]); acc[5] = fmaf(a, b1.y, acc[5]); acc[6] = fmaf(a, b1.z, acc[6]); acc[7] = fmaf(a, b1.w, acc[7]);
+        for (int j2 = 0; j2 < 2; ++j2) {
+            const int C = 16 * mt + 8 * j2 + c2;
+            const int R0 = 32 + 16 * m2 + g8, R1 = R0 + 8;
+            sts_b32(tile_addr(aDB, R0, C >> 3) + (uint32_t)(C & 7) * 2u, pack_bf16(-y[j2][0], -y[j2][1]));
+            sts_b32(tile_addr(aDB, R1, C >> 3) + (uint32_t)(C & 7) * 2u, pack_bf16(-y[j2][2], -y[j2][3]));
         }
-        __syncthreads();                                                          // every M1 has been read
-        sts_f4(aX + ((32 + r) * kLS + c8) * 4, make_float4(-acc[0], -acc[1], -acc[2], -acc[3]));
-        sts_f4(aX + ((32 + r) * kLS + c8 + 4) * 4, make_float4(-acc[4], -acc[5], -acc[6], -acc[7]));
     }
     __syncthreads();
-    // ---- the two scaled copies of Tm, stacked as ONE K-major A operand [128][64] written over the scratch:
-    //      rows 0-63 = Tm diag(beta gamma) (thread half 0), rows 64-127 = Tm diag(beta) (half 1) ----
+    T64_STAMP(7);
+    // ---- the two scaled copies of Tm, stacked as ONE K-major A operand [128][64] written over L_bf / D_bf:
+    //      rows 0-63 = Tm diag(beta gamma) (thread half 0), rows 64-127 = Tm diag(beta) (half 1).  Columns 32..63 of
+    //      the rows below 32 were never written: zero.
     {
         const uint32_t vec = (tid < 64) ? aBG : aBeta;
+        const int nch = (i < 32) ? 4 : 8;             // warp-uniform
         uint32_t pk[32];
 #pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const float4 f = lds_f4(aX + (i * kLS + 4 * q) * 4);                  // Tm[i][4q ..]; above the diagonal: L^T leftovers
-            const float4 s = lds_f4(vec + 16 * q);
-            const float v0 = (4 * q + 0 <= i) ? f.x * s.x : 0.f, v1 = (4 * q + 1 <= i) ? f.y * s.y : 0.f;
-            const float v2 = (4 * q + 2 <= i) ? f.z * s.z : 0.f, v3 = (4 * q + 3 <= i) ? f.w * s.w : 0.f;
-            pk[2 * q] = pack_bf16(v0, v1); pk[2 * q + 1] = pack_bf16(v2, v3);
+        for (int c = 0; c < 8; ++c) {
+            if (c < nch) {
+                float f[8];
+                unpack8(ld_shared_v4(tile_addr(aDB, i, c)), f);
+                const float4 s0 = lds_f4(vec + 32 * c), s1 = lds_f4(vec + 32 * c + 16);
+                pk[4 * c] = pack_bf16(f[0] * s0.x, f[1] * s0.y); pk[4 * c + 1] = pack_bf16(f[2] * s0.z, f[3] * s0.w);
+                pk[4 * c + 2] = pack_bf16(f[4] * s1.x, f[5] * s1.y); pk[4 * c + 3] = pack_bf16(f[6] * s1.z, f[7] * s1.w);
+            } else {
+                pk[4 * c] = pk[4 * c + 1] = pk[4 * c + 2] = pk[4 * c + 3] = 0u;
+            }
         }
-        __syncthreads();                                                          // the scratch has been read by everyone
+        __syncthreads();                                                          // D_bf has been read by everyone
 #pragma unroll
         for (int c = 0; c < 8; ++c) st_shared_v4(aX + swz_chunk_off(row, c, 0), pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
     }
     sync_then_issue();
+    T64_STAMP(8);
 
     // ---- S3: [Tm diag(beta gamma) ; Tm diag(beta)] [K | V] -> TMEM columns 0..127 ----
     if (tid == 0) {
@@ -288,6 +326,7 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         umma_commit(bar_mma);
     }
     wait_mma();
+    T64_STAMP(9);
     {
         // lanes 0-63: W = columns 0..63 -> block 0 of [W | Ut]; lanes 64-127: Ut = columns 64..127 -> block 1
         float v[64];
@@ -309,6 +348,7 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         }
     }
     sync_then_issue();
+    T64_STAMP(10);
 
     // ---- S4: [Kt | P^T]^T [W | Ut] -> lanes 0-63: [G | N] rows, lanes 64-127: [P W | P Ut] rows ----
     if (tid == 0) {
@@ -319,6 +359,7 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         umma_commit(bar_mma);
     }
     wait_mma();
+    T64_STAMP(11);
     if (tid < 64) {
         // summary row m = tid: G bf16 -> the P^T buffer, N fp32 as two [64][32] blocks -> the scratch (both operands are dead)
         const int m = tid;
@@ -356,9 +397,11 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             }
         }
     }
+    T64_STAMP(12);
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
+    T64_STAMP(13);
     if (tid == 0) {
         const int r0 = (int)((long long)bh * p.NT * 128 + (long long)chunk * 64);
         const int z = bh * p.NC + chunk;
@@ -394,6 +437,7 @@ gdn_tok_tile64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     Tile64Maps mp{&tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmOl};
     tile64(smem, tmem, bars, mp, p, (int)blockIdx.x / p.NC, (int)blockIdx.x % p.NC, 0u);
     if (threadIdx.x == 0) tma_store_wait_all();
+    { const int tid = threadIdx.x; T64_STAMP(14); }
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x < 32) tmem_dealloc(tmem, 128);
