@@ -16,6 +16,7 @@
 #include "gdn_tc_frame.cuh"
 #include "gdn_tc_fused.cuh"
 #include "gdn_tc_tile64.cuh"
+#include "gdn_tc_fused64.cuh"
 #include "tc_tmap.cuh"
 
 namespace gdn {
@@ -34,6 +35,10 @@ struct TcPlan {
     CUtensorMap tmG, tmN, tmQt, tmOl, tmSc, tmScS;   // static (workspace) maps; tmScS: [D][64] store box of the chain
     CUtensorMap tmQt64, tmOl64;                      // the same rows with a 64-row box (light 64-token tile workers, d = 64)
     bool tile64 = false;                             // d = 64, C = 64: summaries by gdn_tok_tile64 (activation boxes of 64 tokens)
+    // d = 64, C = 64, single persistent kernel with the two-level scan (gdn_tc_fused64.cuh)
+    bool fused64 = false;
+    F64Params f64{};                                 // workspace pointers / offsets; per-call fields filled at launch
+    CUtensorMap tmM3, tmR2;
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr, *co = nullptr;
     CUtensorMap tmQ, tmK, tmV, tmO;
@@ -78,7 +83,7 @@ inline bool tc_supported(const gdn_config_t& c, gdn_path_t* path, int* chunk, in
     }
     *path = GDN_PATH_TC_TOKEN;
     *chunk = tc_default_chunk(c);
-    *launches = (*chunk == 128 && !(c.flags & GDN_FLAG_UNFUSED)) ? 1 : 3;
+    *launches = ((*chunk == 128 || c.d_k == 64) && !(c.flags & GDN_FLAG_UNFUSED)) ? 1 : 3;
     return true;
 }
 
@@ -171,6 +176,65 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     return GDN_OK;
 }
 
+
+// d = 64, C = 64 token path as one persistent kernel: workspace, flags, the two workspace tensor maps, role split.
+inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int sm_count, std::string* err) {
+    const int sms = sm_count > 0 ? sm_count : 148;
+    const int BH = tp.BH, NC = (c.T + 63) / 64;
+    tp.NC = NC; tp.NSc = NC; tp.fused64 = true; tp.tile64 = true;
+    // segments: chain CTAs (2 NS - 1 per stream) may take up to a quarter of the 4-per-SM CTA slots
+    int NS = 1;
+    while (NS < 4 && (NS + 1) * 2 <= NC && BH * (2 * (NS + 1) - 1) <= sms) ++NS;
+    const int LSEG = (NC + NS - 1) / NS;
+    NS = (NC + LSEG - 1) / LSEG;
+    F64Params& f = tp.f64;
+    f.NS = NS; f.LSEG = LSEG; f.NCH = BH * (1 + 2 * (NS - 1));
+    const size_t nchunk = (size_t)BH * NC, nseg = (size_t)BH * NS;
+    f.zG = 0; f.zN = (int)nchunk; f.zSc = (int)(2 * nchunk); f.zGA = (int)(3 * nchunk); f.zGs = (int)(4 * nchunk); f.zBs = (int)(4 * nchunk + nseg);
+    const size_t slots = 4 * nchunk + 2 * nseg, rows = 2 * nchunk * 64;
+    f.rQt = 0; f.rOl = (long long)(nchunk * 64);
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
+    const size_t oM3 = carve(slots * 8192), oR2 = carve(rows * 128), oGam = carve(nchunk * 4), oGacc = carve(nchunk * 4), oGseg = carve(nseg * 4);
+    const size_t oSegS = carve(nseg * 4096 * 4), oFl = carve((3 * nchunk + 3 * nseg + 2) * 4);
+    if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
+        cudaGetLastError();
+        if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
+        return GDN_ERR_NOMEM;
+    }
+    tp.workspace_bytes = off;
+    uint8_t* w = static_cast<uint8_t*>(tp.workspace);
+    tp.gam = reinterpret_cast<float*>(w + oGam);
+    f.gacc = reinterpret_cast<float*>(w + oGacc);
+    f.gseg = reinterpret_cast<float*>(w + oGseg);
+    f.SegS = reinterpret_cast<float*>(w + oSegS);
+    unsigned int* fl = reinterpret_cast<unsigned int*>(w + oFl);
+    f.f_tile = fl; f.f_snap = fl + nchunk; f.f_snapA = fl + 2 * nchunk;
+    f.f_segA = fl + 3 * nchunk; f.f_segB = f.f_segA + nseg; f.f_segS = f.f_segB + nseg; f.ctr = f.f_segS + nseg;
+    if (cudaMemset(fl, 0, (3 * nchunk + 3 * nseg + 2) * 4) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
+        if (err) *err = "flag initialisation failed";
+        return GDN_ERR_CUDA;
+    }
+    f.n_tile_tasks = LSEG * NS * BH; f.n_out_tasks = LSEG * NS * BH;
+    long long grid = (long long)f.NCH + f.n_tile_tasks;
+    if (grid > 4LL * sms) grid = 4LL * sms;
+    if (grid < f.NCH + 1) grid = f.NCH + 1;
+    tp.grid = (int)grid;
+    bool ok = true;
+    {
+        const uint64_t dims[3] = {64, 64, slots}, str[3] = {2, 128, 8192};
+        const uint32_t box[3] = {64, 64, 1};
+        ok = ok && tc::make_tmap(&tp.tmM3, w + oM3, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+        const uint64_t dims2[2] = {64, rows}, str2[2] = {2, 128};
+        const uint32_t box2[2] = {64, 64};
+        ok = ok && tc::make_tmap(&tp.tmR2, w + oR2, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, dims2, str2, box2, CU_TENSOR_MAP_SWIZZLE_128B, err);
+    }
+    if (!ok) { cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
+    tp.ready = true;
+    return GDN_OK;
+}
+
 inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count, std::string* err) {
     if (c.group != 1) return tc_plan_init_frame(tp, c, sm_count, err);
     tp.mode = GDN_PATH_TC_TOKEN;
@@ -181,6 +245,7 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     tp.NT = (c.T + 127) / 128;
     tp.NC = tp.C == 128 ? tp.NT : 2 * tp.NT;
     tp.NSc = tp.NC;
+    if (tp.D == 64 && tp.C == 64 && c.d_k == 64 && !(c.flags & GDN_FLAG_UNFUSED)) return tc_plan_init_fused64(tp, c, sm_count, err);
     const size_t D = tp.D, BH = tp.BH, NT = tp.NT, NC = tp.NC;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
@@ -354,6 +419,23 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
     return cudaGetLastError();
 }
 
+
+inline cudaError_t tc_launch_fused64(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = set_smem(f64::gdn_tok_fused64, t64::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    F64Params fp = tp.f64;
+    fp.t = p;
+    fp.epoch = ++tp.epoch;
+    if (prof) prof->begin(st);
+    f64::gdn_tok_fused64<<<tp.grid, t64::kThreads, t64::SMEM_BYTES, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmO, tp.tmM3, tp.tmR2, fp);
+    if (prof) prof->mark(st, "gdn_tok_fused64");
+    return cudaGetLastError();
+}
+
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
                                    const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
@@ -418,9 +500,9 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
     }
-    if ((tp.fused || tp.mode == GDN_PATH_TC_FRAME) && out != tp.co) {
+    if ((tp.fused || tp.fused64 || tp.mode == GDN_PATH_TC_FRAME) && out != tp.co) {
         const int Gm = (tp.mode == GDN_PATH_TC_FRAME) ? c.group : c.T;
-        if (!tc::make_act_tmap(&tp.tmO, out, c.B, c.T, c.H, c.d_v, Gm, ts(c.o_token_stride, c.d_v), 128, err)) { tp.co = nullptr; return GDN_ERR_CUDA; }
+        if (!tc::make_act_tmap(&tp.tmO, out, c.B, c.T, c.H, c.d_v, Gm, ts(c.o_token_stride, c.d_v), tp.fused64 ? 64 : 128, err)) { tp.co = nullptr; return GDN_ERR_CUDA; }
         tp.co = out;
     }
     if (tp.mode == GDN_PATH_TC_FRAME) {
@@ -487,7 +569,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.dbg_cta = tp.fused ? tp.NWC : 0;
 #endif
     cudaError_t e;
-    if (tp.fused) e = (tp.D == 64) ? tc_launch_fused<64>(tp, p, st, prof) : tc_launch_fused<128>(tp, p, st, prof);
+    if (tp.fused64) e = tc_launch_fused64(tp, p, st, prof);
+    else if (tp.fused) e = (tp.D == 64) ? tc_launch_fused<64>(tp, p, st, prof) : tc_launch_fused<128>(tp, p, st, prof);
     else if (tp.D == 64) e = (tp.C == 128) ? tc_launch_token<64, 128>(tp, p, st, prof) : tc_launch_token<64, 64>(tp, p, st, prof);
     else            e = (tp.C == 128) ? tc_launch_token<128, 128>(tp, p, st, prof) : tc_launch_token<128, 64>(tp, p, st, prof);
     if (e != cudaSuccess) { if (err) *err = std::string("token tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }

@@ -45,8 +45,11 @@ constexpr uint32_t SMEM_BYTES = OFF_BAR + 64 + 1024;  // + slack for the 1024-by
 
 struct Tile64Maps {
     const CUtensorMap *tmQ, *tmK, *tmV;               // activations, box [64 tokens][64 features]
-    const CUtensorMap *tmG, *tmN;                     // G bf16 box {64, 64, 1}; N fp32 box {32, 64, 1}
+    const CUtensorMap *tmG, *tmN;                     // G bf16 box {64, 64, 1}; N fp32 box {32, 64, 1} (NBF16: bf16 like G)
     const CUtensorMap *tmQt, *tmOl;                   // workspace rows, box {64, 64}
+    int zG, zN;                                       // first summary slot of G / N in their maps
+    long long rows_per_bh;                            // Qt / Ol rows per stream
+    long long rQt, rOl;                               // first row of Qt / Ol in their maps
 };
 
 #ifdef GDN_PHASE_TIMING
@@ -72,17 +75,19 @@ __device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a
 }
 
 // One 64-token chunk `chunk` of stream `bh`.  smem: 1024-byte aligned base; tmem: 128 columns; bars: 4 mbarriers
-// (K+Q landed, V landed, MMA complete, spare) initialised to count 1; `use` = how many chunks this CTA has run before.
+// (K+Q landed, V landed, MMA complete, spare) initialised to count 1; `pl` / `ph` = running parities of the two load
+// barriers (both complete one phase per chunk) and of the MMA barrier, kept by the caller across tasks.
+template <bool NBF16>
 __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* bars, const Tile64Maps& mp, const TokParams& p,
-                                       int bh, int chunk, uint32_t use) {
+                                       int bh, int chunk, uint32_t& pl, uint32_t& ph) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = bh / p.H, h = bh % p.H;
     const uint32_t aK = smem_u32(smem + OFF_K), aQ = smem_u32(smem + OFF_Q), aV = smem_u32(smem + OFF_V);
     const uint32_t aPT = smem_u32(smem + OFF_PT), aX = smem_u32(smem + OFF_X), aVec = smem_u32(smem + OFF_VEC);
     const uint32_t aGam = aVec, aBeta = aVec + 256, aBG = aVec + 512, aKS = aVec + 768, aCF = aVec + 1024;
     uint64_t *bar_kq = &bars[0], *bar_v = &bars[1], *bar_mma = &bars[2];
-    const uint32_t par = use & 1u;
-    uint32_t ph = (3u * use) & 1u;                    // bar_mma completes three phases per chunk
+    const uint32_t par = pl;
+    pl ^= 1u;
     const int row = tid;                              // TMEM lane
     const int i = tid & 63;                           // token row inside the chunk (both halves of the CTA)
     const uint32_t lane_base = (uint32_t)(warp * 32);
@@ -370,12 +375,19 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             st_shared_v4(aPT + swz_chunk_off(m, c, 0), pack_bf16(v[8 * c], v[8 * c + 1]), pack_bf16(v[8 * c + 2], v[8 * c + 3]),
                          pack_bf16(v[8 * c + 4], v[8 * c + 5]), pack_bf16(v[8 * c + 6], v[8 * c + 7]));
         tmem_ld64(tmem_addr(tmem, lane_base, 64), v);
+        if (NBF16) {
 #pragma unroll
-        for (int cc = 0; cc < 2; ++cc)
+            for (int c = 0; c < 8; ++c)
+                st_shared_v4(aX + swz_chunk_off(m, c, 0), pack_bf16(v[8 * c], v[8 * c + 1]), pack_bf16(v[8 * c + 2], v[8 * c + 3]),
+                             pack_bf16(v[8 * c + 4], v[8 * c + 5]), pack_bf16(v[8 * c + 6], v[8 * c + 7]));
+        } else {
 #pragma unroll
-            for (int q = 0; q < 8; ++q)
-                st_shared_v4(aX + cc * kTile + (uint32_t)m * 128u + (uint32_t)((q ^ (m & 7)) << 4), __float_as_uint(v[cc * 32 + 4 * q]),
-                             __float_as_uint(v[cc * 32 + 4 * q + 1]), __float_as_uint(v[cc * 32 + 4 * q + 2]), __float_as_uint(v[cc * 32 + 4 * q + 3]));
+            for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    st_shared_v4(aX + cc * kTile + (uint32_t)m * 128u + (uint32_t)((q ^ (m & 7)) << 4), __float_as_uint(v[cc * 32 + 4 * q]),
+                                 __float_as_uint(v[cc * 32 + 4 * q + 1]), __float_as_uint(v[cc * 32 + 4 * q + 2]), __float_as_uint(v[cc * 32 + 4 * q + 3]));
+        }
     } else {
         // token row i: Qt = gamma_i Q - P W in place, Ol = P Ut over V
         const float gamma_i = fast_exp(gam_i);
@@ -403,13 +415,13 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     __syncthreads();
     T64_STAMP(13);
     if (tid == 0) {
-        const int r0 = (int)((long long)bh * p.NT * 128 + (long long)chunk * 64);
+        const long long r0 = (long long)bh * mp.rows_per_bh + (long long)chunk * 64;
         const int z = bh * p.NC + chunk;
-        tma_store_2d(mp.tmQt, smem + OFF_Q, 0, r0);
-        tma_store_2d(mp.tmOl, smem + OFF_V, 0, r0);
-        tma_store_3d(mp.tmG, smem + OFF_PT, 0, 0, z);
-        tma_store_3d(mp.tmN, smem + OFF_X, 0, 0, z);
-        tma_store_3d(mp.tmN, smem + OFF_X + kTile, 32, 0, z);
+        tma_store_2d(mp.tmQt, smem + OFF_Q, 0, (int)(mp.rQt + r0));
+        tma_store_2d(mp.tmOl, smem + OFF_V, 0, (int)(mp.rOl + r0));
+        tma_store_3d(mp.tmG, smem + OFF_PT, 0, 0, mp.zG + z);
+        tma_store_3d(mp.tmN, smem + OFF_X, 0, 0, mp.zN + z);
+        if (!NBF16) tma_store_3d(mp.tmN, smem + OFF_X + kTile, 32, 0, mp.zN + z);
         tma_store_commit();
         p.gam[(long long)bh * p.NC + chunk] = fast_exp(gam_C);
     }
@@ -434,8 +446,9 @@ gdn_tok_tile64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     pdl_launch_dependents();
-    Tile64Maps mp{&tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmOl};
-    tile64(smem, tmem, bars, mp, p, (int)blockIdx.x / p.NC, (int)blockIdx.x % p.NC, 0u);
+    Tile64Maps mp{&tmQ, &tmK, &tmV, &tmG, &tmN, &tmQt, &tmOl, 0, 0, (long long)p.NT * 128, 0, 0};
+    uint32_t pl = 0, ph = 0;
+    tile64<false>(smem, tmem, bars, mp, p, (int)blockIdx.x / p.NC, (int)blockIdx.x % p.NC, pl, ph);
     if (threadIdx.x == 0) tma_store_wait_all();
     { const int tid = threadIdx.x; T64_STAMP(14); }
     tc_fence_before();
