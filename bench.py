@@ -238,7 +238,7 @@ def run_ours(args):
     first = (gin.make_normalizer_inputs if norm else gin.make_inputs)(wl)
     state = first.state.to(dev)
     zstate = first.extras["z_in"].to(dev) if norm else None
-    flags = (gdn.GDN_FLAG_NORMALIZER if norm else 0) | (gdn.GDN_FLAG_BIDIR if args.bidir else 0)
+    flags = (gdn.GDN_FLAG_NORMALIZER if norm else 0) | (gdn.GDN_FLAG_BIDIR if args.bidir else 0) | (gdn.GDN_FLAG_UNFUSED if args.unfused else 0)
     plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, chunk=wl.chunk, flags=flags,
                        io_dtype=gdn.GDN_BF16 if wl.dtype == torch.bfloat16 else gdn.GDN_FP32)
     info = plan.info
@@ -423,6 +423,7 @@ def main():
     ap.add_argument("--bidir", action="store_true", help="frame mode: bidirectional in-chunk scan (Alg. 1)")
     ap.add_argument("--paper-shape", action="store_true", help="3 x 880 tokens, 20 heads, d = 128, frame-wise")
     ap.add_argument("--d112", action="store_true", help="with --paper-shape: unpadded head dim 112")
+    ap.add_argument("--unfused", action="store_true", help="token mode: the three-kernel path (prepass / chain / output) for A/B runs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

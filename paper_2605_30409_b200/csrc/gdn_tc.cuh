@@ -190,13 +190,14 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     F64Params& f = tp.f64;
     f.NS = NS; f.LSEG = LSEG; f.NCH = BH * (1 + 2 * (NS - 1));
     const size_t nchunk = (size_t)BH * NC, nseg = (size_t)BH * NS;
-    f.zG = 0; f.zN = (int)nchunk; f.zSc = (int)(2 * nchunk); f.zGA = (int)(3 * nchunk); f.zGs = (int)(4 * nchunk); f.zBs = (int)(4 * nchunk + nseg);
-    const size_t slots = 4 * nchunk + 2 * nseg, rows = 2 * nchunk * 64;
+    f.zG = 0; f.zN = (int)nchunk; f.zSc = (int)(2 * nchunk); f.zGA = (int)(3 * nchunk);
+    f.zGs = (int)(4 * nchunk); f.zBs = (int)(4 * nchunk + nseg); f.zSk = (int)(4 * nchunk + 2 * nseg);
+    const size_t slots = 4 * nchunk + 3 * nseg, rows = 2 * nchunk * 64;
     f.rQt = 0; f.rOl = (long long)(nchunk * 64);
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
-    const size_t oM3 = carve(slots * 8192), oR2 = carve(rows * 128), oGam = carve(nchunk * 4), oGacc = carve(nchunk * 4), oGseg = carve(nseg * 4);
-    const size_t oSegS = carve(nseg * 4096 * 4), oFl = carve((3 * nchunk + 3 * nseg + 2) * 4);
+    const size_t nflag = 3 * nchunk + 3 * nseg;
+    const size_t oM3 = carve(slots * 8192), oR2 = carve(rows * 128), oFl = carve(nflag * 8 + f64::kCtlWords * 4);
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -204,14 +205,11 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     }
     tp.workspace_bytes = off;
     uint8_t* w = static_cast<uint8_t*>(tp.workspace);
-    tp.gam = reinterpret_cast<float*>(w + oGam);
-    f.gacc = reinterpret_cast<float*>(w + oGacc);
-    f.gseg = reinterpret_cast<float*>(w + oGseg);
-    f.SegS = reinterpret_cast<float*>(w + oSegS);
-    unsigned int* fl = reinterpret_cast<unsigned int*>(w + oFl);
+    unsigned long long* fl = reinterpret_cast<unsigned long long*>(w + oFl);
     f.f_tile = fl; f.f_snap = fl + nchunk; f.f_snapA = fl + 2 * nchunk;
-    f.f_segA = fl + 3 * nchunk; f.f_segB = f.f_segA + nseg; f.f_segS = f.f_segB + nseg; f.ctr = f.f_segS + nseg;
-    if (cudaMemset(fl, 0, (3 * nchunk + 3 * nseg + 2) * 4) != cudaSuccess) {
+    f.f_segA = fl + 3 * nchunk; f.f_segB = f.f_segA + nseg; f.f_segS = f.f_segB + nseg;
+    f.ctl = reinterpret_cast<unsigned int*>(f.f_segS + nseg);
+    if (cudaMemset(fl, 0, nflag * 8 + f64::kCtlWords * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "flag initialisation failed";
         return GDN_ERR_CUDA;
@@ -221,6 +219,8 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     if (grid > 4LL * sms) grid = 4LL * sms;
     if (grid < f.NCH + 1) grid = f.NCH + 1;
     tp.grid = (int)grid;
+    const int cps = (int)((grid + sms - 1) / sms);                 // CTAs the block scheduler puts on one SM
+    f.NCSM = (f.NCH + cps - 1) / cps;
     bool ok = true;
     {
         const uint64_t dims[3] = {64, 64, slots}, str[3] = {2, 128, 8192};
@@ -562,7 +562,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.dbg = nullptr; p.dbg_cta = 0;
 #ifdef GDN_PHASE_TIMING
     static long long* dbg_dev = nullptr;
-    constexpr size_t kDbgWords = 64 + 160 * 128;      // 64 phase stamps + 128 trace slots per CTA
+    constexpr size_t kDbgWords = 64 + 600 * 192;      // 64 phase stamps + 128 trace slots per CTA
     if (!dbg_dev) cudaMalloc(&dbg_dev, kDbgWords * sizeof(long long));
     cudaMemsetAsync(dbg_dev, 0, kDbgWords * sizeof(long long), st);
     p.dbg = dbg_dev;
@@ -592,7 +592,21 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fprintf(stderr, "[gdn fused chain step 12] prev-publish->top:%lld gfull+gam:%lld Nfma:%lld wait_mma:%lld ld+sub:%lld publish:%lld | mma warp: sready-seen@%lld commit@%lld (rel. to top) state-mma-done@%lld\n",
                 hst[32] - hst[31], hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36],
                 hst[41] - hst[32], hst[42] - hst[32], hst[35] - hst[32]);
-        if (const char* tf = getenv("GDN_TRACE_FILE")) {      // fused kernel: per-CTA globaltimer trace
+        if (const char* tf = tp.fused64 ? getenv("GDN_TRACE_FILE") : nullptr) {
+            std::vector<long long> tr(kDbgWords);
+            cudaMemcpy(tr.data(), p.dbg, kDbgWords * sizeof(long long), cudaMemcpyDeviceToHost);
+            if (FILE* f = fopen(tf, "w")) {
+                fprintf(f, "grid %d nch %d ntile %d", tp.grid, tp.f64.NCH, tp.f64.n_tile_tasks);
+                for (int i = 100; i < 140; ++i) fprintf(f, " %lld", tr[64 + i]);
+                fprintf(f, "\n");
+                for (int cta = 0; cta < tp.grid && cta < 600; ++cta) {
+                    fprintf(f, "%d", cta);
+                    for (int i = 0; i < 192; ++i) fprintf(f, " %lld", tr[64 + (size_t)cta * 192 + i]);
+                    fprintf(f, "\n");
+                }
+                fclose(f);
+            }
+        } else if (const char* tf = getenv("GDN_TRACE_FILE")) {      // fused kernel: per-CTA globaltimer trace
             std::vector<long long> tr(kDbgWords);
             cudaMemcpy(tr.data(), p.dbg, kDbgWords * sizeof(long long), cudaMemcpyDeviceToHost);
             if (FILE* f = fopen(tf, "w")) {

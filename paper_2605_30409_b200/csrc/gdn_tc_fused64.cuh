@@ -13,7 +13,7 @@
 //
 // All CTAs have the footprint of a tile worker (128 threads, ~56 KB, 128 TMEM columns; four per SM).  Roles by blockIdx:
 //   chain CTAs (the first NCH):  P(bh)     plain scan of segment 0 from state_in, then the NS-1 level-2 steps; leaves
-//                                          S_c (bf16) per chunk, S_k (fp32) per segment, state_out;
+//                                          S_c (bf16) per chunk, S_k (bf16) per segment, state_out (fp32);
 //                                B(bh,k)   the B part of segment k from zero  -> B_c per chunk, B_k of the whole segment;
 //                                A(bh,k)   the Gacc part of segment k from zero -> Gacc_c, gacc_c per chunk, and per segment.
 //     One step = ONE M = 64 MMA G_c x (bf16 state) with the fp32 master copy of the state row in registers.
@@ -32,48 +32,89 @@
 namespace gdn {
 
 struct F64Params {
-    TokParams t;                 // alpha, beta, S_in, S_out, out, gam, B, H, T, NC (chunks of 64 per stream), scale, log_alpha
+    TokParams t;                 // alpha, beta, S_in, S_out, out, B, H, T, NC (chunks of 64 per stream), scale, log_alpha
     int NS, LSEG;                // segments per stream, chunks per segment (the last segment may be shorter)
     int NCH;                     // chain CTAs = BH * (1 + 2 (NS - 1))
-    int zG, zN, zSc, zGA, zGs, zBs;     // first [64][64] bf16 slot of each array in the 3-D workspace map
+    int zG, zN, zSc, zGA, zGs, zBs, zSk;   // first [64][64] bf16 slot of each array in the 3-D workspace map
     long long rQt, rOl;          // first row of Qt / Ol in the 2-D workspace map
-    float* gacc;                 // [BH][NC]  gacc_c (prefix inside its segment)
-    float* gseg;                 // [BH][NS]  gamma of the whole segment
-    float* SegS;                 // [BH][NS][64][64] fp32 state at the start of segment k >= 1
-    unsigned int *f_tile, *f_snap, *f_snapA;      // [BH][NC]
-    unsigned int *f_segA, *f_segB, *f_segS;       // [BH][NS]
+    // flag words: low half = epoch of the call that published the item, high half = an fp32 payload
+    unsigned long long *f_tile;  // [BH][NC]  tile summaries of chunk c complete; payload gamma_c
+    unsigned long long *f_snap;  // [BH][NC]  S_c (segment 0) / B_c (segment k >= 1) stored
+    unsigned long long *f_snapA; // [BH][NC]  Gacc_c stored; payload gacc_c
+    unsigned long long *f_segA;  // [BH][NS]  Gacc of the whole segment stored; payload gamma of the segment
+    unsigned long long *f_segB;  // [BH][NS]  B of the whole segment stored
+    unsigned long long *f_segS;  // [BH][NS]  S_k (state at the start of segment k) stored
     unsigned int epoch;
-    unsigned int* ctr;           // [0] task counter, [1] finished CTAs (the last one resets both)
+    unsigned int* ctl;           // kCtlWords control words, all zero between calls (the last CTA of a call clears them):
+                                 //   [0] task counter, [1] finished CTAs, [2] SMs seen, [3] chain units claimed,
+                                 //   [16 ..] CTAs arrived per SM id, [16 + kMaxSm ..] 1 + arrival rank of the SM
+    int NCSM;                    // SMs reserved for chain CTAs: the first NCSM SMs on which a CTA of the grid starts
     int n_tile_tasks, n_out_tasks;
 };
 
 namespace f64 {
 
+constexpr int kMaxSm = 512;                           // upper bound of %smid
+constexpr int kCtlWords = 16 + 2 * kMaxSm;
+constexpr bool kStepRelease = false;                  // chain CTAs release their snapshot flags per step (true) or all at the end
+
+#ifdef GDN_PHASE_TIMING
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define F64_TRACE(slot, val) do { if (fp.t.dbg && threadIdx.x == 0 && (slot) < 192) fp.t.dbg[64 + (long long)blockIdx.x * 192 + (slot)] = (val); } while (0)
+#else
+#define F64_TRACE(slot, val) do { } while (0)
+#endif
+#ifdef GDN_PHASE_TIMING
+#define F64_STAMP(slot) do { if (fp.t.dbg && unit == 0 && e == nchunk + 1) fp.t.dbg[64 + (slot)] = clock64(); } while (0)
+#else
+#define F64_STAMP(slot) do { } while (0)
+#endif
+
 using namespace tc;
 using t64::kTile;
 
-__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+__device__ __forceinline__ unsigned long long ld_acquire64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+__device__ __forceinline__ void st_release64(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long flag_word(unsigned int epoch, float payload) {
+    return ((unsigned long long)__float_as_uint(payload) << 32) | (unsigned long long)epoch;
+}
+__device__ __forceinline__ bool flag_ready(unsigned long long w, unsigned int epoch) { return (unsigned int)w >= epoch; }
+__device__ __forceinline__ float flag_payload(unsigned long long w) { return __uint_as_float((unsigned int)(w >> 32)); }
+// Polling uses relaxed loads (an acquire load invalidates the SM's whole L1 every time, which the other CTAs of the SM
+// feel); ONE acquire fence follows once everything an action needs has been observed (acquire_after_poll).
+__device__ __forceinline__ unsigned long long ld_relaxed64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void acquire_after_poll() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ unsigned long long wait_flag(const unsigned long long* f, unsigned int epoch, unsigned int ns = 20) {
+    unsigned long long w = ld_relaxed64(f);
+    while (!flag_ready(w, epoch)) { __nanosleep(ns); w = ld_relaxed64(f); }
+    return w;
 }
 __device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
-__device__ __forceinline__ void wait_flag(const unsigned int* f, unsigned int epoch) {
-    while (ld_acquire_gpu(f) < epoch) __nanosleep(20);
-}
 __device__ __forceinline__ void tma_store_wait_but1() { asm volatile("cp.async.bulk.wait_group 1;" ::: "memory"); }
 
 // shared-memory carve-up of a chain CTA (same allocation as a tile worker)
-constexpr uint32_t C_STAGE = 2 * kTile;               // G_c | N_c (bf16 [64][64] each)
+constexpr uint32_t C_STAGE = 2 * kTile;               // G | N of an entry (bf16 [64][64] each)
 constexpr uint32_t C_OFF_SB = 2 * C_STAGE;            // two bf16 state operand buffers
-constexpr uint32_t C_OFF_GAM = C_OFF_SB + 2 * kTile;  // gamma of the chunk in each stage
+constexpr uint32_t C_OFF_GAM = C_OFF_SB + 2 * kTile;  // gamma of the entry in each stage
+constexpr uint32_t C_OFF_GH = C_OFF_GAM + 16;         // gamma of every entry done (replayed for the flag payloads), up to 1024 entries
 
 // ---------------------------------------------------------------------------------------------------
-// chain CTA.  Thread (warp w, lane l < 16) owns state row m = 16 w + l (the TMEM lanes of an M = 64 accumulator);
-// thread 0 is also the producer (flag polling, TMA) and the MMA issuer.
+// chain CTA.  Thread (warp w, lane l < 16) owns state row m = 16 w + l (the TMEM lanes of an M = 64 accumulator).
+// The CTA walks a list of ENTRIES (G, N, gamma): the chunks of its segment and, for P, the maps of the segments 1..NS-1
+// behind them (level 2).  Before entry e the bf16 operand buffer holds the state that entry e acts on; it is stored as
+// the snapshot of that entry.  The chores of a step are spread over three warps so that none of them delays its warp's share
+// of the state update: thread 0 issues the MMA, thread 32 stores the snapshot and releases the flag of the previous one,
+// thread 64 pulls entry e+1 (its flag word was requested a step earlier, so nothing waits for L2).
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_t* bars, const CUtensorMap* tmM3, const F64Params& fp, int unit) {
     const TokParams& p = fp.t;
@@ -83,11 +124,20 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     if (unit < BH) { bh = unit; type = 0; k = 0; }
     else { const int u = unit - BH; bh = u / (2 * (NS - 1)); const int r = u % (2 * (NS - 1)); k = 1 + (r >> 1); type = 1 + (r & 1); }
     const int c_lo = k * fp.LSEG, c_hi = min(c_lo + fp.LSEG, NC);
+    const int nchunk = c_hi - c_lo, n = nchunk + (type == 0 ? NS - 1 : 0);
     const int m = 16 * warp + lane;
-    const bool act = lane < 16;
+    const bool act = lane < 16, add_g = type == 2;
     const uint32_t aSt = smem_u32(smem), aSb = smem_u32(smem + C_OFF_SB), aGam = smem_u32(smem + C_OFF_GAM);
     uint64_t *full = &bars[0], *bar_mma = &bars[2];
     const unsigned int ep = fp.epoch;
+    const long long cb = (long long)bh * NC, sb = (long long)bh * NS;
+    // entry e -> operands, readiness flags, snapshot slot and flag
+    auto e_zg = [&](int e) { return e < nchunk ? fp.zG + (int)cb + c_lo + e : fp.zGs + (int)sb + (e - nchunk + 1); };
+    auto e_zn = [&](int e) { return add_g ? -1 : (e < nchunk ? fp.zN + (int)cb + c_lo + e : fp.zBs + (int)sb + (e - nchunk + 1)); };
+    auto e_f0 = [&](int e) { return e < nchunk ? fp.f_tile + cb + c_lo + e : fp.f_segA + sb + (e - nchunk + 1); };
+    auto e_f1 = [&](int e) -> const unsigned long long* { return e < nchunk ? nullptr : fp.f_segB + sb + (e - nchunk + 1); };
+    auto e_snap_z = [&](int e) { return e < nchunk ? (add_g ? fp.zGA : fp.zSc) + (int)cb + c_lo + e : fp.zSk + (int)sb + (e - nchunk + 1); };
+    auto e_snap_f = [&](int e) { return e < nchunk ? (add_g ? fp.f_snapA : fp.f_snap) + cb + c_lo + e : fp.f_segS + sb + (e - nchunk + 1); };
 
     float S[64];
 #pragma unroll
@@ -97,7 +147,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
 #pragma unroll
         for (int q = 0; q < 16; ++q) { const float4 f = __ldcg(src + q); S[4 * q] = f.x; S[4 * q + 1] = f.y; S[4 * q + 2] = f.z; S[4 * q + 3] = f.w; }
     }
-    float gacc = 1.f;
+    float gacc = 1.f;                                 // gamma accumulated over the entries done so far
     auto publish = [&](int buf) {                     // bf16 copy of the state rows -> MN-major B operand `buf`
         if (act) {
             const uint32_t base = aSb + buf * kTile;
@@ -108,39 +158,72 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
         }
         fence_proxy_async();
     };
-    // thread 0: wait for the flags of an entry, then pull its operands into stage `st`
-    auto issue_load = [&](int st, int zg, int zn, const unsigned int* f0, const unsigned int* f1, const float* gsrc) {
-        wait_flag(f0, ep);
-        if (f1) wait_flag(f1, ep);
-        sts_f32(aGam + st * 4, __ldcg(gsrc));
+    // thread 64: entry e is ready (w0 = its first flag word); pull it into stage e & 1
+    auto issue_load = [&](int e, unsigned long long w0) {
+        const int st = e & 1;
+        sts_f32(aGam + st * 4, flag_payload(w0));
         fence_proxy_async_global();
+        const int zn = e_zn(e);
         mbar_expect_tx(&full[st], zn >= 0 ? 2 * kTile : kTile);
-        tma_load_3d(smem + st * C_STAGE, tmM3, &full[st], 0, 0, zg);
+        tma_load_3d(smem + st * C_STAGE, tmM3, &full[st], 0, 0, e_zg(e));
         if (zn >= 0) tma_load_3d(smem + st * C_STAGE + kTile, tmM3, &full[st], 0, 0, zn);
     };
-    uint32_t nstep = 0;                               // steps done (stage / operand buffer / parity bookkeeping)
-    // One step on the entry loaded in stage nstep & 1.  add_g: the additive term is gacc G_c (type A) instead of N_c.
-    // Thread 0, behind the MMA issue: stores the operand buffer (= the state BEFORE this entry) as snapshot `snap_z`,
-    // releases the flag of the previous snapshot (whose store has had a whole step to complete), pulls the next entry.
-    auto step = [&](bool add_g, int snap_z, unsigned int* prev_flag, float* gacc_dst, bool has_next, int nzg, int nzn,
-                    const unsigned int* nf0, const unsigned int* nf1, const float* ngsrc) {
-        const int st = nstep & 1;
-        mbar_wait(&full[st], (nstep >> 1) & 1u);
-        if (tid == 0) {
-            tc_fence_after();
-            const uint32_t id = umma_idesc(64, 64, false, true);
-            const uint32_t aG = aSt + st * C_STAGE, aB = aSb + (nstep & 1) * kTile;
+    F64_TRACE(128, (long long)(1000 + type));
+    F64_TRACE(0, gtime());
+    F64_TRACE(160, clock64()); F64_TRACE(161, gtime());
+    unsigned long long nf0 = 0ull, nf1 = 0ull;       // thread 64: flag words of entry e + 1, requested during step e - 1
+    if (tid == 64) {
+        unsigned long long w0 = wait_flag(e_f0(0), ep);
+        if (e_f1(0)) wait_flag(e_f1(0), ep);
+        acquire_after_poll();
+        issue_load(0, w0);
+        if (n > 1) { nf0 = ld_relaxed64(e_f0(1)); nf1 = e_f1(1) ? ld_relaxed64(e_f1(1)) : ~0ull; }
+#ifdef GDN_PHASE_TIMING
+        if (fp.t.dbg) fp.t.dbg[64 + (long long)blockIdx.x * 192 + 150] = gtime();
+#endif
+    }
+    publish(0);
+    __syncthreads();
+    auto gam_hist = [&](int e) { return lds_f32(aGam + 16 + (e < 1024 ? e : 1023) * 4); };
+    float gh1 = 1.f, gh2 = 1.f, gh3 = 1.f;            // gacc before the last three entries (payload of the trailing flags)
+    for (int e = 0; e < n; ++e) {
+        const int st = e & 1;
+        if (tid == 0) F64_STAMP(100); if (tid == 32) F64_STAMP(110); if (tid == 64) F64_STAMP(120); if (tid == 96) F64_STAMP(130);
+        mbar_wait(&full[st], (uint32_t)(e >> 1) & 1u);
+        if (tid == 0) F64_STAMP(101); if (tid == 32) F64_STAMP(111); if (tid == 64) F64_STAMP(121); if (tid == 96) F64_STAMP(131);
+        if (warp == 0) {
+            // issued under elect.sync: with a plain `tid == 0` every tcgen05.mma sits in a ~70-cycle "waterfall" loop
+            // (ptxas cannot keep its operands in uniform registers), which on this serial chain is exposed latency
+            if (elect_one()) {
+                tc_fence_after();
+                const uint32_t id = umma_idesc(64, 64, false, true);
+                const uint32_t aG = aSt + st * C_STAGE, aB = aSb + st * kTile;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) umma_bf16(tmem, desc_kmajor(aG + s * 32), desc_mnmajor(aB + s * 2048, 0), id, s > 0);
-            umma_commit(bar_mma);
-            if (gacc_dst) *gacc_dst = gacc;
-            if (snap_z >= 0) { tma_store_3d(tmM3, smem + C_OFF_SB + (nstep & 1) * kTile, 0, 0, snap_z); tma_store_commit(); }
-            if (prev_flag) {
-                if (snap_z >= 0) tma_store_wait_but1(); else tma_store_wait_all();
-                st_release_gpu(prev_flag, ep);
+                for (int s = 0; s < 4; ++s) umma_bf16(tmem, desc_kmajor(aG + s * 32), desc_mnmajor(aB + s * 2048, 0), id, s > 0);
+                umma_commit(bar_mma);
             }
-            if (has_next) issue_load(st ^ 1, nzg, nzn, nf0, nf1, ngsrc);
+            __syncwarp();
+            } else if (tid == 64) {
+            if (e + 1 < n) {                          // stage (e + 1) & 1 was released by the barrier that ended step e - 1
+                while (!flag_ready(nf0, ep)) { __nanosleep(40); nf0 = ld_relaxed64(e_f0(e + 1)); }
+                while (!flag_ready(nf1, ep)) { __nanosleep(40); nf1 = ld_relaxed64(e_f1(e + 1)); }
+                acquire_after_poll();
+                issue_load(e + 1, nf0);
+                if (e + 2 < n) { nf0 = ld_relaxed64(e_f0(e + 2)); nf1 = e_f1(e + 2) ? ld_relaxed64(e_f1(e + 2)) : ~0ull; }
+            }
+        } else if (tid == 32) {
+            // snapshot of the state entry e acts on.  Its buffer is rewritten at the end of step e + 1: by then the store
+            // must have READ it (checked one step later, cheap).  Its flag needs the store to be COMPLETE, which takes
+            // longer than a step: flags trail by three steps so that the chain never waits for a store's round trip.
+            tma_store_3d(tmM3, smem + C_OFF_SB + st * kTile, 0, 0, e_snap_z(e));
+            tma_store_commit();
+            asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+            if (kStepRelease && e >= 3) {
+                asm volatile("cp.async.bulk.wait_group 3;" ::: "memory");
+                st_release64(e_snap_f(e - 3), flag_word(ep, gh3));
+            }
         }
+        if (tid == 0) F64_STAMP(102); if (tid == 32) F64_STAMP(112); if (tid == 64) F64_STAMP(122); if (tid == 96) F64_STAMP(132);
         const float gamma = lds_f32(aGam + st * 4);
         if (act) {                                    // state-independent half, while the MMA runs
             const uint32_t src = aSt + st * C_STAGE + (add_g ? 0u : kTile);
@@ -150,71 +233,56 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
                 float f[8];
                 unpack8(ld_shared_v4(src + swz_chunk_off(m, c, 0)), f);
 #pragma unroll
-                for (int e = 0; e < 8; ++e) S[8 * c + e] = fmaf(gamma, S[8 * c + e], w * f[e]);
+                for (int j = 0; j < 8; ++j) S[8 * c + j] = fmaf(gamma, S[8 * c + j], w * f[j]);
             }
         }
+        if (tid == 32 && e < 1024) sts_f32(aGam + 16 + e * 4, gamma);
+        gh3 = gh2; gh2 = gh1; gh1 = gacc;             // gacc before entries e-2, e-1, e (as seen at step e + 1)
         gacc *= gamma;
-        mbar_wait(bar_mma, nstep & 1u);
+        if (tid == 0) F64_STAMP(103); if (tid == 32) F64_STAMP(113); if (tid == 64) F64_STAMP(123); if (tid == 96) F64_STAMP(133);
+        mbar_wait(bar_mma, (uint32_t)e & 1u);
         tc_fence_after();
+        if (tid == 0) F64_STAMP(104); if (tid == 32) F64_STAMP(114); if (tid == 64) F64_STAMP(124); if (tid == 96) F64_STAMP(134);
 #pragma unroll
-        for (int hc = 0; hc < 2; ++hc) {
-            float v[32];
-            tmem_ld32(tmem_addr(tmem, warp * 32, hc * 32), v);
+        for (int hc = 0; hc < 4; ++hc) {
+            float v[16];
+            tmem_ld16(tmem_addr(tmem, warp * 32, hc * 16), v);
 #pragma unroll
-            for (int j = 0; j < 32; ++j) S[hc * 32 + j] -= v[j];
+            for (int j = 0; j < 16; ++j) S[hc * 16 + j] -= v[j];
         }
         tc_fence_before();
-        ++nstep;
-        publish(nstep & 1);
+        if (tid == 0) F64_STAMP(105); if (tid == 32) F64_STAMP(115); if (tid == 64) F64_STAMP(125); if (tid == 96) F64_STAMP(135);
+        publish((e + 1) & 1);
+        if (tid == 0) F64_STAMP(106); if (tid == 32) F64_STAMP(116); if (tid == 64) F64_STAMP(126); if (tid == 96) F64_STAMP(136);
         __syncthreads();
-    };
-
-    // ---- the chunks of this CTA's segment ----
-    const bool add_g = type == 2;
-    const int zsnap0 = (type == 2 ? fp.zGA : fp.zSc) + bh * NC;
-    unsigned int* fsnap = (type == 2 ? fp.f_snapA : fp.f_snap) + (long long)bh * NC;
-    const unsigned int* ftile = fp.f_tile + (long long)bh * NC;
-    const float* gam = p.gam + (long long)bh * NC;
-    const int zg0 = fp.zG + bh * NC, zn0 = fp.zN + bh * NC;
-    if (tid == 0) issue_load(0, zg0 + c_lo, add_g ? -1 : zn0 + c_lo, ftile + c_lo, nullptr, gam + c_lo);
-    publish(0);
-    __syncthreads();
-    for (int c = c_lo; c < c_hi; ++c) {
-        const bool nx = c + 1 < c_hi;
-        step(add_g, zsnap0 + c, c > c_lo ? fsnap + c - 1 : nullptr, add_g ? fp.gacc + (long long)bh * NC + c : nullptr,
-             nx, zg0 + c + 1, add_g ? -1 : zn0 + c + 1, ftile + c + 1, nullptr, gam + c + 1);
+        if (tid == 0) F64_STAMP(107); if (tid == 32) F64_STAMP(117); if (tid == 64) F64_STAMP(127); if (tid == 96) F64_STAMP(137);
+        if (e == 0 || e == nchunk / 2 || e >= nchunk - 1) F64_TRACE(1 + e, gtime());
     }
-    if (tid == 0) { tma_store_wait_all(); st_release_gpu(fsnap + c_hi - 1, ep); }
-
-    if (type != 0) {
-        // the map of the whole segment: Gacc / B at its end (the operand buffer holds it in bf16), gamma of the segment
-        if (tid == 0) {
-            const int idx = bh * NS + k;
-            tma_store_3d(tmM3, smem + C_OFF_SB + (nstep & 1) * kTile, 0, 0, (type == 2 ? fp.zGs : fp.zBs) + idx);
-            tma_store_commit();
-            if (type == 2) fp.gseg[idx] = gacc;
-            tma_store_wait_all();
-            st_release_gpu((type == 2 ? fp.f_segA : fp.f_segB) + idx, ep);
-        }
-        return;
-    }
-    // ---- level 2 (type P): S_{k+1} = gseg_k S_k - Gs_k S_k + Bs_k over the segment maps ----
-    for (int kk = 1; kk < NS; ++kk) {
-        const int idx = bh * NS + kk;
-        if (act) {
-            float4* dst = reinterpret_cast<float4*>(fp.SegS + ((long long)idx * 64 + m) * 64);
-#pragma unroll
-            for (int q = 0; q < 16; ++q) __stcg(dst + q, make_float4(S[4 * q], S[4 * q + 1], S[4 * q + 2], S[4 * q + 3]));
-        }
-        __syncthreads();
-        if (tid == 0) {
+    F64_TRACE(162, clock64()); F64_TRACE(163, gtime());
+    if (tid == 32) {
+        tma_store_wait_all();
+        if (kStepRelease) {
+            if (n >= 3) st_release64(e_snap_f(n - 3), flag_word(ep, gh3));
+            if (n >= 2) st_release64(e_snap_f(n - 2), flag_word(ep, gh2));
+            st_release64(e_snap_f(n - 1), flag_word(ep, gh1));
+        } else {
+            // all snapshot flags at once: one fence, then relaxed stores (payload: gacc before the entry, replayed)
             __threadfence();
-            st_release_gpu(fp.f_segS + idx, ep);
-            issue_load(nstep & 1, fp.zGs + idx, fp.zBs + idx, fp.f_segA + idx, fp.f_segB + idx, fp.gseg + idx);
+            float ga = 1.f;
+            for (int e = 0; e < n; ++e) {
+                asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(e)), "l"(flag_word(ep, ga)) : "memory");
+                ga *= gam_hist(e);
+            }
         }
-        step(false, -1, nullptr, nullptr, false, 0, 0, nullptr, nullptr, nullptr);
+        if (type != 0) {
+            // the map of the whole segment: Gacc / B at its end (the operand buffer holds it in bf16), gamma of the segment
+            tma_store_3d(tmM3, smem + C_OFF_SB + (n & 1) * kTile, 0, 0, (add_g ? fp.zGs : fp.zBs) + (int)sb + k);
+            tma_store_commit();
+            tma_store_wait_all();
+            st_release64((add_g ? fp.f_segA : fp.f_segB) + sb + k, flag_word(ep, gacc));
+        }
     }
-    if (act && p.S_out) {
+    if (type == 0 && act && p.S_out) {
         float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * 64 + m) * 64);
 #pragma unroll
         for (int q = 0; q < 16; ++q) dst[q] = make_float4(S[4 * q], S[4 * q + 1], S[4 * q + 2], S[4 * q + 3]);
@@ -223,57 +291,54 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
 
 // ---------------------------------------------------------------------------------------------------
 // output task (worker CTA): chunk c of stream bh, segment k.  Thread (warp w, lane l < 16) owns token row 16 w + l.
-//   shared memory (offsets of t64): Qt -> OFF_Q, Ol -> OFF_V (the finished tile is staged over it), state operand -> OFF_K,
-//   Gacc_c -> OFF_PT, B_c -> OFF_X.
+//   shared memory (offsets of t64): Qt -> OFF_Q, Ol -> OFF_V (the finished tile is staged over it), state operand
+//   (S_c, or S_k then S_c) -> OFF_K, Gacc_c -> OFF_PT, B_c -> OFF_X.
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void output_task(uint8_t* smem, uint32_t tmem, uint64_t* bars, const CUtensorMap* tmM3, const CUtensorMap* tmR2,
-                                            const CUtensorMap* tmO, const F64Params& fp, int bh, int c, int k, uint32_t& pl, uint32_t& ph) {
+                                            const CUtensorMap* tmO, const F64Params& fp, int bh, int c, int k, uint32_t& pl, uint32_t& ph,
+                                            unsigned long long* pend_flag, unsigned long long pend_val) {
     const TokParams& p = fp.t;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int NC = p.NC, NS = fp.NS;
     const int m = 16 * warp + lane;
     const bool act = lane < 16;
     const uint32_t aS = smem_u32(smem + t64::OFF_K), aQ = smem_u32(smem + t64::OFF_Q), aO = smem_u32(smem + t64::OFF_V);
-    const uint32_t aGA = smem_u32(smem + t64::OFF_PT), aB = smem_u32(smem + t64::OFF_X);
+    const uint32_t aGA = smem_u32(smem + t64::OFF_PT), aB = smem_u32(smem + t64::OFF_X), aVec = smem_u32(smem + t64::OFF_VEC);
     uint64_t *bar_ld = &bars[0], *bar_mma = &bars[2];
     const unsigned int ep = fp.epoch;
     const long long ci = (long long)bh * NC + c;
     const bool comp = k > 0;
     if (tid == 0) {
         tma_store_wait_read();                        // the previous task's stores have left the staging buffers
-        wait_flag(fp.f_snap + ci, ep);
-        if (comp) wait_flag(fp.f_snapA + ci, ep);
+        if (pend_flag) { tma_store_wait_all(); st_release64(pend_flag, pend_val); }
+        wait_flag(fp.f_snap + ci, ep, 200);
+        if (comp) {
+            sts_f32(aVec, flag_payload(wait_flag(fp.f_snapA + ci, ep, 200)));
+            wait_flag(fp.f_segS + (long long)bh * NS + k, ep, 200);
+        }
+        acquire_after_poll();
         fence_proxy_async_global();
         const int r0 = (int)(ci * 64);
-        mbar_expect_tx(bar_ld, (comp ? 4u : 3u) * kTile);
+        mbar_expect_tx(bar_ld, (comp ? 5u : 3u) * kTile);
         tma_load_2d(smem + t64::OFF_Q, tmR2, bar_ld, 0, (int)(fp.rQt + r0));
         tma_load_2d(smem + t64::OFF_V, tmR2, bar_ld, 0, (int)(fp.rOl + r0));
         if (comp) {
             tma_load_3d(smem + t64::OFF_PT, tmM3, bar_ld, 0, 0, fp.zGA + (int)ci);
             tma_load_3d(smem + t64::OFF_X, tmM3, bar_ld, 0, 0, fp.zSc + (int)ci);
+            tma_load_3d(smem + t64::OFF_K, tmM3, bar_ld, 0, 0, fp.zSk + bh * NS + k);
         } else {
             tma_load_3d(smem + t64::OFF_K, tmM3, bar_ld, 0, 0, fp.zSc + (int)ci);
         }
-        if (comp) wait_flag(fp.f_segS + (long long)bh * NS + k, ep);
-    }
-    auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
-    auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
-    if (comp) {
-        // S_c = gacc_c S_k - Gacc_c S_k + B_c: S_k (fp32, global) -> registers and bf16 operand; one MMA; fp32 combination
-        __syncthreads();                              // thread 0 has seen the flag of S_k
-        float S[64];
-        const float4* src = reinterpret_cast<const float4*>(fp.SegS + (((long long)bh * NS + k) * 64 + (act ? m : 0)) * 64);
-#pragma unroll
-        for (int q = 0; q < 16; ++q) { const float4 f = __ldcg(src + q); S[4 * q] = f.x; S[4 * q + 1] = f.y; S[4 * q + 2] = f.z; S[4 * q + 3] = f.w; }
-        const float ga = __ldcg(fp.gacc + ci);
-        if (act) {
-#pragma unroll
-            for (int cc = 0; cc < 8; ++cc)
-                st_shared_v4(aS + swz_chunk_off(m, cc, 0), pack_bf16(S[8 * cc], S[8 * cc + 1]), pack_bf16(S[8 * cc + 2], S[8 * cc + 3]),
-                             pack_bf16(S[8 * cc + 4], S[8 * cc + 5]), pack_bf16(S[8 * cc + 6], S[8 * cc + 7]));
-        }
         mbar_wait(bar_ld, pl);
-        sync_then_issue();
+    }
+    // Only thread 0 polls (flags, then the load barrier); the others sleep in the CTA barrier instead of spinning on the
+    // mbarrier: this CTA shares its SM with chain CTAs whose steps are the critical path.
+    __syncthreads();
+    auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
+    mbar_wait(bar_ld, pl);
+    pl ^= 1u;
+    if (comp) {
+        // S_c = gacc_c S_k - Gacc_c S_k + B_c: one MMA on the bf16 S_k, fp32 combination, S_c (bf16) over S_k
         if (tid == 0) {
             tc_fence_after();
             const uint32_t id = umma_idesc(64, 64, false, true);
@@ -281,22 +346,25 @@ __device__ __forceinline__ void output_task(uint8_t* smem, uint32_t tmem, uint64
             for (int s = 0; s < 4; ++s) umma_bf16(tmem, desc_kmajor(aGA + s * 32), desc_mnmajor(aS + s * 2048, 0), id, s > 0);
             umma_commit(bar_mma);
         }
+        const float ga = lds_f32(aVec);
+        float S[64];
         if (act) {
 #pragma unroll
             for (int cc = 0; cc < 8; ++cc) {
-                float f[8];
-                unpack8(ld_shared_v4(aB + swz_chunk_off(m, cc, 0)), f);
+                float f[8], g[8];
+                unpack8(ld_shared_v4(aS + swz_chunk_off(m, cc, 0)), f);
+                unpack8(ld_shared_v4(aB + swz_chunk_off(m, cc, 0)), g);
 #pragma unroll
-                for (int e = 0; e < 8; ++e) S[8 * cc + e] = fmaf(ga, S[8 * cc + e], f[e]);
+                for (int e = 0; e < 8; ++e) S[8 * cc + e] = fmaf(ga, f[e], g[e]);
             }
         }
         wait_mma();
 #pragma unroll
-        for (int hc = 0; hc < 2; ++hc) {
-            float v[32];
-            tmem_ld32(tmem_addr(tmem, warp * 32, hc * 32), v);
+        for (int hc = 0; hc < 4; ++hc) {
+            float v[16];
+            tmem_ld16(tmem_addr(tmem, warp * 32, hc * 16), v);
 #pragma unroll
-            for (int j = 0; j < 32; ++j) S[hc * 32 + j] -= v[j];
+            for (int j = 0; j < 16; ++j) S[hc * 16 + j] -= v[j];
         }
         tc_fence_before();
         if (act) {
@@ -305,11 +373,10 @@ __device__ __forceinline__ void output_task(uint8_t* smem, uint32_t tmem, uint64
                 st_shared_v4(aS + swz_chunk_off(m, cc, 0), pack_bf16(S[8 * cc], S[8 * cc + 1]), pack_bf16(S[8 * cc + 2], S[8 * cc + 3]),
                              pack_bf16(S[8 * cc + 4], S[8 * cc + 5]), pack_bf16(S[8 * cc + 6], S[8 * cc + 7]));
         }
-        sync_then_issue();
-    } else {
-        mbar_wait(bar_ld, pl);
+        fence_proxy_async();
+        tc_fence_before();
+        __syncthreads();
     }
-    pl ^= 1u;
     // O_c = scale (Qt_c S_c + Ol_c)
     if (tid == 0) {
         tc_fence_after();
@@ -355,7 +422,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + t64::OFF_BAR);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
-    int* s_task = reinterpret_cast<int*>(bars + 5);
     const int tid = threadIdx.x;
     if (tid == 0) {
         for (int s = 0; s < 4; ++s) mbar_init(&bars[s], 1);
@@ -368,21 +434,46 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const uint32_t tmem = *tmem_slot;
     const TokParams& p = fp.t;
     const int BH = p.B * p.H;
-    if ((int)blockIdx.x < fp.NCH) {
-        chain_role(smem, tmem, bars, &tmM3, fp, (int)blockIdx.x);
+    // Roles.  A chain step is a dependent sequence of a few hundred instructions on four warps; on an SM it shares with
+    // busy workers it runs three to five times slower (measured), and the chain is the critical path.  So the chain CTAs
+    // get SMs of their own: the first NCSM SMs on which a CTA of this grid starts are chain SMs, the CTAs that land there
+    // claim the chain units, everybody else is a worker.  (Units left unclaimed by an unexpected placement are picked up
+    // by workers before their first output task, so every placement makes progress.)
+    int* s_word = reinterpret_cast<int*>(bars + 5);
+    if (tid == 0) {
+        unsigned int smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        smid &= (unsigned int)(kMaxSm - 1);
+        unsigned int* cnt = fp.ctl + 16 + smid;
+        unsigned int* rank = fp.ctl + 16 + kMaxSm + smid;
+        unsigned int r;
+        if (atomicAdd(cnt, 1u) == 0u) {
+            r = atomicAdd(fp.ctl + 2, 1u);
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(rank), "r"(r + 1u) : "memory");
+        } else {
+            unsigned int v;
+            do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(rank) : "memory"); } while (v == 0u);
+            r = v - 1u;
+        }
+        int unit = -1;
+        if ((int)r < fp.NCSM) { const unsigned int u = atomicAdd(fp.ctl + 3, 1u); if ((int)u < fp.NCH) unit = (int)u; }
+        *s_word = unit;
+    }
+    __syncthreads();
+    const int my_unit = *s_word;
+    __syncthreads();
+    if (my_unit >= 0) {
+        chain_role(smem, tmem, bars, &tmM3, fp, my_unit);
     } else {
         t64::Tile64Maps mp{&tmQ, &tmK, &tmV, &tmM3, &tmM3, &tmR2, &tmR2, fp.zG, fp.zN, (long long)p.NC * 64, fp.rQt, fp.rOl};
         uint32_t pl = 0, ph = 0;
         const int total = fp.n_tile_tasks + fp.n_out_tasks;
-        for (;;) {
-            if (tid == 0) *s_task = (int)atomicAdd(fp.ctr, 1u);
-            __syncthreads();
-            const int task = *s_task;
-            __syncthreads();
-            if (task >= total) break;
-            const int tt = task < fp.n_tile_tasks ? task : task - fp.n_tile_tasks;
-            int bh, c, k;
-            if (task < fp.n_tile_tasks) {             // segments interleaved: (j, k, bh)
+        int ntask = 0;
+        // task -> (is tile task, stream, chunk, segment); chunk >= NC: nothing to do (the last segment is shorter)
+        auto decode = [&](int task, bool& tile, int& bh, int& c, int& k) {
+            tile = task < fp.n_tile_tasks;
+            const int tt = tile ? task : task - fp.n_tile_tasks;
+            if (tile) {                               // segments interleaved: (j, k, bh)
                 const int j = tt / (fp.NS * BH), r = tt % (fp.NS * BH);
                 k = r / BH; bh = r % BH; c = k * fp.LSEG + j;
             } else {                                  // segment-major: (k, j, bh)
@@ -390,26 +481,119 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const int r = tt % (fp.LSEG * BH);
                 bh = r % BH; c = k * fp.LSEG + r / BH;
             }
-            if (c >= p.NC) continue;                  // the last segment is shorter
-            if (task < fp.n_tile_tasks) {
-                if (tid == 0) tma_store_wait_read();  // an output task before this one may still be reading its staging
-                t64::tile64<true>(smem, tmem, bars, mp, p, bh, c, pl, ph);
-                if (tid == 0) {
-                    tma_store_wait_all();
-                    st_release_gpu(fp.f_tile + (long long)bh * p.NC + c, fp.epoch);
+            if (c >= (k + 1) * fp.LSEG) c = p.NC;
+        };
+        unsigned long long* pend_flag = nullptr;      // flag of this CTA's last tile task, released inside the next task
+        unsigned long long pend_val = 0ull;
+        const uint32_t aRaw = smem_u32(smem + t64::OFF_RAW);
+        int raw_sel = 0;                              // raw gate buffer of the current task
+        bool have_cur = false;
+        // dynamic queue: one atomic counter.  A worker claims its next task at the start of the current one (so that the
+        // next task's inputs can be prefetched) -- except during its very first task, otherwise every worker would hold
+        // two tasks from the start and the second wave of tile tasks would no longer complete in task order.
+        auto claim = [&]() {
+            if (tid == 0) *s_word = (int)atomicAdd(fp.ctl, 1u);
+            __syncthreads();
+            const int t = *s_word;
+            __syncthreads();
+            return t;
+        };
+        int task = claim();
+        bool first = true, chain_checked = false;
+        while (task < total) {
+            int next = total;
+            if (!first) next = claim();
+            bool tile, ntile = false;
+            int bh, c, k, nbh = 0, nc = 0, nk = 0;
+            decode(task, tile, bh, c, k);
+            if (next < total) decode(next, ntile, nbh, nc, nk);
+            const bool have_next = next < total && ntile && nc < p.NC;
+            if (have_next) {
+                // the next chunk's gates -> raw buffer (ntask + 1) & 1 with 4-byte asynchronous copies (padding rows:
+                // alpha = 1, beta = 0), its K / Q / V tiles -> L2
+                if (tid < 128) {
+                    const int j = tid & 63, t = nc * 64 + j;
+                    const bool is_b = tid >= 64;
+                    const uint32_t dst = aRaw + (uint32_t)(raw_sel ^ 1) * 512u + (uint32_t)tid * 4u;
+                    if (t < p.T) {
+                        const float* src = (is_b ? p.beta : p.alpha) + (long long)nbh * p.T + t;
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+                    } else {
+                        sts_f32(dst, is_b ? 0.f : (p.log_alpha ? 0.f : 1.f));
+                    }
+                    asm volatile("cp.async.commit_group;" ::: "memory");
                 }
-            } else {
-                output_task(smem, tmem, bars, &tmM3, &tmR2, &tmO, fp, bh, c, k, pl, ph);
+                if (tid == 0) {
+                    const int b = nbh / p.H, h = nbh % p.H;
+                    tma_prefetch_5d(&tmK, 0, h, nc * 64, 0, b);
+                    tma_prefetch_5d(&tmQ, 0, h, nc * 64, 0, b);
+                    tma_prefetch_5d(&tmV, 0, h, nc * 64, 0, b);
+                }
             }
+            if (c < p.NC) {
+                F64_TRACE(2 * ntask, gtime()); F64_TRACE(128 + ntask, (long long)task);
+                if (tile) {
+                    if (tid == 0) tma_store_wait_read();  // the previous task's stores have left the staging buffers
+                    float gam_c = 0.f;
+                    t64::tile64<true>(smem, tmem, bars, mp, p, bh, c, pl, ph, have_cur ? aRaw + (uint32_t)raw_sel * 512u : 0u, pend_flag, pend_val, &gam_c);
+                    pend_flag = fp.f_tile + (long long)bh * p.NC + c;
+                    pend_val = flag_word(fp.epoch, gam_c);
+                } else {
+                    if (!chain_checked) {
+                        // safety net (see the role assignment): chain units nobody claimed are run here, before this
+                        // worker can block on a flag.  With the expected placement this is one atomic.
+                        chain_checked = true;
+                        for (;;) {
+                            if (tid == 0) *s_word = (int)atomicAdd(fp.ctl + 3, 1u);
+                            __syncthreads();
+                            const int u = *s_word;
+                            __syncthreads();
+                            if (u >= fp.NCH) break;
+                            if (tid == 0) {
+                                tma_store_wait_all();
+                                if (pend_flag) st_release64(pend_flag, pend_val);
+                                for (int b4 = 0; b4 < 4; ++b4) mbar_init(&bars[b4], 1);
+                                mbar_fence_init();
+                            }
+                            pend_flag = nullptr;
+                            __syncthreads();
+                            chain_role(smem, tmem, bars, &tmM3, fp, u);
+                            __syncthreads();
+                            if (tid == 0) {
+                                tma_store_wait_all();
+                                for (int b4 = 0; b4 < 4; ++b4) mbar_init(&bars[b4], 1);
+                                mbar_fence_init();
+                            }
+                            pl = 0; ph = 0;
+                            __syncthreads();
+                        }
+                    }
+                    output_task(smem, tmem, bars, &tmM3, &tmR2, &tmO, fp, bh, c, k, pl, ph, pend_flag, pend_val);
+                    pend_flag = nullptr;
+                }
+                F64_TRACE(2 * ntask + 1, gtime()); ++ntask;
+            }
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            raw_sel ^= 1;
+            have_cur = have_next;
+            if (first) { next = claim(); first = false; }
+            task = next;
+            __syncthreads();
         }
-        if (tid == 0) tma_store_wait_all();
+        if (tid == 0) {
+            tma_store_wait_all();
+            if (pend_flag) st_release64(pend_flag, pend_val);
+        }
     }
     tc_fence_before();
     __syncthreads();
     if (tid < 32) tmem_dealloc(tmem, 128);
     if (tid == 0) {
         __threadfence();
-        if (atomicAdd(fp.ctr + 1, 1u) == gridDim.x - 1) { fp.ctr[0] = 0u; fp.ctr[1] = 0u; __threadfence(); }
+        if (atomicAdd(fp.ctl + 1, 1u) == gridDim.x - 1) {      // the last CTA of the call: control words back to zero
+            for (int w = 0; w < kCtlWords; ++w) fp.ctl[w] = 0u;
+            __threadfence();
+        }
     }
 }
 

@@ -40,7 +40,8 @@ constexpr uint32_t OFF_X = 32768;                     // L_bf | D_bf (bf16 [64][
                                                       //   -> [W | Ut] bf16 2 x [64][64] -> staging of N
 constexpr uint32_t X_BYTES = 2 * kTile + 4096;
 constexpr uint32_t OFF_VEC = OFF_X + X_BYTES;         // Gam[64], Beta[64], BG[64], KS[64], CF[32]
-constexpr uint32_t OFF_BAR = OFF_VEC + 1280;
+constexpr uint32_t OFF_RAW = OFF_VEC + 1280;              // 2 x {alpha[64], beta[64]} of the next chunk, copied ahead (persistent workers)
+constexpr uint32_t OFF_BAR = OFF_RAW + 1024;
 constexpr uint32_t SMEM_BYTES = OFF_BAR + 64 + 1024;  // + slack for the 1024-byte alignment of the dynamic base
 
 struct Tile64Maps {
@@ -79,7 +80,11 @@ __device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a
 // barriers (both complete one phase per chunk) and of the MMA barrier, kept by the caller across tasks.
 template <bool NBF16>
 __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* bars, const Tile64Maps& mp, const TokParams& p,
-                                       int bh, int chunk, uint32_t& pl, uint32_t& ph) {
+                                       int bh, int chunk, uint32_t& pl, uint32_t& ph, uint32_t pre_gates = 0u,
+                                       unsigned long long* pend_flag = nullptr, unsigned long long pend_val = 0ull, float* gamma_out = nullptr) {
+    // pre_gates: shared-space address of {alpha[64], beta[64]} of the chunk, copied ahead by the caller (0: read them here).  pend_flag / pend_val: a flag word of the caller's previous task, released by thread 0 once that
+    // task's bulk stores have completed (behind this chunk's first MMA issue, where the wait costs nothing).  gamma_out:
+    // receives gamma_C (thread 0) instead of p.gam.
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = bh / p.H, h = bh % p.H;
     const uint32_t aK = smem_u32(smem + OFF_K), aQ = smem_u32(smem + OFF_Q), aV = smem_u32(smem + OFF_V);
@@ -105,8 +110,11 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     {
         const int t0 = chunk * 64 + lane, t1 = t0 + 32;
         float a0 = p.log_alpha ? 0.f : 1.f, a1 = a0, b0 = 0.f, b1 = 0.f;       // padding rows: alpha = 1, beta = 0
-        if (t0 < p.T) { a0 = p.alpha[(long long)bh * p.T + t0]; b0 = p.beta[(long long)bh * p.T + t0]; }
-        if (t1 < p.T) { a1 = p.alpha[(long long)bh * p.T + t1]; b1 = p.beta[(long long)bh * p.T + t1]; }
+        if (pre_gates) { a0 = lds_f32(pre_gates + lane * 4); a1 = lds_f32(pre_gates + (32 + lane) * 4); b0 = lds_f32(pre_gates + (64 + lane) * 4); b1 = lds_f32(pre_gates + (96 + lane) * 4); }
+        else {
+            if (t0 < p.T) { a0 = p.alpha[(long long)bh * p.T + t0]; b0 = p.beta[(long long)bh * p.T + t0]; }
+            if (t1 < p.T) { a1 = p.alpha[(long long)bh * p.T + t1]; b1 = p.beta[(long long)bh * p.T + t1]; }
+        }
         float x0 = p.log_alpha ? a0 : logf(a0), x1 = p.log_alpha ? a1 : logf(a1);
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -140,6 +148,10 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
 #pragma unroll
         for (int s = 0; s < 4; ++s) umma_bf16(tmem, desc_kmajor(aK + s * 32), desc_kmajor(aK + s * 32), id, s > 0);
         umma_commit(bar_mma);
+        if (pend_flag) {
+            tma_store_wait_all();
+            asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(pend_flag), "l"(pend_val) : "memory");
+        }
     }
     wait_mma();
     T64_STAMP(3);
@@ -423,7 +435,8 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         tma_store_3d(mp.tmN, smem + OFF_X, 0, 0, mp.zN + z);
         if (!NBF16) tma_store_3d(mp.tmN, smem + OFF_X + kTile, 32, 0, mp.zN + z);
         tma_store_commit();
-        p.gam[(long long)bh * p.NC + chunk] = fast_exp(gam_C);
+        if (gamma_out) *gamma_out = fast_exp(gam_C);
+        else p.gam[(long long)bh * p.NC + chunk] = fast_exp(gam_C);
     }
 }
 
