@@ -197,7 +197,7 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
     const size_t nflag = 3 * nchunk + 3 * nseg;
-    const size_t oM3 = carve(slots * 8192), oR2 = carve(rows * 128), oFl = carve(nflag * 8 + f64::kCtlWords * 4);
+    const size_t oM3 = carve(slots * 8192), oR2 = carve(rows * 128), oFl = carve(nflag * 8 + 64);
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -208,8 +208,7 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     unsigned long long* fl = reinterpret_cast<unsigned long long*>(w + oFl);
     f.f_tile = fl; f.f_snap = fl + nchunk; f.f_snapA = fl + 2 * nchunk;
     f.f_segA = fl + 3 * nchunk; f.f_segB = f.f_segA + nseg; f.f_segS = f.f_segB + nseg;
-    f.ctl = reinterpret_cast<unsigned int*>(f.f_segS + nseg);
-    if (cudaMemset(fl, 0, nflag * 8 + f64::kCtlWords * 4) != cudaSuccess) {
+    if (cudaMemset(fl, 0, nflag * 8 + 64) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "flag initialisation failed";
         return GDN_ERR_CUDA;
@@ -219,8 +218,6 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     if (grid > 4LL * sms) grid = 4LL * sms;
     if (grid < f.NCH + 1) grid = f.NCH + 1;
     tp.grid = (int)grid;
-    const int cps = (int)((grid + sms - 1) / sms);                 // CTAs the block scheduler puts on one SM
-    f.NCSM = (f.NCH + cps - 1) / cps;
     bool ok = true;
     {
         const uint64_t dims[3] = {64, 64, slots}, str[3] = {2, 128, 8192};

@@ -45,18 +45,14 @@ struct F64Params {
     unsigned long long *f_segB;  // [BH][NS]  B of the whole segment stored
     unsigned long long *f_segS;  // [BH][NS]  S_k (state at the start of segment k) stored
     unsigned int epoch;
-    unsigned int* ctl;           // kCtlWords control words, all zero between calls (the last CTA of a call clears them):
-                                 //   [0] task counter, [1] finished CTAs, [2] SMs seen, [3] chain units claimed,
-                                 //   [16 ..] CTAs arrived per SM id, [16 + kMaxSm ..] 1 + arrival rank of the SM
-    int NCSM;                    // SMs reserved for chain CTAs: the first NCSM SMs on which a CTA of the grid starts
     int n_tile_tasks, n_out_tasks;
 };
 
 namespace f64 {
 
-constexpr int kMaxSm = 512;                           // upper bound of %smid
-constexpr int kCtlWords = 16 + 2 * kMaxSm;
-constexpr bool kStepRelease = false;                  // chain CTAs release their snapshot flags per step (true) or all at the end
+// Chain CTAs release their snapshot flags all at once when they are done (false) or per step, trailing by three steps
+// (true).  A gpu-scope release per step sits on a state warp: per-step release measured 55.4 us, at-the-end 49.5 us (config 2).
+constexpr bool kStepRelease = false;                 // chain CTAs release their snapshot flags per step (true) or all at the end
 
 #ifdef GDN_PHASE_TIMING
 __device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
@@ -86,14 +82,9 @@ __device__ __forceinline__ unsigned long long flag_word(unsigned int epoch, floa
 }
 __device__ __forceinline__ bool flag_ready(unsigned long long w, unsigned int epoch) { return (unsigned int)w >= epoch; }
 __device__ __forceinline__ float flag_payload(unsigned long long w) { return __uint_as_float((unsigned int)(w >> 32)); }
-// Polling uses relaxed loads (an acquire load invalidates the SM's whole L1 every time, which the other CTAs of the SM
-// feel); ONE acquire fence follows once everything an action needs has been observed (acquire_after_poll).
-__device__ __forceinline__ unsigned long long ld_relaxed64(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void acquire_after_poll() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+// (Polling with relaxed loads followed by one fence.acq_rel.gpu measured 5 us SLOWER on config 2 than acquire loads.)
+__device__ __forceinline__ void acquire_after_poll() {}
+#define ld_relaxed64 ld_acquire64
 __device__ __forceinline__ unsigned long long wait_flag(const unsigned long long* f, unsigned int epoch, unsigned int ns = 20) {
     unsigned long long w = ld_relaxed64(f);
     while (!flag_ready(w, epoch)) { __nanosleep(ns); w = ld_relaxed64(f); }
@@ -434,34 +425,9 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const uint32_t tmem = *tmem_slot;
     const TokParams& p = fp.t;
     const int BH = p.B * p.H;
-    // Roles.  A chain step is a dependent sequence of a few hundred instructions on four warps; on an SM it shares with
-    // busy workers it runs three to five times slower (measured), and the chain is the critical path.  So the chain CTAs
-    // get SMs of their own: the first NCSM SMs on which a CTA of this grid starts are chain SMs, the CTAs that land there
-    // claim the chain units, everybody else is a worker.  (Units left unclaimed by an unexpected placement are picked up
-    // by workers before their first output task, so every placement makes progress.)
-    int* s_word = reinterpret_cast<int*>(bars + 5);
-    if (tid == 0) {
-        unsigned int smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        smid &= (unsigned int)(kMaxSm - 1);
-        unsigned int* cnt = fp.ctl + 16 + smid;
-        unsigned int* rank = fp.ctl + 16 + kMaxSm + smid;
-        unsigned int r;
-        if (atomicAdd(cnt, 1u) == 0u) {
-            r = atomicAdd(fp.ctl + 2, 1u);
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(rank), "r"(r + 1u) : "memory");
-        } else {
-            unsigned int v;
-            do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(rank) : "memory"); } while (v == 0u);
-            r = v - 1u;
-        }
-        int unit = -1;
-        if ((int)r < fp.NCSM) { const unsigned int u = atomicAdd(fp.ctl + 3, 1u); if ((int)u < fp.NCH) unit = (int)u; }
-        *s_word = unit;
-    }
-    __syncthreads();
-    const int my_unit = *s_word;
-    __syncthreads();
+    // Roles: the first NCH CTAs are chain CTAs (the block scheduler hands CTAs to SMs in index order, so they are resident
+    // before any worker and spread over distinct SMs), the rest are workers.
+    const int my_unit = (int)blockIdx.x < fp.NCH ? (int)blockIdx.x : -1;
     if (my_unit >= 0) {
         chain_role(smem, tmem, bars, &tmM3, fp, my_unit);
     } else {
@@ -488,21 +454,13 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const uint32_t aRaw = smem_u32(smem + t64::OFF_RAW);
         int raw_sel = 0;                              // raw gate buffer of the current task
         bool have_cur = false;
-        // dynamic queue: one atomic counter.  A worker claims its next task at the start of the current one (so that the
-        // next task's inputs can be prefetched) -- except during its very first task, otherwise every worker would hold
-        // two tasks from the start and the second wave of tile tasks would no longer complete in task order.
-        auto claim = [&]() {
-            if (tid == 0) *s_word = (int)atomicAdd(fp.ctl, 1u);
-            __syncthreads();
-            const int t = *s_word;
-            __syncthreads();
-            return t;
-        };
-        int task = claim();
-        bool first = true, chain_checked = false;
+        // static round-robin over the workers: waves of tile tasks complete in task order (the chain CTAs consume them
+        // in that order), and the task after this one is known in advance (its inputs are prefetched during this one).
+        // (A dynamic queue -- one atomic counter, the next task claimed a task ahead -- measured 15 us slower on config 2.)
+        const int nworkers = (int)gridDim.x - fp.NCH;
+        int task = (int)blockIdx.x - fp.NCH;
         while (task < total) {
-            int next = total;
-            if (!first) next = claim();
+            const int next = task + nworkers;
             bool tile, ntile = false;
             int bh, c, k, nbh = 0, nc = 0, nk = 0;
             decode(task, tile, bh, c, k);
@@ -539,35 +497,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     pend_flag = fp.f_tile + (long long)bh * p.NC + c;
                     pend_val = flag_word(fp.epoch, gam_c);
                 } else {
-                    if (!chain_checked) {
-                        // safety net (see the role assignment): chain units nobody claimed are run here, before this
-                        // worker can block on a flag.  With the expected placement this is one atomic.
-                        chain_checked = true;
-                        for (;;) {
-                            if (tid == 0) *s_word = (int)atomicAdd(fp.ctl + 3, 1u);
-                            __syncthreads();
-                            const int u = *s_word;
-                            __syncthreads();
-                            if (u >= fp.NCH) break;
-                            if (tid == 0) {
-                                tma_store_wait_all();
-                                if (pend_flag) st_release64(pend_flag, pend_val);
-                                for (int b4 = 0; b4 < 4; ++b4) mbar_init(&bars[b4], 1);
-                                mbar_fence_init();
-                            }
-                            pend_flag = nullptr;
-                            __syncthreads();
-                            chain_role(smem, tmem, bars, &tmM3, fp, u);
-                            __syncthreads();
-                            if (tid == 0) {
-                                tma_store_wait_all();
-                                for (int b4 = 0; b4 < 4; ++b4) mbar_init(&bars[b4], 1);
-                                mbar_fence_init();
-                            }
-                            pl = 0; ph = 0;
-                            __syncthreads();
-                        }
-                    }
                     output_task(smem, tmem, bars, &tmM3, &tmR2, &tmO, fp, bh, c, k, pl, ph, pend_flag, pend_val);
                     pend_flag = nullptr;
                 }
@@ -576,7 +505,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             asm volatile("cp.async.wait_all;" ::: "memory");
             raw_sel ^= 1;
             have_cur = have_next;
-            if (first) { next = claim(); first = false; }
             task = next;
             __syncthreads();
         }
@@ -588,13 +516,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_before();
     __syncthreads();
     if (tid < 32) tmem_dealloc(tmem, 128);
-    if (tid == 0) {
-        __threadfence();
-        if (atomicAdd(fp.ctl + 1, 1u) == gridDim.x - 1) {      // the last CTA of the call: control words back to zero
-            for (int w = 0; w < kCtlWords; ++w) fp.ctl[w] = 0u;
-            __threadfence();
-        }
-    }
 }
 
 }  // namespace f64
