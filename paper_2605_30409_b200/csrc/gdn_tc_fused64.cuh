@@ -52,6 +52,7 @@ namespace f64 {
 
 // Chain CTAs release their snapshot flags all at once when they are done (false) or per step, trailing by three steps
 // (true).  A gpu-scope release per step sits on a state warp: per-step release measured 55.4 us, at-the-end 49.5 us (config 2).
+constexpr int kReleaseBatch = 1 << 20;                // ... in batches of this many steps (4: 51.2 us, never: 49.6 us on config 2)
 constexpr bool kStepRelease = false;                 // chain CTAs release their snapshot flags per step (true) or all at the end
 
 #ifdef GDN_PHASE_TIMING
@@ -176,12 +177,12 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     publish(0);
     __syncthreads();
     auto gam_hist = [&](int e) { return lds_f32(aGam + 16 + (e < 1024 ? e : 1023) * 4); };
+    int released = 0;                                 // thread 32: snapshot flags released so far, and gacc before that entry
+    float ga_rel = 1.f;
     float gh1 = 1.f, gh2 = 1.f, gh3 = 1.f;            // gacc before the last three entries (payload of the trailing flags)
     for (int e = 0; e < n; ++e) {
         const int st = e & 1;
-        if (tid == 0) F64_STAMP(100); if (tid == 32) F64_STAMP(110); if (tid == 64) F64_STAMP(120); if (tid == 96) F64_STAMP(130);
         mbar_wait(&full[st], (uint32_t)(e >> 1) & 1u);
-        if (tid == 0) F64_STAMP(101); if (tid == 32) F64_STAMP(111); if (tid == 64) F64_STAMP(121); if (tid == 96) F64_STAMP(131);
         if (warp == 0) {
             // issued under elect.sync: with a plain `tid == 0` every tcgen05.mma sits in a ~70-cycle "waterfall" loop
             // (ptxas cannot keep its operands in uniform registers), which on this serial chain is exposed latency
@@ -213,8 +214,16 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
                 asm volatile("cp.async.bulk.wait_group 3;" ::: "memory");
                 st_release64(e_snap_f(e - 3), flag_word(ep, gh3));
             }
+            if (!kStepRelease && e >= released + kReleaseBatch + 1) {
+                // a batch of flags: the snapshots before entry e - 1 are complete; one fence, then relaxed stores
+                asm volatile("cp.async.bulk.wait_group 2;" ::: "memory");
+                __threadfence();
+                for (; released < e - 1; ++released) {
+                    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
+                    ga_rel *= gam_hist(released);
+                }
+            }
         }
-        if (tid == 0) F64_STAMP(102); if (tid == 32) F64_STAMP(112); if (tid == 64) F64_STAMP(122); if (tid == 96) F64_STAMP(132);
         const float gamma = lds_f32(aGam + st * 4);
         if (act) {                                    // state-independent half, while the MMA runs
             const uint32_t src = aSt + st * C_STAGE + (add_g ? 0u : kTile);
@@ -230,10 +239,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
         if (tid == 32 && e < 1024) sts_f32(aGam + 16 + e * 4, gamma);
         gh3 = gh2; gh2 = gh1; gh1 = gacc;             // gacc before entries e-2, e-1, e (as seen at step e + 1)
         gacc *= gamma;
-        if (tid == 0) F64_STAMP(103); if (tid == 32) F64_STAMP(113); if (tid == 64) F64_STAMP(123); if (tid == 96) F64_STAMP(133);
         mbar_wait(bar_mma, (uint32_t)e & 1u);
         tc_fence_after();
-        if (tid == 0) F64_STAMP(104); if (tid == 32) F64_STAMP(114); if (tid == 64) F64_STAMP(124); if (tid == 96) F64_STAMP(134);
 #pragma unroll
         for (int hc = 0; hc < 4; ++hc) {
             float v[16];
@@ -242,11 +249,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
             for (int j = 0; j < 16; ++j) S[hc * 16 + j] -= v[j];
         }
         tc_fence_before();
-        if (tid == 0) F64_STAMP(105); if (tid == 32) F64_STAMP(115); if (tid == 64) F64_STAMP(125); if (tid == 96) F64_STAMP(135);
         publish((e + 1) & 1);
-        if (tid == 0) F64_STAMP(106); if (tid == 32) F64_STAMP(116); if (tid == 64) F64_STAMP(126); if (tid == 96) F64_STAMP(136);
         __syncthreads();
-        if (tid == 0) F64_STAMP(107); if (tid == 32) F64_STAMP(117); if (tid == 64) F64_STAMP(127); if (tid == 96) F64_STAMP(137);
         if (e == 0 || e == nchunk / 2 || e >= nchunk - 1) F64_TRACE(1 + e, gtime());
     }
     F64_TRACE(162, clock64()); F64_TRACE(163, gtime());
@@ -257,12 +261,11 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
             if (n >= 2) st_release64(e_snap_f(n - 2), flag_word(ep, gh2));
             st_release64(e_snap_f(n - 1), flag_word(ep, gh1));
         } else {
-            // all snapshot flags at once: one fence, then relaxed stores (payload: gacc before the entry, replayed)
+            // the remaining snapshot flags: one fence, then relaxed stores (payload: gacc before the entry, replayed)
             __threadfence();
-            float ga = 1.f;
-            for (int e = 0; e < n; ++e) {
-                asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(e)), "l"(flag_word(ep, ga)) : "memory");
-                ga *= gam_hist(e);
+            for (; released < n; ++released) {
+                asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
+                ga_rel *= gam_hist(released);
             }
         }
         if (type != 0) {
