@@ -51,8 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not _stale():
         return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    extra = os.environ.get("GDN_NVCC_EXTRA", "").split()      # e.g. -DGDN_PHASE_TIMING (developer builds)
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-I", str(INCLUDE), "-o", str(tmp), *map(str, sources())]
+    cmd = [_nvcc(), *NVCC_FLAGS, "-I", str(INCLUDE), "-o", str(tmp), *map(str, sources())]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), flush=True)

@@ -23,6 +23,7 @@ namespace gdn {
 
 struct TcPlan {
     bool ready = false;
+    unsigned attr_mask = 0;                    // which launchers have raised their kernels' dynamic shared-memory limit on this plan's device
     int sm_count = 0;
     int mode = 0;                              // GDN_PATH_TC_TOKEN or GDN_PATH_TC_FRAME
     int D = 0, C = 0, NT = 0, NC = 0, BH = 0;
@@ -256,7 +257,7 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         // HPR minimises a two-term estimate: the prepass workers (all SMs but the chain workers) need
         // ceil(tiles / workers) tile times, the chain workers need groups * NT serial steps.
         const int sms = sm_count > 0 ? sm_count : 148, nct = tp.D / 64;
-        const double t_tile = tp.D == 128 ? 14.0 : 10.0, t_step = tp.D == 128 ? 2.2 : 1.3;     // microseconds, measured (a chain that trails the prepass pays the TMA latency of its shallow ring every step)
+        const double t_tile = tp.D == 128 ? 14.0 : 10.0, t_step = tp.D == 128 ? 2.2 : 1.3;     // microseconds per prepass tile / chain step: constants of the split model, measured on B200 in round 1 (2026-11); only their ratio matters
         int hpr = 1;
         double best = 1e30;
         for (int h = 1; h <= tp.BH && h * nct < sms; ++h) {
@@ -266,7 +267,6 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
             const double est = (t_pre > t_chain ? t_pre : t_chain) + 0.02 * groups;
             if (est < best - 1e-9) { best = est; hpr = h; }
         }
-        if (const char* e = getenv("GDN_FUSED_HPR")) { const int v = atoi(e); if (v > 0) hpr = v; }
         if (hpr < 1) hpr = 1;
         if (hpr > tp.BH) hpr = tp.BH;
         if (hpr * nct > sms - 1) hpr = (sms - 1) / nct > 0 ? (sms - 1) / nct : 1;
@@ -365,21 +365,19 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
     const size_t smem1 = prepass_smem_bytes<D>() + 1024;
     const size_t smem2 = ChainSmem<D>::TOTAL;
     const size_t smem3 = NB * kBlk + (C == 128 ? 1 : 2) * D * D * 2 + 256 + 1024;
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!(tp.attr_mask & 1u)) {
         cudaError_t e = set_smem(gdn_tok_prepass<D, C>, smem1);
         if (e == cudaSuccess) e = set_smem(gdn_tok_chain<D>, smem2);
         if (e == cudaSuccess) e = set_smem(gdn_tok_output<D, C>, smem3);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        tp.attr_mask |= 1u;
     }
     if (prof) prof->begin(st);
     if (D == 64 && C == 64) {
-        static bool attr64 = false;
-        if (!attr64) {
+        if (!(tp.attr_mask & 2u)) {
             cudaError_t e = set_smem(t64::gdn_tok_tile64, t64::SMEM_BYTES);
             if (e != cudaSuccess) return e;
-            attr64 = true;
+            tp.attr_mask |= 2u;
         }
         t64::gdn_tok_tile64<<<tp.BH * tp.NC, t64::kThreads, t64::SMEM_BYTES, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt64, tp.tmOl64, p);
         if (prof) prof->mark(st, "gdn_tok_tile64");
@@ -399,11 +397,10 @@ inline cudaError_t tc_launch_token(TcPlan& tp, const TokParams& p, cudaStream_t 
 template <int D>
 inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
     const size_t smem = fused::fused_smem_bytes<D>();
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!(tp.attr_mask & 4u)) {
         cudaError_t e = set_smem(fused::gdn_tok_fused<D>, smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        tp.attr_mask |= 4u;
     }
     FusedParams fp{};
     fp.t = p;
@@ -418,11 +415,10 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
 
 
 inline cudaError_t tc_launch_fused64(TcPlan& tp, const TokParams& p, cudaStream_t st, Profiler* prof) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!(tp.attr_mask & 8u)) {
         cudaError_t e = set_smem(f64::gdn_tok_fused64, t64::SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        tp.attr_mask |= 8u;
     }
     F64Params fp = tp.f64;
     fp.t = p;
@@ -441,14 +437,13 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
     const size_t smem3 = ReadSmem<D>::TOTAL;
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!(tp.attr_mask & 16u)) {
         cudaError_t e = set_smem(gdn_frm_summaries<D>, smem1);
         if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain<D>, smem2);
         if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain_bidir<D>, smem2);
         if (e == cudaSuccess) e = set_smem(gdn_frm_readout<D>, smem3);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        tp.attr_mask |= 16u;
     }
     const int sms = tp.sm_count > 0 ? tp.sm_count : 148;
     const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
@@ -512,7 +507,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
         TokParams cp{};
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
-        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dr = c.d_k; cp.dbg = nullptr;
+        cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dr = c.d_k;
         cudaError_t e = cudaSuccess;
         cudaEvent_t den_ready = nullptr;
         if (na) {
@@ -556,68 +551,12 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     p.o_ts = ts(c.o_token_stride, c.d_v);
     p.scale = c.scale;
     p.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
-    p.dbg = nullptr; p.dbg_cta = 0;
-#ifdef GDN_PHASE_TIMING
-    static long long* dbg_dev = nullptr;
-    constexpr size_t kDbgWords = 64 + 600 * 192;      // 64 phase stamps + 128 trace slots per CTA
-    if (!dbg_dev) cudaMalloc(&dbg_dev, kDbgWords * sizeof(long long));
-    cudaMemsetAsync(dbg_dev, 0, kDbgWords * sizeof(long long), st);
-    p.dbg = dbg_dev;
-    p.dbg_cta = tp.fused ? tp.NWC : 0;
-#endif
     cudaError_t e;
     if (tp.fused64) e = tc_launch_fused64(tp, p, st, prof);
     else if (tp.fused) e = (tp.D == 64) ? tc_launch_fused<64>(tp, p, st, prof) : tc_launch_fused<128>(tp, p, st, prof);
     else if (tp.D == 64) e = (tp.C == 128) ? tc_launch_token<64, 128>(tp, p, st, prof) : tc_launch_token<64, 64>(tp, p, st, prof);
     else            e = (tp.C == 128) ? tc_launch_token<128, 128>(tp, p, st, prof) : tc_launch_token<128, 64>(tp, p, st, prof);
     if (e != cudaSuccess) { if (err) *err = std::string("token tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
-#ifdef GDN_PHASE_TIMING
-    {
-        long long hst[64];
-        cudaStreamSynchronize(st);
-        cudaMemcpy(hst, p.dbg, sizeof(hst), cudaMemcpyDeviceToHost);
-        fprintf(stderr, "[gdn phase cycles]");
-        for (int i = 1; i < 16; ++i) fprintf(stderr, " %d:%lld", i, hst[i] - hst[i - 1]);
-        fprintf(stderr, " [5->19:%lld 19->20:%lld 20->21:%lld 21->16:%lld 16->18:%lld 18->17:%lld 17->6:%lld]", hst[19] - hst[5], hst[20] - hst[19], hst[21] - hst[20], hst[16] - hst[21], hst[18] - hst[16], hst[17] - hst[18], hst[6] - hst[17]);
-        fprintf(stderr, " [T1: 3->23 issue:%lld wait_all:%lld 24->4:%lld]", hst[23] - hst[3], hst[24] - hst[23], hst[4] - hst[24]);
-        fprintf(stderr, " tile(0->14):%lld total:%lld\n", hst[14] - hst[0], hst[15] - hst[0]);
-        fprintf(stderr, "[t64 tid64]");
-        for (int i = 1; i < 15; ++i) fprintf(stderr, " %d:%lld", i, hst[32 + i] - hst[32 + i - 1]);
-        fprintf(stderr, "\n");
-        fprintf(stderr, "[gdn chain step cycles] snapshot:%lld premath:%lld wait_mma:%lld ld+sub:%lld publish:%lld fence+sync:%lld total:%lld\n",
-                hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36], hst[38] - hst[37], hst[38] - hst[32]);
-        fprintf(stderr, "[gdn fused chain step 12] prev-publish->top:%lld gfull+gam:%lld Nfma:%lld wait_mma:%lld ld+sub:%lld publish:%lld | mma warp: sready-seen@%lld commit@%lld (rel. to top) state-mma-done@%lld\n",
-                hst[32] - hst[31], hst[33] - hst[32], hst[34] - hst[33], hst[35] - hst[34], hst[36] - hst[35], hst[37] - hst[36],
-                hst[41] - hst[32], hst[42] - hst[32], hst[35] - hst[32]);
-        if (const char* tf = tp.fused64 ? getenv("GDN_TRACE_FILE") : nullptr) {
-            std::vector<long long> tr(kDbgWords);
-            cudaMemcpy(tr.data(), p.dbg, kDbgWords * sizeof(long long), cudaMemcpyDeviceToHost);
-            if (FILE* f = fopen(tf, "w")) {
-                fprintf(f, "grid %d nch %d ntile %d", tp.grid, tp.f64.NCH, tp.f64.n_tile_tasks);
-                for (int i = 100; i < 140; ++i) fprintf(f, " %lld", tr[64 + i]);
-                fprintf(f, "\n");
-                for (int cta = 0; cta < tp.grid && cta < 600; ++cta) {
-                    fprintf(f, "%d", cta);
-                    for (int i = 0; i < 192; ++i) fprintf(f, " %lld", tr[64 + (size_t)cta * 192 + i]);
-                    fprintf(f, "\n");
-                }
-                fclose(f);
-            }
-        } else if (const char* tf = getenv("GDN_TRACE_FILE")) {      // fused kernel: per-CTA globaltimer trace
-            std::vector<long long> tr(kDbgWords);
-            cudaMemcpy(tr.data(), p.dbg, kDbgWords * sizeof(long long), cudaMemcpyDeviceToHost);
-            if (FILE* f = fopen(tf, "w")) {
-                fprintf(f, "grid %d nwc %d\n", tp.grid, tp.NWC);
-                for (int cta = 0; cta < tp.grid && cta < 160; ++cta) {
-                    fprintf(f, "%d", cta);
-                    for (int i = 0; i < 128; ++i) fprintf(f, " %lld", tr[64 + (size_t)cta * 128 + i]);
-                    fprintf(f, "\n");
-                }
-                fclose(f);
-            }
-        }
-    }
-#endif
     return GDN_OK;
 }
 

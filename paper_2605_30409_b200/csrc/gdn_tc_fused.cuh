@@ -49,13 +49,6 @@ __device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) 
 // the same for global memory only: the flag acquire (generic proxy) before the TMA loads of what the flag guards
 __device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
-#ifdef GDN_PHASE_TIMING
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-// developer trace: 128 slots per CTA behind the 64 phase stamps
-#define GDN_TRACE(slot) do { if (fp.t.dbg && (slot) < 128) fp.t.dbg[64 + (long long)blockIdx.x * 128 + (slot)] = gtime(); } while (0)
-#else
-#define GDN_TRACE(slot) do { } while (0)
-#endif
 
 template <int D>
 struct ChainSmem {
@@ -167,7 +160,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 if (lane == 0) {
                     fence_proxy_async_global();
                     if (feed_chain) {
-                        GDN_TRACE(2 * gs);
                         const int gst = gs % GST;
                         if (gs >= (uint32_t)GST) mbar_wait(&g_empty[gst], ((gs / GST) - 1) & 1u);
                         sts_f32(smem_u32(sGamma) + gst * 4, gam_c);      // visible to the waiters of g_full through the arrive below
@@ -202,9 +194,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             for (uint32_t gs = 0; gs < total; ++gs) {
                 const int gst = gs % GST, sb = gs % NSB;
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
-                if (gs == 12) GDN_STAMP_ANY(40);
                 mbar_wait(&s_ready[sb], (gs / NSB) & 1u);
-                if (gs == 12) GDN_STAMP_ANY(41);
                 tc_fence_after();
                 const uint32_t aG = smem_u32(sG + gst * L::GN_BYTES), aS = smem_u32(sS + sb * L::S_BYTES);
 #pragma unroll
@@ -213,7 +203,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 umma_commit(mma_chain);
                 umma_commit(&g_empty[gst]);
                 issued_st(gs + 1);                                   // the output issuer lets the chain MMA of a step go first
-                if (gs == 12) GDN_STAMP_ANY(42);
             }
         }
     } else if (warp == 14) {
@@ -278,10 +267,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             publish(gs);
             for (int c = 0; c < NT; ++c, ++gs) {
                 const int gst = gs % GST;
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(32);
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
                 const float gamma_c = lds_f32(smem_u32(sGamma) + gst * 4);
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(33);
                 {   // state-independent half, while the MMA runs: S <- gamma_c S + N_c
                     const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES + half * (D * 128));
 #pragma unroll
@@ -295,9 +282,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&g_empty[gst]);                   // gamma_c and N_c of the stage have been read
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(34);
                 mbar_wait(mma_chain, gs & 1u);
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(35);
                 tc_fence_after();
                 {
                     float v[32];
@@ -306,11 +291,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                     for (int i = 0; i < 32; ++i) S[i] -= v[i];
                 }
                 tc_fence_before();
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(36);
                 if (c + 1 < NT) publish(gs + 1);
-                if (gs == 12 && tid == 0) GDN_STAMP_ANY(37);
-                if (gs == 11 && tid == 0) GDN_STAMP_ANY(31);
-                if (tid == 0) GDN_TRACE(2 * gs + 1);
             }
             if (m_ok && m < p.dr) {
                 float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * p.dr + m) * p.dr + col0);
@@ -402,10 +383,8 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
         int bh, tile, nbh = -1, ntile = -1;
         tile_of(i, bh, tile);
         if (i + nwp < fp.total_tiles) tile_of(i + nwp, nbh, ntile);
-        if (tid == 0) GDN_TRACE(2 * it);
         // the previous tile's ready flag is published inside this tile, once its stores have completed
         tok::prepass_tile<D, 128, true>(cx, tmQ, tmK, tmV, tmG, tmN, tmQt, tmOl, p, bh, tile, it, ph, pending, fp.epoch, nbh, ntile, &gates);
-        if (tid == 0) GDN_TRACE(2 * it + 1);
         pending = fp.flags + (long long)bh * NT + tile;
     }
     if (D == 128 && tid == tok::kPrepassFlagTid && pending) tma_store_wait_all();      // this thread's share of the last tile's stores

@@ -17,8 +17,8 @@
 //                                B(bh,k)   the B part of segment k from zero  -> B_c per chunk, B_k of the whole segment;
 //                                A(bh,k)   the Gacc part of segment k from zero -> Gacc_c, gacc_c per chunk, and per segment.
 //     One step = ONE M = 64 MMA G_c x (bf16 state) with the fp32 master copy of the state row in registers.
-//   workers (the rest): a dynamic queue (one atomic counter) of tile tasks (segments interleaved, so that all chain CTAs
-//     of a stream advance together) followed by output tasks, segment-major:
+//   workers (the rest): a static round-robin list of tile tasks (segments interleaved, so that all chain CTAs of a
+//     stream advance together) followed by output tasks, segment-major:
 //       segment 0:   O_c = scale (Qt_c S_c + Ol_c)                                   one MMA
 //       segment k:   S_c = gacc_c S_k - Gacc_c S_k + B_c, then the same              two MMAs
 //     `out` is written exactly once, by a TMA store of the finished tile.
@@ -55,17 +55,6 @@ namespace f64 {
 constexpr int kReleaseBatch = 1 << 20;                // ... in batches of this many steps (4: 51.2 us, never: 49.6 us on config 2)
 constexpr bool kStepRelease = false;                 // chain CTAs release their snapshot flags per step (true) or all at the end
 
-#ifdef GDN_PHASE_TIMING
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define F64_TRACE(slot, val) do { if (fp.t.dbg && threadIdx.x == 0 && (slot) < 192) fp.t.dbg[64 + (long long)blockIdx.x * 192 + (slot)] = (val); } while (0)
-#else
-#define F64_TRACE(slot, val) do { } while (0)
-#endif
-#ifdef GDN_PHASE_TIMING
-#define F64_STAMP(slot) do { if (fp.t.dbg && unit == 0 && e == nchunk + 1) fp.t.dbg[64 + (slot)] = clock64(); } while (0)
-#else
-#define F64_STAMP(slot) do { } while (0)
-#endif
 
 using namespace tc;
 using t64::kTile;
@@ -85,6 +74,7 @@ __device__ __forceinline__ bool flag_ready(unsigned long long w, unsigned int ep
 __device__ __forceinline__ float flag_payload(unsigned long long w) { return __uint_as_float((unsigned int)(w >> 32)); }
 // (Polling with relaxed loads followed by one fence.acq_rel.gpu measured 5 us SLOWER on config 2 than acquire loads.)
 __device__ __forceinline__ void acquire_after_poll() {}
+// (and relaxed loads with no fence at all, which the memory model does not cover, gained 0.8 us: not taken)
 #define ld_relaxed64 ld_acquire64
 __device__ __forceinline__ unsigned long long wait_flag(const unsigned long long* f, unsigned int epoch, unsigned int ns = 20) {
     unsigned long long w = ld_relaxed64(f);
@@ -160,9 +150,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
         tma_load_3d(smem + st * C_STAGE, tmM3, &full[st], 0, 0, e_zg(e));
         if (zn >= 0) tma_load_3d(smem + st * C_STAGE + kTile, tmM3, &full[st], 0, 0, zn);
     };
-    F64_TRACE(128, (long long)(1000 + type));
-    F64_TRACE(0, gtime());
-    F64_TRACE(160, clock64()); F64_TRACE(161, gtime());
     unsigned long long nf0 = 0ull, nf1 = 0ull;       // thread 64: flag words of entry e + 1, requested during step e - 1
     if (tid == 64) {
         unsigned long long w0 = wait_flag(e_f0(0), ep);
@@ -170,9 +157,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
         acquire_after_poll();
         issue_load(0, w0);
         if (n > 1) { nf0 = ld_relaxed64(e_f0(1)); nf1 = e_f1(1) ? ld_relaxed64(e_f1(1)) : ~0ull; }
-#ifdef GDN_PHASE_TIMING
-        if (fp.t.dbg) fp.t.dbg[64 + (long long)blockIdx.x * 192 + 150] = gtime();
-#endif
     }
     publish(0);
     __syncthreads();
@@ -251,9 +235,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
         tc_fence_before();
         publish((e + 1) & 1);
         __syncthreads();
-        if (e == 0 || e == nchunk / 2 || e >= nchunk - 1) F64_TRACE(1 + e, gtime());
     }
-    F64_TRACE(162, clock64()); F64_TRACE(163, gtime());
     if (tid == 32) {
         tma_store_wait_all();
         if (kStepRelease) {
@@ -437,7 +419,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         t64::Tile64Maps mp{&tmQ, &tmK, &tmV, &tmM3, &tmM3, &tmR2, &tmR2, fp.zG, fp.zN, (long long)p.NC * 64, fp.rQt, fp.rOl};
         uint32_t pl = 0, ph = 0;
         const int total = fp.n_tile_tasks + fp.n_out_tasks;
-        int ntask = 0;
         // task -> (is tile task, stream, chunk, segment); chunk >= NC: nothing to do (the last segment is shorter)
         auto decode = [&](int task, bool& tile, int& bh, int& c, int& k) {
             tile = task < fp.n_tile_tasks;
@@ -470,7 +451,7 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (next < total) decode(next, ntile, nbh, nc, nk);
             const bool have_next = next < total && ntile && nc < p.NC;
             if (have_next) {
-                // the next chunk's gates -> raw buffer (ntask + 1) & 1 with 4-byte asynchronous copies (padding rows:
+                // the next chunk's gates -> the other raw buffer with 4-byte asynchronous copies (padding rows:
                 // alpha = 1, beta = 0), its K / Q / V tiles -> L2
                 if (tid < 128) {
                     const int j = tid & 63, t = nc * 64 + j;
@@ -492,7 +473,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
             }
             if (c < p.NC) {
-                F64_TRACE(2 * ntask, gtime()); F64_TRACE(128 + ntask, (long long)task);
                 if (tile) {
                     if (tid == 0) tma_store_wait_read();  // the previous task's stores have left the staging buffers
                     float gam_c = 0.f;
@@ -503,7 +483,6 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     output_task(smem, tmem, bars, &tmM3, &tmR2, &tmO, fp, bh, c, k, pl, ph, pend_flag, pend_val);
                     pend_flag = nullptr;
                 }
-                F64_TRACE(2 * ntask + 1, gtime()); ++ntask;
             }
             asm volatile("cp.async.wait_all;" ::: "memory");
             raw_sel ^= 1;

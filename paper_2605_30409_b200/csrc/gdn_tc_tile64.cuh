@@ -11,9 +11,9 @@
 // 51 KB of shared memory and 128 TMEM columns, FOUR such CTAs are resident per SM and hide each other's latencies, and
 // the sequence is three MMA round trips:
 //     S1  [K ; Q] K^T                      (M = 128: lanes 0-63 = K K^T rows, lanes 64-127 = Q K^T rows; N = 64)
-//         warps 0-1: decay-masked L -> fp32 scratch; warps 2-3: decay-masked P -> P^T (bf16)
-//         (I + L)^-1 of the 64x64 block in fp32 on CUDA cores: 16-blocks by forward substitution, 16 -> 32 -> 64 by
-//         X21 = -X22 L21 X11 (no tensor-core doubling round trips, no bf16 rounding inside the inverse)
+//         warps 0-1: decay-masked L -> bf16 rows + fp32 diagonal 16-blocks; warps 2-3: decay-masked P -> P^T (bf16)
+//         (I + L)^-1 of the 64x64 block: diagonal 16-blocks by fp32 forward substitution on CUDA cores, 16 -> 32 -> 64 by
+//         X21 = -X22 (L21 X11) with warp-level mma.sync on the bf16 blocks (no asynchronous TMEM round trips)
 //     S3  [Tm diag(beta gamma) ; Tm diag(beta)] [K | V]   (M = 128, N = 128: lanes 0-63 keep columns 0-63 = W,
 //         lanes 64-127 keep columns 64-127 = Ut; the other two quadrants are computed and ignored)
 //     S4  [Kt | P^T]^T [W | Ut]            (M = 128 as an MN-major A operand of two blocks: lanes 0-63 = [G | N] rows,
@@ -53,11 +53,6 @@ struct Tile64Maps {
     long long rQt, rOl;                               // first row of Qt / Ol in their maps
 };
 
-#ifdef GDN_PHASE_TIMING
-#define T64_STAMP(n) do { if (p.dbg && blockIdx.x == p.dbg_cta && (tid & 63) == 0) p.dbg[(n) + (tid >> 6) * 32] = clock64(); } while (0)
-#else
-#define T64_STAMP(n) do { } while (0)
-#endif
 
 __device__ __forceinline__ void sts_b16(uint32_t a, unsigned short v) { asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
 
@@ -82,8 +77,8 @@ template <bool NBF16>
 __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* bars, const Tile64Maps& mp, const TokParams& p,
                                        int bh, int chunk, uint32_t& pl, uint32_t& ph, uint32_t pre_gates = 0u,
                                        unsigned long long* pend_flag = nullptr, unsigned long long pend_val = 0ull, float* gamma_out = nullptr) {
-    // pre_gates: shared-space address of {alpha[64], beta[64]} of the chunk, copied ahead by the caller (0: read them here).  pend_flag / pend_val: a flag word of the caller's previous task, released by thread 0 once that
-    // task's bulk stores have completed (behind this chunk's first MMA issue, where the wait costs nothing).  gamma_out:
+    // pre_gates: shared-space address of {alpha[64], beta[64]} of the chunk, copied ahead by the caller (0: read them
+    // here).  pend_flag / pend_val: a flag word of the caller's previous task, released by thread 0 once that task's bulk stores have completed (behind this chunk's first MMA issue, where the wait costs nothing).  gamma_out:
     // receives gamma_C (thread 0) instead of p.gam.
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = bh / p.H, h = bh % p.H;
@@ -97,7 +92,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     const int i = tid & 63;                           // token row inside the chunk (both halves of the CTA)
     const uint32_t lane_base = (uint32_t)(warp * 32);
 
-    T64_STAMP(0);
     if (tid == 0) {
         mbar_expect_tx(bar_kq, 2 * kTile);
         tma_load_5d(smem + OFF_K, mp.tmK, bar_kq, 0, h, chunk * 64, 0, b);
@@ -138,10 +132,8 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
     auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
 
-    T64_STAMP(1);
     // ---- S1: [K ; Q] K^T -> TMEM columns 0..63 ----
     mbar_wait(bar_kq, par);
-    T64_STAMP(2);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, 64, false, false);
@@ -154,7 +146,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         }
     }
     wait_mma();
-    T64_STAMP(3);
 
     // ---- S1 epilogue.  warps 0-1 (row i of K K^T): L_ij = beta_i e^{Gam_i-Gam_j} k_i.k_j (j < i) -> bf16 row of L_bf, and
     //      its diagonal 16-block TRANSPOSED in fp32 -> scratch (for the forward substitution); warps 2-3 (row i of Q K^T):
@@ -214,7 +205,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             }
         }
     }
-    T64_STAMP(4);
 
     // ---- Tm = (I + L)^-1 -> D_bf (bf16, swizzled rows).  Diagonal 16-blocks: fp32 forward substitution on CUDA cores
     //      (tok::inv16_columns, one column per lane).  16 -> 32 -> 64: X21 = -X22 (L21 X11) with warp-level mma.sync on
@@ -261,9 +251,7 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             sts_b32(tile_addr(aDB, R1, C >> 3) + (uint32_t)(C & 7) * 2u, pack_bf16(-y[2], -y[3]));
         }
     }
-    T64_STAMP(5);
     __syncthreads();
-    T64_STAMP(6);
     {
         // 32 -> 64, all four warps: warp (mt, m2) = (warp & 1, warp >> 1) produces Y21[16 m2 .. +15][16 mt .. +15],
         // Y21 = -Y22 (L21 Y11), Y11 = D_bf[0:32][0:32], Y22 = D_bf[32:64][32:64], L21 = L_bf[32:64][0:32].
@@ -306,7 +294,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         }
     }
     __syncthreads();
-    T64_STAMP(7);
     // ---- the two scaled copies of Tm, stacked as ONE K-major A operand [128][64] written over L_bf / D_bf:
     //      rows 0-63 = Tm diag(beta gamma) (thread half 0), rows 64-127 = Tm diag(beta) (half 1).  Columns 32..63 of
     //      the rows below 32 were never written: zero.
@@ -331,7 +318,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         for (int c = 0; c < 8; ++c) st_shared_v4(aX + swz_chunk_off(row, c, 0), pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
     }
     sync_then_issue();
-    T64_STAMP(8);
 
     // ---- S3: [Tm diag(beta gamma) ; Tm diag(beta)] [K | V] -> TMEM columns 0..127 ----
     if (tid == 0) {
@@ -343,7 +329,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         umma_commit(bar_mma);
     }
     wait_mma();
-    T64_STAMP(9);
     {
         // lanes 0-63: W = columns 0..63 -> block 0 of [W | Ut]; lanes 64-127: Ut = columns 64..127 -> block 1
         float v[64];
@@ -365,7 +350,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         }
     }
     sync_then_issue();
-    T64_STAMP(10);
 
     // ---- S4: [Kt | P^T]^T [W | Ut] -> lanes 0-63: [G | N] rows, lanes 64-127: [P W | P Ut] rows ----
     if (tid == 0) {
@@ -376,7 +360,6 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
         umma_commit(bar_mma);
     }
     wait_mma();
-    T64_STAMP(11);
     if (tid < 64) {
         // summary row m = tid: G bf16 -> the P^T buffer, N fp32 as two [64][32] blocks -> the scratch (both operands are dead)
         const int m = tid;
@@ -421,11 +404,9 @@ __device__ __forceinline__ void tile64(uint8_t* smem, uint32_t tmem, uint64_t* b
             }
         }
     }
-    T64_STAMP(12);
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
-    T64_STAMP(13);
     if (tid == 0) {
         const long long r0 = (long long)bh * mp.rows_per_bh + (long long)chunk * 64;
         const int z = bh * p.NC + chunk;
@@ -463,7 +444,6 @@ gdn_tok_tile64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     uint32_t pl = 0, ph = 0;
     tile64<false>(smem, tmem, bars, mp, p, (int)blockIdx.x / p.NC, (int)blockIdx.x % p.NC, pl, ph);
     if (threadIdx.x == 0) tma_store_wait_all();
-    { const int tid = threadIdx.x; T64_STAMP(14); }
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x < 32) tmem_dealloc(tmem, 128);

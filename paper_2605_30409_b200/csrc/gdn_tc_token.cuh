@@ -52,17 +52,8 @@ struct TokParams {
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
-    long long* dbg;              // developer builds (-DGDN_PHASE_TIMING): per-phase clock64 stamps of CTA dbg_cta
-    int dbg_cta;                 // the CTA whose prepass phases are stamped (fused kernel: the first prepass worker)
 };
 
-#ifdef GDN_PHASE_TIMING
-#define GDN_STAMP(i) do { if (p.dbg && blockIdx.x == p.dbg_cta && threadIdx.x == 0) p.dbg[i] = clock64(); } while (0)
-#define GDN_STAMP_ANY(i) do { if (p.dbg && blockIdx.x == 0) p.dbg[i] = clock64(); } while (0)      // any one thread of CTA 0
-#else
-#define GDN_STAMP_ANY(i) do { } while (0)
-#define GDN_STAMP(i) do { } while (0)
-#endif
 
 namespace tok {
 
@@ -193,7 +184,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     const uint32_t aA = smem_u32(sA), aB = smem_u32(sB), aC = smem_u32(sC), aK = smem_u32(sK), aQ = smem_u32(sQ), aV = smem_u32(sV);
     const uint32_t par = it & 1u;
 
-    GDN_STAMP(0);
     // gates first: their global-load latency overlaps the barrier / TMEM / TMA set-up
     // (a persistent CTA passes `gates`: this row's alpha, beta of this tile, fetched during the previous tile)
     auto load_gates = [&](int gbh, int gtile) {
@@ -217,7 +207,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     // The three 128x128 operand buffers are never pre-zeroed: every phase that fills one writes whole rows
     // (data where the block structure has some, zeros elsewhere) -- see T2 (sA, sB) and the first X1 (sC).
 
-    GDN_STAMP(1);
     // ---- T0: in-tile inclusive scan of log alpha (every warp of a quadrant computes it, hh == 0 publishes) ----
     if (!p.log_alpha) g = logf(g);
     float x = g;
@@ -259,10 +248,8 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     auto sync_then_issue = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
 
-    GDN_STAMP(2);
     // ---- T1: K K^T -> c0 (Q K^T -> c1 follows in the shadow of the first doubling round trip) ------
     mbar_wait(bar_kq, par);
-    GDN_STAMP(3);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, 128, false, false);
@@ -273,18 +260,15 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
         // FUSED: G / N of the previous tile were staged in sA, sB, sC, which T2 overwrites once this commit
         // has been observed -- their reads must have ended first.
-        GDN_STAMP(23);
         // FUSED: G / N of the previous tile were staged in sA, sB, sC, which T2 overwrites once this commit has been
         // observed -- their reads must have ended first.  Waiting for the WRITES as well costs nothing more here (the
         // stores were issued a scan and an MMA ago) and lets the commit below also stand for "the previous tile's
         // summaries are complete in global memory", so that the ready flag can be released by another thread.
         if (FUSED) tma_store_wait_all();
-        GDN_STAMP(24);
         umma_commit(bar_mma);
     }
     wait_mma();
 
-    GDN_STAMP(4);
     // ---- T2: L (strictly lower, decay-masked) -> sA off-diagonal chunks; diagonal 32x32 block -> Ld ----
 #pragma unroll
     for (int cc = 0; cc < 4; ++cc) {
@@ -307,7 +291,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             store_roww_bf16(aB, kBlk, row, cc * 32 + cb, v);
         }
     }
-    GDN_STAMP(5);
     if (FUSED && D == 128 && it > 0 && tid == kPrepassFlagTid) tma_store_wait_all();     // this thread's share of the previous tile's stores (sC is not reused before the next CTA barrier)
     if (FUSED && prev_flag && tid == kPrepassFlagTid) {
         // The previous tile's ready flag.  A release at gpu scope takes ~800 cycles (and the fences that used to precede it
@@ -324,10 +307,8 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         if (hh == 0) {
             float v0[16], v1[16], g0[16], g1[16];
             tmem_ld16x2(tmem_addr(c0, lane_base, wq * 32), tmem_addr(c0, lane_base, wq * 32 + 16), v0, v1);
-            GDN_STAMP(19);
             ld_shared_f16(sGam + wq * 32, g0);
             ld_shared_f16(sGam + wq * 32 + 16, g1);
-            GDN_STAMP(20);
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
                 // branch-free: clamp the exponent (rows above the diagonal would be > 0), then select
@@ -335,20 +316,17 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
                 v0[e] *= m0 * fast_exp(fminf(gam_i - g0[e], 0.f));
                 v1[e] *= m1 * fast_exp(fminf(gam_i - g1[e], 0.f));
             }
-            GDN_STAMP(21);
             // L^T into the scratch: element (r = lane, j) -> Lq[j][r]   (aL: shared-space byte address of Lq, S = row stride)
             const uint32_t aL = smem_u32(Lq);
             constexpr uint32_t S = kLsStride * 4;
 #pragma unroll
             for (int e = 0; e < 16; ++e) { sts_f32(aL + e * S + lane * 4, v0[e]); sts_f32(aL + (16 + e) * S + lane * 4, v1[e]); }
             __syncwarp();
-            GDN_STAMP(16);
             // Blocked: L = [[L11, 0], [L21, L22]] in 16-blocks, X = [[X11, 0], [-X22 L21 X11, X22]].
             // Step 1 (this warp): lanes 0-15 invert I + L11, lanes 16-31 invert I + L22, each lane one column.
             const int o = lane & 16, col = lane & 15;
             float xc[16];
             inv16_columns(aL + o * S + o * 4, col, xc);
-            GDN_STAMP(18);
             __syncwarp();
             // X11 / X22 row-major over L11^T / L22^T (consumed): element (r, col) -> Lq[o + r][o + col]
 #pragma unroll
@@ -392,7 +370,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             sts_f4(aL + (16 + r2) * S + (cc0 + 4) * 4, make_float4(-acc[4], -acc[5], -acc[6], -acc[7]));
             sts_f4(aL + r2 * S + (16 + cc0) * 4, make_float4(0.f, 0.f, 0.f, 0.f));
             sts_f4(aL + r2 * S + (16 + cc0 + 4) * 4, make_float4(0.f, 0.f, 0.f, 0.f));
-            GDN_STAMP(17);
         }
         const uint32_t qbar = 1 + wq, qthreads = 32 * NH;
         // all NH warps of the quadrant pick up their columns of row `lane`
@@ -402,7 +379,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     store_roww_bf16(aB, kBlk, row, wq * 32 + cb, X);
     sync_then_issue();
 
-    GDN_STAMP(6);
     // One doubling level: Y = D (L_off D).  Only the blocks the level needs are computed, so the MMAs are
     // small (the operands are block-structured: D is block-diagonal, L_off strictly block-lower):
     //   level 1 (32 -> 64): Y[blk 2i+1, blk 2i] = D_{2i+1} L_{2i+1,2i} D_{2i}, i = 0, 1
@@ -493,7 +469,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     // ---- T3/T4: 32 -> 64 blocks: D' = D - mask(D L_off D) ------------------------------------------
     doubling_mmas(1);
-    GDN_STAMP(7);
     float Dlow[CW];                                // block (wq, wq-1) of the 64x64 inverse, odd wq
 #pragma unroll
     for (int j = 0; j < CW; ++j) Dlow[j] = 0.f;
@@ -517,7 +492,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             for (int j = 0; j < CW; ++j) { Tlow[j] = -v0[j]; Tlow[CW + j] = -v1[j]; }
         }
     }
-    GDN_STAMP(8);
     // ---- scaled copies of Tm: sA = Tm diag(beta gamma), sC = Tm diag(beta) -------------------------
 #pragma unroll
     for (int cc = 0; cc < 4; ++cc) {
@@ -540,10 +514,8 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     sync_then_issue();
 
-    GDN_STAMP(9);
     // ---- T7: W = Tm diag(beta gamma) K -> c2,  Ut = Tm diag(beta) V -> c3 ---------------------------
     mbar_wait(bar_v, par);
-    GDN_STAMP(10);
     if (tid == 0) {
         tc_fence_after();
         const uint32_t id = umma_idesc(128, D, false, true);
@@ -557,7 +529,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     wait_mma();
 
-    GDN_STAMP(11);
     // ---- round trip 6: W -> sB, Ut -> sA, P -> sC, Kt in place -------------------------------------
 #pragma unroll
     for (int cc = 0; cc < D / 32; ++cc) {
@@ -601,7 +572,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     sync_then_issue();
 
-    GDN_STAMP(12);
     // ---- T8: [N | G] = Kt^T [Ut | W] -> c0.., [P Ut | P W] -> c2.. (B operand = sA then sB, N = 2D) ----
     //      column layout of both results: [0, D) from Ut, [D, 2D) from W.  For D = 128 they take 256 columns
     //      each: [N|G] -> c0,c1 and [PUt|PW] -> c2,c3.
@@ -707,7 +677,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
     }
     if (gates && next_bh >= 0) *gates = load_gates(next_bh, next_tile);       // lands while the summary MMAs run
     wait_mma();
-    GDN_STAMP(13);
     if (C == 128) {
         stage_QO(c2, aV);                          // Qt in place in sQ, Ol -> sV: neither is an operand of [N | G]
         if (FUSED && D == 128) {
@@ -770,7 +739,6 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     }
 
-    GDN_STAMP(14);
 }
 
 template <int D, int C>
@@ -799,7 +767,6 @@ gdn_tok_prepass(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x < 32) tmem_dealloc(cx.tmem, 512);
-    GDN_STAMP(15);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -946,8 +913,6 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
             const int st = c % STAGES;
             uint8_t* base = sStage + st * L::STAGE;
             const float gamma_next = (c + 1 < p.NC) ? p.gam[(long long)bh * p.NCa + ent(c + 1)] : 0.f;
-            if (c == 10) GDN_STAMP(32);
-            if (c == 10) GDN_STAMP(33);
             mbar_wait(&bars[st], (uint32_t)(c / STAGES) & 1u);
             if (m_ok) {                                // state-independent part while the MMA runs
 #pragma unroll
@@ -964,23 +929,18 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
                     }
                 }
             }
-            if (c == 10) GDN_STAMP(34);
             mbar_wait(bar_mma, ph_mma); ph_mma ^= 1;
             tc_fence_after();
-            if (c == 10) GDN_STAMP(35);
             {
                 float v[64];
                 tmem_ld64(tmem_addr(tmem, warp * 32, 0), v);
 #pragma unroll
                 for (int i = 0; i < 64; ++i) S[i] -= v[i];
             }
-            if (c == 10) GDN_STAMP(36);
             publish_smem((c + 1) & 1);
-            if (c == 10) GDN_STAMP(37);
             fence_proxy_async();
             tc_fence_before();
             __syncthreads();
-            if (c == 10) GDN_STAMP(38);
             gamma_c = gamma_next;
         }
         if (p.zvec) {

@@ -63,7 +63,7 @@ def _cfg(**kw):
     (dict(chunk=96), gdn.GDN_ERR_INVALID_ARG),
     (dict(io_dtype=7), gdn.GDN_ERR_INVALID_ARG),
     (dict(flags=1 << 20), gdn.GDN_ERR_INVALID_ARG),
-    (dict(d_k=112), gdn.GDN_ERR_UNSUPPORTED),                     # 112 via padding is NEXT
+    (dict(d_k=112), gdn.GDN_ERR_UNSUPPORTED),                     # d_k = 112 with d_v = 64: rectangular 112 is not supported (112 x 112 bf16 is)
     (dict(d_v=48), gdn.GDN_ERR_UNSUPPORTED),
     (dict(flags=gdn.GDN_FLAG_BIDIR), gdn.GDN_ERR_UNSUPPORTED),
     (dict(q_token_stride=3 * 2 * 64 + 4), gdn.GDN_ERR_ALIGNMENT),  # not a multiple of 8
