@@ -139,6 +139,70 @@ gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan,
                                     gdn_stream_t stream);
 
 /*
+ * Front end of the GDN block (App. G.2-G.3, G.5; Alg. 1 "Require: qkv, beta, decay alpha, normalization
+ * weights, RoPE tables", L325).  bf16 plans only; D = cfg.d_k = cfg.d_v a multiple of 8, at most 128.
+ *
+ * gdn_featmap_args_t: the operands of the feature map of Eq. 12 (L552) with the key rescale of L554,
+ *     x^ = rho_3D(ReLU(RMSNorm(x))),  K and K^ additionally * 1/sqrt(D N),  N = cfg.group tokens per frame.
+ *   q, k       [B,T,H,D] bf16 raw projections (Eq. 11), token strides cfg.q_token_stride / cfg.k_token_stride
+ *              (a packed qkv [B,T,3,H,D] tensor works), device
+ *   rms_wq/wk  [H,D] fp32 RMSNorm weights; RMSNorm is taken over the D channels of one head:
+ *              x_i / sqrt(mean_j x_j^2 + rms_eps) * w_i (reading 23), device
+ *   rope_cos/sin [T, D/2] fp32: the rotation of the ADJACENT channel pair (2i, 2i+1) of token t (reading 24), device
+ */
+typedef struct {
+    const void *q, *k;
+    const float *rms_wq, *rms_wk;
+    const float *rope_cos, *rope_sin;
+    float rms_eps;
+} gdn_featmap_args_t;
+
+/*
+ * gdn_feature_map: q_rot, k_rot (for the KV memory, Eq. 18-19, 22) and q_raw, k_raw (un-rotated, for the normaliser,
+ *   Eq. 20-22) from ONE read of q and k.  Outputs: dense [B,T,H,D] bf16, device, caller-owned, must not alias the inputs.
+ */
+gdn_status_t gdn_feature_map(gdn_plan_t* plan, const gdn_featmap_args_t* args,
+                             void* q_rot, void* k_rot, void* q_raw, void* k_raw, gdn_stream_t stream);
+
+/*
+ * gdn_gate_args_t / gdn_compute_gates: the gates of Eq. 13-15 (L562-L572) from the per-head latent features x:
+ *     alpha_f = exp(-e^{A_log} softplus(W_alpha . mean_n x_{f,n} + b_alpha))  per frame (group) and head,
+ *     beta_n  = sigmoid(W_beta . x_n + b_beta)                                 per token and head.
+ *   x [B,T,H,D] bf16 with token stride x_token_stride (0 = dense); w_alpha, w_beta [H,D] fp32; b_alpha, a_log, b_beta [H]
+ *   fp32; all device.  alpha_out [B,H,T/G] fp32 receives alpha, or log(alpha) when the plan carries GDN_FLAG_LOG_ALPHA
+ *   (recommended: the path only ever uses differences of cumulative logs); beta_out [B,H,T] fp32.
+ *   Sums have a fixed order: results are bit-identical from run to run.
+ */
+typedef struct {
+    const void* x;
+    int64_t x_token_stride;
+    const float *w_alpha, *b_alpha, *a_log, *w_beta, *b_beta;
+} gdn_gate_args_t;
+
+gdn_status_t gdn_compute_gates(gdn_plan_t* plan, const gdn_gate_args_t* args, float* alpha_out, float* beta_out,
+                               gdn_stream_t stream);
+
+/*
+ * gdn_forward_chunk_full: the operator at the boundary of the paper's kernel (Alg. 1): feature map on q, k
+ *   -> [gates from x] -> GDN recurrence with normalised readout (and the bidirectional in-chunk scan when the plan
+ *   carries GDN_FLAG_BIDIR) -> output gate, out = G (.) Y (Eq. 23; the projection W_o is outside).
+ *   Frame-wise bf16 tensor-core plans created with GDN_FLAG_NORMALIZER only (else UNSUPPORTED).
+ *   fm         feature-map operands (required)
+ *   v          [B,T,H,D] bf16, token stride cfg.v_token_stride
+ *   gates      NULL: alpha [B,H,T/G] and beta [B,H,T] are given; else they are computed into plan-owned buffers
+ *              (alpha, beta ignored)
+ *   out_gate   G_f = SiLU(W_g X_f + b_g) evaluated (Eq. 16), [B,T,H,D] bf16 with token stride cfg.o_token_stride, or
+ *              NULL (no gate)
+ *   S_in, z_in, out, S_out, z_out: as gdn_forward_chunk_norm.
+ *   The four feature tensors live in plan-owned device buffers (4 x B*T*H*D bf16, allocated at the first call).
+ */
+gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* fm, const void* v,
+                                    const gdn_gate_args_t* gates, const float* alpha, const float* beta,
+                                    const void* out_gate,
+                                    const float* S_in, const float* z_in,
+                                    void* out, float* S_out, float* z_out, gdn_stream_t stream);
+
+/*
  * gdn_forward_chunk_host: the same operator with HOST buffers (dense layouts, strides in the plan are
  *   ignored; pinned memory recommended).  Copies the inputs to plan-owned device staging buffers on
  *   `stream`, runs gdn_forward_chunk, copies out and state_out back, and returns without synchronising:

@@ -31,6 +31,7 @@ GDN_FLAG_NORMALIZER, GDN_FLAG_BIDIR, GDN_FLAG_LOG_ALPHA, GDN_FLAG_FORCE_SIMT, GD
 PATH_NAMES = {0: "simt_fp32", 1: "tc_token", 2: "tc_frame"}
 EXPORTED_SYMBOLS = [
     "gdn_plan", "gdn_forward_chunk", "gdn_forward_chunk_norm", "gdn_forward_chunk_host", "gdn_destroy",
+    "gdn_feature_map", "gdn_compute_gates", "gdn_forward_chunk_full",
     "gdn_plan_get_info", "gdn_plan_set_profiling", "gdn_plan_kernel_times", "gdn_status_string", "gdn_last_error",
     "gdn_version",
 ]
@@ -53,6 +54,18 @@ class GdnPlanInfo(ctypes.Structure):
     """Mirror of gdn_plan_info_t."""
     _fields_ = [("path", ctypes.c_int32), ("chunk", ctypes.c_int32), ("launches_per_call", ctypes.c_int32),
                 ("sm_count", ctypes.c_int32), ("workspace_bytes", ctypes.c_uint64)]
+
+
+class GdnFeatmapArgs(ctypes.Structure):
+    """Mirror of gdn_featmap_args_t."""
+    _fields_ = [("q", ctypes.c_void_p), ("k", ctypes.c_void_p), ("rms_wq", ctypes.c_void_p), ("rms_wk", ctypes.c_void_p),
+                ("rope_cos", ctypes.c_void_p), ("rope_sin", ctypes.c_void_p), ("rms_eps", ctypes.c_float)]
+
+
+class GdnGateArgs(ctypes.Structure):
+    """Mirror of gdn_gate_args_t."""
+    _fields_ = [("x", ctypes.c_void_p), ("x_token_stride", ctypes.c_int64), ("w_alpha", ctypes.c_void_p),
+                ("b_alpha", ctypes.c_void_p), ("a_log", ctypes.c_void_p), ("w_beta", ctypes.c_void_p), ("b_beta", ctypes.c_void_p)]
 
 
 class GdnError(RuntimeError):
@@ -83,6 +96,13 @@ def lib() -> ctypes.CDLL:
         L.gdn_forward_chunk_norm.argtypes = [vp] + [vp] * 5 + [fp] * 4 + [vp, fp, fp, vp]
         L.gdn_forward_chunk_host.restype = ctypes.c_int
         L.gdn_forward_chunk_host.argtypes = [vp, vp, vp, vp, fp, fp, fp, vp, fp, vp]
+        L.gdn_feature_map.restype = ctypes.c_int
+        L.gdn_feature_map.argtypes = [vp, ctypes.POINTER(GdnFeatmapArgs), vp, vp, vp, vp, vp]
+        L.gdn_compute_gates.restype = ctypes.c_int
+        L.gdn_compute_gates.argtypes = [vp, ctypes.POINTER(GdnGateArgs), fp, fp, vp]
+        L.gdn_forward_chunk_full.restype = ctypes.c_int
+        L.gdn_forward_chunk_full.argtypes = [vp, ctypes.POINTER(GdnFeatmapArgs), vp, ctypes.POINTER(GdnGateArgs), fp, fp, vp,
+                                             fp, fp, vp, fp, fp, vp]
         L.gdn_destroy.restype = ctypes.c_int
         L.gdn_destroy.argtypes = [vp]
         L.gdn_plan_get_info.restype = ctypes.c_int
@@ -170,6 +190,30 @@ def gdn_forward_chunk_host(plan, q, k, v, alpha, beta, state_in, out, state_out,
                                               _ptr(state_in), _ptr(out), _ptr(state_out), _stream_handle(stream)))
 
 
+def make_featmap_args(q, k, rms_wq, rms_wk, rope_cos, rope_sin, rms_eps=1e-6) -> GdnFeatmapArgs:
+    return GdnFeatmapArgs(_ptr(q), _ptr(k), _ptr(rms_wq), _ptr(rms_wk), _ptr(rope_cos), _ptr(rope_sin), rms_eps)
+
+
+def make_gate_args(x, w_alpha, b_alpha, a_log, w_beta, b_beta, x_token_stride=0) -> GdnGateArgs:
+    return GdnGateArgs(_ptr(x), x_token_stride, _ptr(w_alpha), _ptr(b_alpha), _ptr(a_log), _ptr(w_beta), _ptr(b_beta))
+
+
+def gdn_feature_map(plan, fm: GdnFeatmapArgs, q_rot, k_rot, q_raw, k_raw, stream=None) -> None:
+    _check(plan, lib().gdn_feature_map(plan, ctypes.byref(fm), _ptr(q_rot), _ptr(k_rot), _ptr(q_raw), _ptr(k_raw),
+                                       _stream_handle(stream)))
+
+
+def gdn_compute_gates(plan, ga: GdnGateArgs, alpha_out, beta_out, stream=None) -> None:
+    _check(plan, lib().gdn_compute_gates(plan, ctypes.byref(ga), _ptr(alpha_out), _ptr(beta_out), _stream_handle(stream)))
+
+
+def gdn_forward_chunk_full(plan, fm: GdnFeatmapArgs, v, gates: Optional[GdnGateArgs], alpha, beta, out_gate, S_in, z_in,
+                           out, S_out, z_out, stream=None) -> None:
+    _check(plan, lib().gdn_forward_chunk_full(plan, ctypes.byref(fm), _ptr(v), ctypes.byref(gates) if gates is not None else None,
+                                              _ptr(alpha), _ptr(beta), _ptr(out_gate), _ptr(S_in), _ptr(z_in), _ptr(out),
+                                              _ptr(S_out), _ptr(z_out), _stream_handle(stream)))
+
+
 def gdn_destroy(plan) -> None:
     if plan:
         lib().gdn_destroy(plan)
@@ -212,6 +256,15 @@ class GdnPlan:
 
     def forward_norm(self, *a, stream=None):
         gdn_forward_chunk_norm(self.handle, *a, stream=stream)
+
+    def feature_map(self, fm, q_rot, k_rot, q_raw, k_raw, stream=None):
+        gdn_feature_map(self.handle, fm, q_rot, k_rot, q_raw, k_raw, stream)
+
+    def compute_gates(self, ga, alpha_out, beta_out, stream=None):
+        gdn_compute_gates(self.handle, ga, alpha_out, beta_out, stream)
+
+    def forward_full(self, fm, v, gates, alpha, beta, out_gate, S_in, z_in, out, S_out, z_out, stream=None):
+        gdn_forward_chunk_full(self.handle, fm, v, gates, alpha, beta, out_gate, S_in, z_in, out, S_out, z_out, stream)
 
     def forward_host(self, q, k, v, alpha, beta, state_in, out, state_out, stream=None):
         gdn_forward_chunk_host(self.handle, q, k, v, alpha, beta, state_in, out, state_out, stream)

@@ -11,6 +11,7 @@
 #include <string>
 #include <vector>
 
+#include "gdn_frontend.cuh"
 #include "gdn_profile.cuh"
 #include "gdn_simt.cuh"
 #include "gdn_tc.cuh"
@@ -74,6 +75,10 @@ struct gdn_plan {
     void* workspace = nullptr;
     size_t workspace_bytes = 0;
     float* z_stage = nullptr;     // copy of z_in when z_out aliases it
+    // front end (gdn_feature_map / gdn_compute_gates / gdn_forward_chunk_full), allocated at first use
+    void* fe_feat = nullptr;      // q_rot | k_rot | q_raw | k_raw, dense [B,T,H,D] bf16 each
+    float* fe_gates = nullptr;    // alpha [B,H,F] | beta [B,H,T] | partial frame sums | counters
+    int fe_nspl = 1;
     Staging host;
     gdn::TcPlan tc;               // tensor-core path state (tensor maps, workspace carving)
     gdn::Profiler prof;           // optional per-kernel CUDA events (bench roofline)
@@ -123,7 +128,8 @@ gdn_status_t check_device(gdn_plan_t* p) {
 gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const void* v,
                           const void* q_raw, const void* k_raw,
                           const float* alpha, const float* beta, const float* S_in, const float* z_in,
-                          void* out, float* S_out, float* z_out, cudaStream_t st, bool normalizer) {
+                          void* out, float* S_out, float* z_out, cudaStream_t st, bool normalizer,
+                          const void* out_gate = nullptr, bool dense_qk = false) {
     const gdn_config_t& c = p->cfg;
     const size_t state_elems = (size_t)c.B * c.H * c.d_k * c.d_v;
     if (c.B == 0 || c.H == 0) return GDN_OK;
@@ -159,6 +165,7 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
     if (p->path != GDN_PATH_SIMT_FP32) {
         std::string msg;
         gdn::NormArgs na{q_raw, k_raw, z_in, z_out};
+        na.gate = out_gate; na.g_ts = c.o_token_stride; na.dense_qk = dense_qk;
         gdn_status_t ts = gdn::tc_forward(p->tc, c, q, k, v, alpha, beta, S_in, out, S_out, st, &p->prof, &msg, normalizer ? &na : nullptr);
         if (ts != GDN_OK) return fail(p, ts, msg);
         return GDN_OK;
@@ -188,6 +195,88 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e, "gdn_simt_kernel launch");
     return GDN_OK;
+}
+
+
+// ---- front end ----------------------------------------------------------------------------------------
+gdn_status_t fe_check(gdn_plan_t* p) {
+    const gdn_config_t& c = p->cfg;
+    if (c.io_dtype != GDN_BF16 || c.d_k != c.d_v || c.d_k % 8 != 0 || c.d_k > 128)
+        return fail(p, GDN_ERR_UNSUPPORTED, "the front end needs a bf16 plan with d_k = d_v a multiple of 8, at most 128");
+    gdn_status_t ds = check_device(p);
+    if (ds != GDN_OK) return ds;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device)
+        return fail(p, GDN_ERR_INVALID_ARG, "the current device is not the one the plan was created on");
+    return GDN_OK;
+}
+
+gdn_status_t featmap_impl(gdn_plan_t* p, const gdn_featmap_args_t* a, void* q_rot, void* k_rot, void* q_raw, void* k_raw, cudaStream_t st, bool mark = true) {
+    const gdn_config_t& c = p->cfg;
+    if (!a || !a->q || !a->k || !a->rms_wq || !a->rms_wk || !a->rope_cos || !a->rope_sin || !q_rot || !k_rot || !q_raw || !k_raw)
+        return fail(p, GDN_ERR_INVALID_ARG, "a required feature-map pointer is NULL");
+    const void* ptrs[] = {a->q, a->k, a->rms_wq, a->rms_wk, a->rope_cos, a->rope_sin, q_rot, k_rot, q_raw, k_raw};
+    for (const void* ptr : ptrs) if (!aligned16(ptr)) return fail(p, GDN_ERR_ALIGNMENT, "tensor pointers must be 16-byte aligned");
+    if (c.B == 0 || c.H == 0 || c.T == 0) return GDN_OK;
+    gdn::FeatmapParams fp{};
+    fp.q = static_cast<const __nv_bfloat16*>(a->q); fp.k = static_cast<const __nv_bfloat16*>(a->k);
+    fp.wq = a->rms_wq; fp.wk = a->rms_wk; fp.cosT = a->rope_cos; fp.sinT = a->rope_sin;
+    fp.q_rot = static_cast<__nv_bfloat16*>(q_rot); fp.k_rot = static_cast<__nv_bfloat16*>(k_rot);
+    fp.q_raw = static_cast<__nv_bfloat16*>(q_raw); fp.k_raw = static_cast<__nv_bfloat16*>(k_raw);
+    fp.q_ts = tok_stride(c.q_token_stride, c.H, c.d_k); fp.k_ts = tok_stride(c.k_token_stride, c.H, c.d_k);
+    fp.B = c.B; fp.T = c.T; fp.H = c.H; fp.D = c.d_k;
+    fp.rms_eps = a->rms_eps;
+    fp.kscale = 1.f / sqrtf((float)c.d_k * (float)c.group);
+    const long long rows = (long long)c.B * c.T * c.H;
+    long long blocks = (rows + 15) / 16;
+    const long long cap = 8LL * (p->sm_count > 0 ? p->sm_count : 148);
+    if (blocks > cap) blocks = cap;
+    gdn::fe::gdn_featmap_kernel<<<(int)blocks, gdn::fe::kFeThreads, 0, st>>>(fp);
+    if (mark) p->prof.mark(st, "gdn_featmap_kernel");
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_featmap_kernel launch");
+}
+
+size_t fe_up4(size_t n) { return (n + 3) / 4 * 4; }        // 16-byte aligned sub-buffers
+
+gdn_status_t fe_gate_buffers(gdn_plan_t* p) {
+    if (p->fe_gates) return GDN_OK;
+    const gdn_config_t& c = p->cfg;
+    const size_t BH = (size_t)c.B * c.H, F = (size_t)(c.T / c.group);
+    // splits per frame: enough CTAs to fill the GPU, at least 64 tokens each
+    int nspl = (int)((4 * (size_t)(p->sm_count > 0 ? p->sm_count : 148) + BH * F - 1) / (BH * F));
+    const int max_spl = (c.group + 63) / 64;
+    if (nspl > max_spl) nspl = max_spl;
+    if (nspl < 1) nspl = 1;
+    p->fe_nspl = nspl;
+    const size_t words = fe_up4(BH * F) + fe_up4(BH * c.T) + BH * F * nspl + BH * F;      // alpha | beta | partials | counters
+    if (cudaMalloc(&p->fe_gates, words * 4) != cudaSuccess) { cudaGetLastError(); return fail(p, GDN_ERR_NOMEM, "gate buffer allocation failed"); }
+    if (cudaMemset(p->fe_gates, 0, words * 4) != cudaSuccess) { cudaGetLastError(); return fail(p, GDN_ERR_CUDA, "gate buffer initialisation failed"); }
+    return GDN_OK;
+}
+
+gdn_status_t gates_impl(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_out, float* beta_out, cudaStream_t st, bool mark = true) {
+    const gdn_config_t& c = p->cfg;
+    if (!a || !a->x || !a->w_alpha || !a->b_alpha || !a->a_log || !a->w_beta || !a->b_beta || !alpha_out || !beta_out)
+        return fail(p, GDN_ERR_INVALID_ARG, "a required gate pointer is NULL");
+    if (!aligned16(a->x) || (a->x_token_stride % 8) != 0) return fail(p, GDN_ERR_ALIGNMENT, "x must be 16-byte aligned with a token stride that is a multiple of 8");
+    if (c.B == 0 || c.H == 0 || c.T == 0) return GDN_OK;
+    gdn_status_t bs = fe_gate_buffers(p);
+    if (bs != GDN_OK) return bs;
+    const size_t BH = (size_t)c.B * c.H, F = (size_t)(c.T / c.group);
+    gdn::GateParams gp{};
+    gp.x = static_cast<const __nv_bfloat16*>(a->x);
+    gp.w_alpha = a->w_alpha; gp.b_alpha = a->b_alpha; gp.a_log = a->a_log; gp.w_beta = a->w_beta; gp.b_beta = a->b_beta;
+    gp.alpha_out = alpha_out; gp.beta_out = beta_out;
+    gp.part = p->fe_gates + fe_up4(BH * F) + fe_up4(BH * c.T);
+    gp.counters = reinterpret_cast<unsigned int*>(gp.part + BH * F * p->fe_nspl);
+    gp.x_ts = tok_stride(a->x_token_stride, c.H, c.d_k);
+    gp.B = c.B; gp.T = c.T; gp.H = c.H; gp.D = c.d_k; gp.G = c.group; gp.F = (int)F; gp.NSPL = p->fe_nspl;
+    gp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
+    gdn::fe::gdn_gates_kernel<<<dim3((unsigned)(BH * F), (unsigned)p->fe_nspl), gdn::fe::kFeThreads, 0, st>>>(gp);
+    if (mark) p->prof.mark(st, "gdn_gates_kernel");
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_gates_kernel launch");
 }
 
 }  // namespace
@@ -290,6 +379,58 @@ gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan, const void* q_rot, const v
         return fail(plan, GDN_ERR_INVALID_ARG, "plan was not created with GDN_FLAG_NORMALIZER");
     return forward_impl(plan, q_rot, k_rot, v, q_raw, k_raw, alpha, beta, S_in, z_in, out, S_out, z_out,
                         static_cast<cudaStream_t>(stream), true);
+}
+
+
+gdn_status_t gdn_feature_map(gdn_plan_t* plan, const gdn_featmap_args_t* args, void* q_rot, void* k_rot, void* q_raw, void* k_raw,
+                             gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    gdn_status_t s = fe_check(plan);
+    if (s != GDN_OK) return s;
+    plan->prof.begin(static_cast<cudaStream_t>(stream));
+    return featmap_impl(plan, args, q_rot, k_rot, q_raw, k_raw, static_cast<cudaStream_t>(stream));
+}
+
+gdn_status_t gdn_compute_gates(gdn_plan_t* plan, const gdn_gate_args_t* args, float* alpha_out, float* beta_out, gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    gdn_status_t s = fe_check(plan);
+    if (s != GDN_OK) return s;
+    plan->prof.begin(static_cast<cudaStream_t>(stream));
+    return gates_impl(plan, args, alpha_out, beta_out, static_cast<cudaStream_t>(stream));
+}
+
+gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* fm, const void* v, const gdn_gate_args_t* gates,
+                                    const float* alpha, const float* beta, const void* out_gate, const float* S_in, const float* z_in,
+                                    void* out, float* S_out, float* z_out, gdn_stream_t stream) {
+    if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
+    const gdn_config_t& c = plan->cfg;
+    if (!(c.flags & GDN_FLAG_NORMALIZER) || plan->path != GDN_PATH_TC_FRAME)
+        return fail(plan, GDN_ERR_UNSUPPORTED, "gdn_forward_chunk_full needs a frame-wise bf16 tensor-core plan created with GDN_FLAG_NORMALIZER");
+    gdn_status_t s = fe_check(plan);
+    if (s != GDN_OK) return s;
+    if (!S_out || !z_out || !out || !v) return fail(plan, GDN_ERR_INVALID_ARG, "a required tensor pointer is NULL");
+    if (out_gate && !aligned16(out_gate)) return fail(plan, GDN_ERR_ALIGNMENT, "out_gate must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (c.B == 0 || c.H == 0 || c.T == 0)
+        return forward_impl(plan, nullptr, nullptr, nullptr, nullptr, nullptr, alpha, beta, S_in, z_in, out, S_out, z_out, st, true);
+    const size_t feat = (size_t)c.B * c.T * c.H * c.d_k;
+    if (!plan->fe_feat) {
+        if (cudaMalloc(&plan->fe_feat, 4 * feat * 2) != cudaSuccess) { cudaGetLastError(); return fail(plan, GDN_ERR_NOMEM, "feature buffer allocation failed"); }
+    }
+    __nv_bfloat16* fb = static_cast<__nv_bfloat16*>(plan->fe_feat);
+    if (gates) {
+        s = fe_gate_buffers(plan);
+        if (s != GDN_OK) return s;
+        float* a_buf = plan->fe_gates;
+        float* b_buf = plan->fe_gates + fe_up4((size_t)c.B * c.H * (c.T / c.group));
+        s = gates_impl(plan, gates, a_buf, b_buf, st, false);
+        if (s != GDN_OK) return s;
+        alpha = a_buf; beta = b_buf;
+    }
+    s = featmap_impl(plan, fm, fb, fb + feat, fb + 2 * feat, fb + 3 * feat, st, false);
+    if (s != GDN_OK) return s;
+    return forward_impl(plan, fb, fb + feat, v, fb + 2 * feat, fb + 3 * feat, alpha, beta, S_in, z_in, out, S_out, z_out, st, true,
+                        out_gate, true);
 }
 
 gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const void* k_host, const void* v_host,
@@ -412,6 +553,7 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
 }
 
 gdn_status_t gdn_destroy(gdn_plan_t* plan) {
+    if (plan) { if (plan->fe_feat) cudaFree(plan->fe_feat); if (plan->fe_gates) cudaFree(plan->fe_gates); plan->fe_feat = nullptr; plan->fe_gates = nullptr; }
     if (!plan) return GDN_OK;
     gdn::tc_plan_free(plan->tc);
     plan->prof.set_enabled(false);

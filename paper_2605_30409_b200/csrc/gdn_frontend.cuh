@@ -1,0 +1,183 @@
+// gdn_frontend.cuh -- the front end of the GDN block around the recurrence (App. G.2, G.3; Alg. 1 "Require:
+// qkv, beta, decay alpha, normalization weights, RoPE tables", L325): both are HBM-bound element-wise / reduction passes
+// (no contraction worth a tensor core), written for coalesced 16-byte accesses.
+//
+//   gdn_featmap_kernel   Eq. 12 (L552) + key rescale (L554): per (token, head) row of D channels
+//                            y = ReLU(RMSNorm(x) * w),  raw = y,  rot = rho(y) on adjacent channel pairs,
+//                            keys additionally * 1/sqrt(D N).  q and k are read ONCE and all four feature tensors the
+//                            recurrence needs (q_rot, k_rot for the KV memory; q_raw, k_raw for the normaliser) leave.
+//   gdn_gates_kernel     Eq. 13-15 (L562-L572): beta_n = sigmoid(W_beta . x_n + b_beta) per token,
+//                            alpha_f = exp(-e^{A_log} softplus(W_alpha . mean_n x_n + b_alpha)) per frame.  The mean
+//                            commutes with the projection, so the frame sum of the per-token dots is accumulated in a
+//                            FIXED order (per 16-lane group, then over groups, then over the splits of a frame by the
+//                            last CTA to arrive): reruns are bit-identical.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gdn {
+
+struct FeatmapParams {
+    const __nv_bfloat16 *q, *k;            // [B][T][H][D], token strides q_ts / k_ts (elements)
+    const float *wq, *wk;                  // [H][D] RMSNorm weights
+    const float *cosT, *sinT;              // [T][D/2] rotation tables
+    __nv_bfloat16 *q_rot, *k_rot, *q_raw, *k_raw;   // dense [B][T][H][D]
+    long long q_ts, k_ts;
+    int B, T, H, D;
+    float rms_eps, kscale;                 // kscale = 1 / sqrt(D N)
+};
+
+struct GateParams {
+    const __nv_bfloat16* x;                // [B][T][H][D], token stride x_ts
+    const float *w_alpha, *b_alpha, *a_log, *w_beta, *b_beta;   // [H][D], [H], [H], [H][D], [H]
+    float *alpha_out, *beta_out;           // [B][H][F], [B][H][T]
+    float* part;                           // [B*H*F][NSPL] partial frame sums of W_alpha . x_n
+    unsigned int* counters;                // [B*H*F], zero between calls (self-resetting)
+    long long x_ts;
+    int B, T, H, D, G, F, NSPL;
+    int log_alpha;                         // write log(alpha) instead of alpha (plans with GDN_FLAG_LOG_ALPHA)
+};
+
+namespace fe {
+
+__device__ __forceinline__ void unpack8f(const uint4& u, float (&f)[8]) {
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const float2 t = __bfloat1622float2(h[i]); f[2 * i] = t.x; f[2 * i + 1] = t.y; }
+}
+__device__ __forceinline__ uint4 pack8f(const float (&f)[8]) {
+    uint4 u;
+    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&u);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
+    return u;
+}
+// sum over the 16 lanes of a half-warp (xor butterflies stay inside the half)
+__device__ __forceinline__ float group16_sum(float v) {
+#pragma unroll
+    for (int o = 8; o >= 1; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+constexpr int kFeThreads = 256;            // 16 rows of 16 lanes; a lane owns 8 consecutive channels (D <= 128)
+
+__global__ void __launch_bounds__(kFeThreads)
+gdn_featmap_kernel(const FeatmapParams p) {
+    const int g = threadIdx.x >> 4, l = threadIdx.x & 15;
+    const long long rows = (long long)p.B * p.T * p.H;
+    const int c0 = l * 8;
+    const bool on = c0 < p.D;
+    const float inv_d = 1.f / (float)p.D;
+    for (long long r0 = (long long)blockIdx.x * 16; r0 < rows; r0 += (long long)gridDim.x * 16) {     // uniform trip count: the
+        const bool valid = r0 + g < rows;                                                             // shuffles need the whole warp
+        const long long r = valid ? r0 + g : rows - 1;
+        const int h = (int)(r % p.H);
+        const long long bt = r / p.H;
+        const int t = (int)(bt % p.T);
+        float xq[8], xk[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { xq[i] = 0.f; xk[i] = 0.f; }
+        if (on) {
+            unpack8f(__ldg(reinterpret_cast<const uint4*>(p.q + bt * p.q_ts + (long long)h * p.D + c0)), xq);
+            unpack8f(__ldg(reinterpret_cast<const uint4*>(p.k + bt * p.k_ts + (long long)h * p.D + c0)), xk);
+        }
+        float sq = 0.f, sk = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { sq = fmaf(xq[i], xq[i], sq); sk = fmaf(xk[i], xk[i], sk); }
+        sq = group16_sum(sq);
+        sk = group16_sum(sk);
+        if (!on || !valid) continue;
+        const float rq = rsqrtf(sq * inv_d + p.rms_eps), rk = rsqrtf(sk * inv_d + p.rms_eps);
+        const float4 wq0 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0));
+        const float4 wq1 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0 + 4));
+        const float4 wk0 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0));
+        const float4 wk1 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0 + 4));
+        const float wqv[8] = {wq0.x, wq0.y, wq0.z, wq0.w, wq1.x, wq1.y, wq1.z, wq1.w};
+        const float wkv[8] = {wk0.x, wk0.y, wk0.z, wk0.w, wk1.x, wk1.y, wk1.z, wk1.w};
+        const float4 cs = __ldg(reinterpret_cast<const float4*>(p.cosT + (long long)t * (p.D / 2) + c0 / 2));
+        const float4 sn = __ldg(reinterpret_cast<const float4*>(p.sinT + (long long)t * (p.D / 2) + c0 / 2));
+        const float cv[4] = {cs.x, cs.y, cs.z, cs.w}, sv[4] = {sn.x, sn.y, sn.z, sn.w};
+        float qr[8], kr[8], qo[8], ko[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            qr[i] = fmaxf(xq[i] * rq * wqv[i], 0.f);
+            kr[i] = fmaxf(xk[i] * rk * wkv[i], 0.f) * p.kscale;
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            qo[2 * i] = qr[2 * i] * cv[i] - qr[2 * i + 1] * sv[i];
+            qo[2 * i + 1] = qr[2 * i] * sv[i] + qr[2 * i + 1] * cv[i];
+            ko[2 * i] = kr[2 * i] * cv[i] - kr[2 * i + 1] * sv[i];
+            ko[2 * i + 1] = kr[2 * i] * sv[i] + kr[2 * i + 1] * cv[i];
+        }
+        const long long o = r * p.D + c0;
+        *reinterpret_cast<uint4*>(p.q_raw + o) = pack8f(qr);
+        *reinterpret_cast<uint4*>(p.k_raw + o) = pack8f(kr);
+        *reinterpret_cast<uint4*>(p.q_rot + o) = pack8f(qo);
+        *reinterpret_cast<uint4*>(p.k_rot + o) = pack8f(ko);
+    }
+}
+
+// grid = (B*H*F, NSPL).  Split s of frame (b, h, f) owns the tokens n = s*16*per + ... : group g of the CTA takes tokens
+// base + g, base + g + 16, ... in order, so every partial sum has a fixed association.
+__global__ void __launch_bounds__(kFeThreads)
+gdn_gates_kernel(const GateParams p) {
+    __shared__ float s_sum[16];
+    __shared__ unsigned int s_last;
+    const int g = threadIdx.x >> 4, l = threadIdx.x & 15;
+    const int bhf = blockIdx.x, s = blockIdx.y;
+    const int f = bhf % p.F, bh = bhf / p.F, b = bh / p.H, h = bh % p.H;
+    const int per = (p.G + p.NSPL - 1) / p.NSPL;               // tokens per split
+    const int n_lo = s * per, n_hi = min(n_lo + per, p.G);
+    const int c0 = l * 8;
+    const bool on = c0 < p.D;
+    float wa[8], wb[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { wa[i] = 0.f; wb[i] = 0.f; }
+    if (on) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { wa[i] = __ldg(p.w_alpha + (long long)h * p.D + c0 + i); wb[i] = __ldg(p.w_beta + (long long)h * p.D + c0 + i); }
+    }
+    const float bb = __ldg(p.b_beta + h);
+    float acc = 0.f;                                           // sum of W_alpha . x_n over this group's tokens
+    for (int n0 = n_lo; n0 < n_hi; n0 += 16) {                 // uniform trip count: the shuffles need the whole warp
+        const int n = n0 + g;
+        const bool valid = n < n_hi;
+        const long long t = (long long)f * p.G + (valid ? n : n_lo);
+        float x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = 0.f;
+        if (on && valid) unpack8f(__ldg(reinterpret_cast<const uint4*>(p.x + ((long long)b * p.T + t) * p.x_ts + (long long)h * p.D + c0)), x);
+        float da = 0.f, db = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { da = fmaf(wa[i], x[i], da); db = fmaf(wb[i], x[i], db); }
+        da = group16_sum(da);
+        db = group16_sum(db);
+        acc += da;                                             // da = 0 for a tail group (x = 0)
+        if (l == 0 && valid) p.beta_out[(long long)bh * p.T + t] = 1.f / (1.f + __expf(-(db + bb)));      // Eq. 15
+    }
+    if (l == 0) s_sum[g] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float tot = 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) tot += s_sum[i];
+        p.part[(long long)bhf * p.NSPL + s] = tot;
+        __threadfence();
+        s_last = atomicAdd(p.counters + bhf, 1u) == (unsigned int)(p.NSPL - 1) ? 1u : 0u;
+        if (s_last) {
+            __threadfence();
+            float sum = 0.f;
+            for (int i = 0; i < p.NSPL; ++i) sum += __ldcg(p.part + (long long)bhf * p.NSPL + i);
+            const float pre = sum / (float)p.G + __ldg(p.b_alpha + h);                           // W_alpha . x_bar + b_alpha (Eq. 13-14)
+            const float delta = fmaxf(pre, 0.f) + log1pf(__expf(-fabsf(pre)));                   // softplus
+            const float la = -__expf(__ldg(p.a_log + h)) * delta;
+            p.alpha_out[(long long)bh * p.F + f] = p.log_alpha ? la : __expf(la);
+            p.counters[bhf] = 0u;
+        }
+    }
+}
+
+}  // namespace fe
+}  // namespace gdn

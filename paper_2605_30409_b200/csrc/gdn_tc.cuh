@@ -61,10 +61,15 @@ struct TcPlan {
     CUtensorMap tmQr, tmKr;
 };
 
-struct NormArgs {                                  // the extra operands of gdn_forward_chunk_norm
+struct NormArgs {                                  // the extra operands of gdn_forward_chunk_norm / gdn_forward_chunk_full
     const void *q_raw, *k_raw;
     const float* z_in;
     float* z_out;
+    const void* gate = nullptr;                    // output gate G_f (Eq. 23) or NULL
+    long long g_ts = 0;
+    // gdn_forward_chunk_full: the four feature tensors are the plan's own dense buffers, whatever strides the plan's
+    // config gives for the caller's q / k
+    bool dense_qk = false;
 };
 
 inline int tc_default_chunk(const gdn_config_t& c) { return c.chunk ? c.chunk : 128; }
@@ -486,8 +491,9 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
     if (q != tp.cq || k != tp.ck || v != tp.cv) {
         const int Gm = (tp.mode == GDN_PATH_TC_FRAME) ? c.group : c.T;      // token-wise: one "frame" of T tokens
         const int rows = tp.tile64 ? 64 : 128;
-        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, Gm, ts(c.q_token_stride, c.d_k), rows, err) &&
-                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, Gm, ts(c.k_token_stride, c.d_k), rows, err) &&
+        const bool dense = na && na->dense_qk;         // the plan's own feature buffers (gdn_forward_chunk_full)
+        bool ok = tc::make_act_tmap(&tp.tmQ, q, c.B, c.T, c.H, c.d_k, Gm, ts(dense ? 0 : c.q_token_stride, c.d_k), rows, err) &&
+                  tc::make_act_tmap(&tp.tmK, k, c.B, c.T, c.H, c.d_k, Gm, ts(dense ? 0 : c.k_token_stride, c.d_k), rows, err) &&
                   tc::make_act_tmap(&tp.tmV, v, c.B, c.T, c.H, c.d_v, Gm, ts(c.v_token_stride, c.d_v), rows, err);
         if (!ok) { tp.cq = tp.ck = tp.cv = nullptr; return GDN_ERR_CUDA; }
         tp.cq = q; tp.ck = k; tp.cv = v;
@@ -516,8 +522,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             // until the division in Phase C, so it runs beside it on its own stream and workspace.
             TcPlan& zt = *tp.zplan;
             if (na->q_raw != tp.cqr || na->k_raw != tp.ckr) {
-                bool ok = tc::make_act_tmap(&tp.tmQr, na->q_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.q_token_stride, c.d_k), 128, err) &&
-                          tc::make_act_tmap(&tp.tmKr, na->k_raw, c.B, c.T, c.H, c.d_k, c.group, ts(c.k_token_stride, c.d_k), 128, err);
+                bool ok = tc::make_act_tmap(&tp.tmQr, na->q_raw, c.B, c.T, c.H, c.d_k, c.group, ts(na->dense_qk ? 0 : c.q_token_stride, c.d_k), 128, err) &&
+                          tc::make_act_tmap(&tp.tmKr, na->k_raw, c.B, c.T, c.H, c.d_k, c.group, ts(na->dense_qk ? 0 : c.k_token_stride, c.d_k), 128, err);
                 if (!ok) { tp.cqr = tp.ckr = nullptr; return GDN_ERR_CUDA; }
                 tp.cqr = na->q_raw; tp.ckr = na->k_raw;
             }
@@ -537,6 +543,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
             if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             fp.den = tp.den; fp.den_mode = 2; fp.eps = c.eps;
+            fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
             den_ready = tp.zev1;
         }
         e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready)

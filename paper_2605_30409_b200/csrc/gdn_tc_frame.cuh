@@ -46,6 +46,11 @@ struct FrmParams {
     float* den;                  // [B][T][H] fp32: q_raw . z_f per token
     int den_mode;                // readout: 0 = plain, 1 = write den (column 0 of Q_raw S^z), 2 = out = scale Q S / (den + eps)
     float eps;
+    // output gate (Eq. 23, the Hadamard product G (.) Y): multiplied in the readout's epilogue, before the
+    // bf16 rounding of the tile.  gate [B][T][H][dr] bf16, token stride g_ts; NULL = no gate.
+    const __nv_bfloat16* gate;
+    long long g_ts;
+    int dr;                      // real head dim (112 when padded to D = 128): channels >= dr are clipped by the store
 };
 
 namespace frm {
@@ -464,6 +469,8 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const long long tok = ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.H + (bh % p.H);   // index into den [B][T][H]
             float mul = p.scale;
             if (p.den_mode == 2 && n < p.G) mul = p.scale / (__ldg(p.den + tok) + p.eps);          // Eq. 22: eps after the dot product, no clamp
+            const __nv_bfloat16* grow = (p.gate && n < p.G)
+                ? p.gate + ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.g_ts + (long long)(bh % p.H) * p.dr : nullptr;
             if (p.den_mode == 1) {
                 // z pass: only column 0 of Q_raw S^z is the normaliser q_raw . z_f; nothing goes to `out`
                 mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
@@ -492,10 +499,20 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     if (lane == 0) mbar_arrive(&acc_empty[a]);
                 }
 #pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4)
+                for (int q4 = 0; q4 < 4; ++q4) {
+                    float m[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) m[e] = mul;
+                    if (grow && cc * 32 + q4 * 8 < p.dr) {
+                        float gv[8];
+                        unpack8(__ldg(reinterpret_cast<const uint4*>(grow + cc * 32 + q4 * 8)), gv);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) m[e] *= gv[e];
+                    }
                     st_shared_v4(stg + swz_chunk_off(row, cc * 4 + q4, kBlk),
-                                 pack_bf16(mul * v[8 * q4], mul * v[8 * q4 + 1]), pack_bf16(mul * v[8 * q4 + 2], mul * v[8 * q4 + 3]),
-                                 pack_bf16(mul * v[8 * q4 + 4], mul * v[8 * q4 + 5]), pack_bf16(mul * v[8 * q4 + 6], mul * v[8 * q4 + 7]));
+                                 pack_bf16(m[0] * v[8 * q4], m[1] * v[8 * q4 + 1]), pack_bf16(m[2] * v[8 * q4 + 2], m[3] * v[8 * q4 + 3]),
+                                 pack_bf16(m[4] * v[8 * q4 + 4], m[5] * v[8 * q4 + 5]), pack_bf16(m[6] * v[8 * q4 + 6], m[7] * v[8 * q4 + 7]));
+                }
             }
             fence_proxy_async();
             asm volatile("bar.sync 1, 128;" ::: "memory");

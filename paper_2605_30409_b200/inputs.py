@@ -123,6 +123,41 @@ def make_normalizer_inputs(wl: GdnWorkload, seed: Optional[int] = None) -> GdnIn
     return inp
 
 
+def make_frontend_inputs(wl: GdnWorkload, seed: Optional[int] = None, grid_w: int = 40) -> dict:
+    """Seeded operands of the block's front end (App. G.2-G.3, Alg. 1): a packed qkv tensor
+    [B,T,3,H,D] of raw projections, the per-head latent features x [B,T,H,D], RMSNorm weights, rotation tables
+    for a (frame, row, column) position with three frequency bands, gate parameters, an evaluated output gate.
+    Only random draws and table look-ups: none of the method's arithmetic."""
+    g = torch.Generator(device="cpu")
+    g.manual_seed(int(wl.seed if seed is None else seed))
+    B, H, T, D, G = wl.B, wl.H, wl.T, wl.d_k, wl.group
+    dt = wl.dtype
+    qkv = torch.randn(B, T, 3, H, D, generator=g, dtype=torch.float32).to(dt).contiguous()
+    x = torch.randn(B, T, H, D, generator=g, dtype=torch.float32).to(dt).contiguous()
+    w_q = 0.5 + torch.rand(H, D, generator=g, dtype=torch.float32)
+    w_k = 0.5 + torch.rand(H, D, generator=g, dtype=torch.float32)
+    # position of token t: frame t // G, row (t % G) // grid_w, column (t % G) % grid_w; pair i belongs to one of three bands
+    t = torch.arange(T)
+    pos = torch.stack([t // G, (t % G) // grid_w, (t % G) % grid_w], dim=1).to(torch.float32)        # [T, 3]
+    npair = D // 2
+    band = torch.arange(npair) % 3
+    freq = 1.0 / (10000.0 ** (torch.arange(npair, dtype=torch.float32) / npair))
+    ang = pos[:, band] * freq[None, :]
+    out = {
+        "qkv": qkv, "x": x, "w_q": w_q.contiguous(), "w_k": w_k.contiguous(),
+        "cos": torch.cos(ang).contiguous(), "sin": torch.sin(ang).contiguous(),
+        "w_alpha": (torch.randn(H, D, generator=g) / math.sqrt(D)).contiguous(),
+        "b_alpha": torch.randn(H, generator=g).contiguous() - 2.0,
+        "a_log": (0.5 * torch.randn(H, generator=g)).contiguous(),
+        "w_beta": (torch.randn(H, D, generator=g) / math.sqrt(D)).contiguous(),
+        "b_beta": torch.randn(H, generator=g).contiguous(),
+        "gate": torch.nn.functional.silu(torch.randn(B, T, H, D, generator=g, dtype=torch.float32)).to(dt).contiguous(),
+        "state": (wl.state_std * torch.randn(B, H, D, D, generator=g, dtype=torch.float32)).contiguous(),
+        "z_in": (wl.state_std * torch.rand(B, H, D, generator=g, dtype=torch.float32)).contiguous(),
+    }
+    return out
+
+
 # --- BASELINE.json's five configs (mode T = literal; *_F = the paper's frame-wise semantics) -------
 def config(idx: int, *, T: Optional[int] = None, chunk: int = 0, frame: bool = False,
            chunk_index: int = 0) -> GdnWorkload:

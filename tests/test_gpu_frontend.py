@@ -1,0 +1,124 @@
+"""GPU parity of the block's front end against oracle/frontend.py (Eq. 12-15, 23, L554; Alg. 1 boundary):
+gdn_feature_map, gdn_compute_gates, gdn_forward_chunk_full.  All through the C ABI."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2605_30409_b200 as gdn
+from paper_2605_30409_b200 import inputs as gin
+from tests.gpu_util import rel_err
+
+pytestmark = pytest.mark.gpu
+TOL_BF16 = 2e-2
+DEV = "cuda:0"
+
+
+def _packed_views(fi):
+    qkv = fi["qkv"]
+    return qkv[:, :, 0], qkv[:, :, 1], qkv[:, :, 2]
+
+
+def _plan(B, H, T, D, G, flags, packed=True):
+    kw = {}
+    if packed:
+        kw = dict(q_token_stride=3 * H * D, k_token_stride=3 * H * D, v_token_stride=3 * H * D)
+    return gdn.GdnPlan(B=B, H=H, T=T, d_k=D, d_v=D, group=G, flags=flags, **kw)
+
+
+@pytest.mark.parametrize("D,G,F,H", [(112, 880, 3, 20), (128, 352, 2, 4), (64, 200, 3, 3)])
+def test_feature_map_matches_oracle(D, G, F, H):
+    from oracle import frontend as fe
+    B, T = 2 if D != 112 else 1, G * F
+    wl = gin.GdnWorkload("fm", B, H, T, D, D, group=G, seed=300 + D)
+    fi = gin.make_frontend_inputs(wl)
+    qkv = fi["qkv"].to(DEV)
+    q_d, k_d = qkv[:, :, 0], qkv[:, :, 1]
+    outs = [torch.empty(B, T, H, D, device=DEV, dtype=torch.bfloat16) for _ in range(4)]
+    with _plan(B, H, T, D, G, gdn.GDN_FLAG_NORMALIZER) as p:
+        fm = gdn.make_featmap_args(q_d, k_d, fi["w_q"].to(DEV), fi["w_k"].to(DEV), fi["cos"].to(DEV), fi["sin"].to(DEV), 1e-6)
+        wq, wk, cs, sn = (fi[n].to(DEV) for n in ("w_q", "w_k", "cos", "sin"))
+        fm = gdn.make_featmap_args(q_d, k_d, wq, wk, cs, sn, 1e-6)
+        p.feature_map(fm, *outs)
+        torch.cuda.synchronize()
+    q, k, _ = _packed_views(fi)
+    ref = fe.feature_map(q, k, fi["w_q"], fi["w_k"], fi["cos"], fi["sin"], group=G, eps_rms=1e-6)
+    for name, got, want in zip(("q_rot", "k_rot", "q_raw", "k_raw"), outs, ref):
+        err = np.abs(got.cpu().double().numpy() - want).max() / np.abs(want).max()
+        assert err <= 2 ** -8, f"{name}: {err:.3e}"          # one bf16 rounding of an fp32 evaluation
+    assert (outs[2].cpu().float() >= 0).all() and (outs[3].cpu().float() >= 0).all()
+
+
+@pytest.mark.parametrize("log_alpha", [False, True])
+@pytest.mark.parametrize("D,G,F,H,B", [(112, 880, 3, 20, 1), (64, 3520, 1, 2, 1), (128, 100, 4, 3, 2)])
+def test_gates_match_oracle_and_are_deterministic(D, G, F, H, B, log_alpha):
+    from oracle import frontend as fe
+    T = G * F
+    wl = gin.GdnWorkload("gates", B, H, T, D, D, group=G, seed=400 + D)
+    fi = gin.make_frontend_inputs(wl)
+    dev = {n: fi[n].to(DEV) for n in ("x", "w_alpha", "b_alpha", "a_log", "w_beta", "b_beta")}
+    flags = gdn.GDN_FLAG_NORMALIZER | (gdn.GDN_FLAG_LOG_ALPHA if log_alpha else 0)
+    res = []
+    with _plan(B, H, T, D, G, flags, packed=False) as p:
+        ga = gdn.make_gate_args(dev["x"], dev["w_alpha"], dev["b_alpha"], dev["a_log"], dev["w_beta"], dev["b_beta"])
+        for _ in range(2):
+            a = torch.full((B, H, F), float("nan"), device=DEV)
+            b = torch.full((B, H, T), float("nan"), device=DEV)
+            p.compute_gates(ga, a, b)
+            torch.cuda.synchronize()
+            res.append((a.cpu(), b.cpu()))
+    assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])      # fixed summation order
+    alpha, la, beta = fe.gates(fi["x"], fi["w_alpha"], fi["b_alpha"], fi["a_log"], fi["w_beta"], fi["b_beta"], group=G)
+    want_a = la if log_alpha else alpha
+    np.testing.assert_allclose(res[0][0].double().numpy(), want_a, rtol=2e-5, atol=2e-6)
+    np.testing.assert_allclose(res[0][1].double().numpy(), beta, rtol=2e-5, atol=2e-6)
+
+
+def _full_reference(fi, wl, G, use_gates, alpha, beta, bidir, gate):
+    import oracle
+    from oracle import frontend as fe
+    q, k, v = _packed_views(fi)
+    q_rot, k_rot, q_raw, k_raw = fe.feature_map(q, k, fi["w_q"], fi["w_k"], fi["cos"], fi["sin"], group=G, eps_rms=1e-6)
+    if use_gates:
+        alpha, _, beta = fe.gates(fi["x"], fi["w_alpha"], fi["b_alpha"], fi["a_log"], fi["w_beta"], fi["b_beta"], group=G)
+    o, S, z = oracle.gdn_forward(q_rot, k_rot, v, alpha, beta, fi["state"], group=G, q_raw=q_raw, k_raw=k_raw, z_in=fi["z_in"],
+                                 normalizer=True, bidir=bidir)
+    if gate:
+        o = fe.output_gate(o, fi["gate"])
+    return o, S, z
+
+
+@pytest.mark.parametrize("D,G,F,H,bidir,use_gates,gate", [
+    (112, 880, 3, 20, True, True, True),          # the paper's production chunk, its full operator (Alg. 1)
+    (128, 352, 2, 4, False, False, True),
+    (64, 200, 3, 3, True, True, False),
+])
+def test_forward_full_matches_oracle(D, G, F, H, bidir, use_gates, gate):
+    B, T = 1, G * F
+    wl = gin.GdnWorkload("full", B, H, T, D, D, group=G, seed=500 + D)
+    fi = gin.make_frontend_inputs(wl)
+    g = torch.Generator().manual_seed(7)
+    alpha = torch.sigmoid(3 + torch.randn(B, H, F, generator=g))
+    beta = torch.sigmoid(torch.randn(B, H, T, generator=g))
+    qkv = fi["qkv"].to(DEV)
+    dv = {n: fi[n].to(DEV) for n in ("x", "w_q", "w_k", "cos", "sin", "w_alpha", "b_alpha", "a_log", "w_beta", "b_beta", "gate")}
+    S = fi["state"].to(DEV)
+    z = fi["z_in"].to(DEV)
+    out = torch.empty(B, T, H, D, device=DEV, dtype=torch.bfloat16)
+    flags = gdn.GDN_FLAG_NORMALIZER | (gdn.GDN_FLAG_BIDIR if bidir else 0)
+    with _plan(B, H, T, D, G, flags) as p:
+        fm = gdn.make_featmap_args(qkv[:, :, 0], qkv[:, :, 1], dv["w_q"], dv["w_k"], dv["cos"], dv["sin"], 1e-6)
+        ga = gdn.make_gate_args(dv["x"], dv["w_alpha"], dv["b_alpha"], dv["a_log"], dv["w_beta"], dv["b_beta"]) if use_gates else None
+        p.forward_full(fm, qkv[:, :, 2], ga, None if use_gates else alpha.to(DEV), None if use_gates else beta.to(DEV),
+                       dv["gate"] if gate else None, S, z, out, S, z)
+        torch.cuda.synchronize()
+    o_ref, S_ref, z_ref = _full_reference(fi, wl, G, use_gates, alpha, beta, bidir, gate)
+    eo, es, ez = rel_err(out.cpu(), o_ref), rel_err(S.cpu(), S_ref), rel_err(z.cpu(), z_ref)
+    print(f"full D={D} G={G} F={F} bidir={bidir} gates={use_gates} gate={gate}: err_o={eo:.2e} err_S={es:.2e} err_z={ez:.2e}")
+    assert eo <= TOL_BF16 and es <= TOL_BF16 and ez <= TOL_BF16
+
+
+def test_front_end_rejects_unsupported_plans():
+    with gdn.GdnPlan(B=1, H=2, T=256, d_k=64, d_v=64, group=1) as p:         # token-wise: no full operator
+        with pytest.raises(gdn.GdnError) as ei:
+            p.forward_full(gdn.make_featmap_args(0, 0, 0, 0, 0, 0), 0, None, 0, 0, None, None, None, 0, 0, 0)
+        assert ei.value.status == gdn.GDN_ERR_UNSUPPORTED
