@@ -53,8 +53,24 @@ def flops_per_call(wl, chunk):
     th = wl.B * wl.H * wl.T
     if wl.group == 1:
         C = chunk or 64
-        return th * (6 * d * d + 10 * C * d)
+        return th * (6 * d * d + 10 * C * d)           # depends on the compute tile C: see flops_report for the C = 64 figure
     return th * 6 * d * d + wl.B * wl.H * (wl.T // wl.group) * 2 * d ** 3
+
+
+def flops_report(wl, chunk, ms_per_step, by, pk):
+    """TFLOP/s and % of the bf16 peak with BOTH flop formulas of SURVEY 8d (the token-wise count grows with the compute
+    tile C the implementation picks, so the C = 64 figure is the one that compares across implementations), and the
+    HBM-limited cap of each: flops / algorithmic bytes x measured HBM peak, as % of the measured bf16 peak."""
+    out = {}
+    for tag, C in (("c_in_use", chunk or 64), ("c64", 64)):
+        fl = flops_per_call(wl, C)
+        tf = fl / (ms_per_step * 1e-3) / 1e12
+        out[tag] = {"C": C if wl.group == 1 else None, "gflop_per_call": fl / 1e9, "tflops": tf,
+                    "pct_bf16_peak": 100 * tf / pk["bf16_tflops"],
+                    "hbm_limited_cap_pct_bf16_peak": 100 * (fl / by) * pk["hbm_gbs"] * 1e9 / 1e12 / pk["bf16_tflops"]}
+        if wl.group != 1:
+            break
+    return out
 
 
 def bytes_per_call(wl):
@@ -269,7 +285,6 @@ def run_ours(args):
     e1.record(stream)
     barrier()
     ms = max_over_ranks(e0.elapsed_time(e1), dist, dev)
-    clocks = sampler.stop()
     assert torch.isfinite(state).all(), "state diverged"
     ms_per_step = ms / args.steps
     tokens_per_s = job_tokens_per_s(world, wl, args.steps, ms)
@@ -299,6 +314,7 @@ def run_ours(args):
                "h2d_bytes_per_step": nbytes(hq, hk, hv, ha, hb, hs), "d2h_bytes_per_step": nbytes(hout, hs),
                "steps": k_e2e, "ms_per_step": ms_e / k_e2e}
 
+    clocks = sampler.stop()                        # sampled from before the warm-up to the end of the e2e leg
     pk, pk_src = peaks()
     fl = flops_per_call(wl, info.chunk)
     by = bytes_per_call(wl)
@@ -314,6 +330,7 @@ def run_ours(args):
         "config": config_dict(wl, (gdn.PATH_NAMES[info.path], info.chunk, info.launches_per_call),
                               {"l2": f"rotating {n_sets} input sets ({n_sets * set_bytes / 1e6:.0f} MB > 126 MB L2), carried state"}),
         "tflops": tflops, "pct_bf16_peak": 100 * tflops / pk["bf16_tflops"], "peaks": pk_src,
+        "flops": flops_report(wl, info.chunk, ms_per_step, by, pk),
         "hbm_gbs_algorithmic": by / (ms_per_step * 1e-3) / 1e9,
         "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * info.launches_per_call,
         "roofline": roof, "kernels": kernels,
@@ -385,6 +402,7 @@ def kernel_bytes(name, wl, by_call):
     st = wl.B * wl.H * wl.d_k * wl.d_v * 4
     table = {
         "gdn_tok_prepass": th * ((2 * wl.d_k + wl.d_v) * es + 8),
+        "gdn_tok_tile64": th * ((2 * wl.d_k + wl.d_v) * es + 8),
         "gdn_tok_output": th * wl.d_v * es,
         "gdn_tok_chain": 2 * st,
         "gdn_frm_summaries": th * ((wl.d_k + wl.d_v) * es + 4),
@@ -403,7 +421,10 @@ def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
         dur_ms, name = top["avg_us"] * 1e-3, top["name"]
         kb = kernel_bytes(name, wl, by)
     achieved = kb / (dur_ms * 1e-3) / 1e9
-    return {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
+    # what the measurements say limits the kernel: below half of the HBM roofline (and, for the token path, with the
+    # tensor pipe at 10-20 % in the ncu captures) the dominant kernel is bound by the latency of its dependent steps
+    limiter = "hbm" if achieved / pk["hbm_gbs"] >= 0.5 else "latency (dependent MMA round trips / per-SM TMA rate; see DESIGN.md section 7)"
+    return {"bound": "hbm", "observed_limiter": limiter, "kernel": name, "achieved": achieved, "peak": pk["hbm_gbs"], "unit": "GB/s",
             "frac": achieved / pk["hbm_gbs"], "traffic": ncu_traffic(name, wl), "peak_source": pk_src,
             "algorithmic_bytes": kb, "kernel_avg_us": dur_ms * 1e3, "ncu": ncu_counters(name, wl),
             "whole_call": {"algorithmic_bytes": by, "achieved": by / (ms_per_step * 1e-3) / 1e9,

@@ -671,3 +671,50 @@ def test_config5_frame_T65536_all_streams():
         for h in range(h0, h1):
             eo, es = rel_err(out[b, :, h], o_ref[:, h - h0]), rel_err(S[b, h], S_ref[h - h0])
             assert eo <= TOL_BF16 and es <= TOL_BF16, f"stream {(b, h)}: err_o={eo:.3e} err_S={es:.3e}"
+
+
+# =====================================================================================================
+# d = 64, C = 64: light 64-token tile workers (gdn_tc_tile64.cuh) and the single persistent kernel with the
+# two-level, segment-parallel scan (gdn_tc_fused64.cuh, Eq. 5)
+# =====================================================================================================
+@pytest.mark.parametrize("T", [64, 200, 704, 3520])
+def test_tile64_three_kernel_path(T):
+    """GDN_FLAG_UNFUSED + chunk 64 at d = 64: gdn_tok_tile64 feeds the chain and output kernels."""
+    wl = gin.GdnWorkload("tile64u", 2, 3, T, 64, 64, seed=900 + T, chunk=64)
+    eo, es, info = check(gin.make_inputs(wl), flags=gdn.GDN_FLAG_UNFUSED)
+    assert info == (1, 64, 3)
+
+
+@pytest.mark.parametrize("B,H,T", [(1, 16, 3520), (2, 32, 704), (1, 2, 8192), (1, 1, 130), (3, 5, 64)])
+def test_fused64_two_level_scan(B, H, T):
+    """One launch; the number of segments per stream follows the stream count (64 streams: plain scan, NS = 1;
+    few streams: NS up to 4), so the shapes cover segment 0, the identity-started segments, level 2 and short tails."""
+    wl = gin.GdnWorkload("fused64", B, H, T, 64, 64, seed=950 + T + H, chunk=64)
+    eo, es, info = check(gin.make_inputs(wl))
+    assert info == (1, 64, 1)
+    print(f"fused64 B={B} H={H} T={T}: err_o={eo:.2e} err_S={es:.2e}")
+
+
+def test_fused64_stream_with_carried_state_and_rerun_is_bit_identical():
+    """Carried state over four calls on one plan (epoch-stamped flags are never reset), log-alpha input, and the same
+    bits on a second pass over the same inputs (fixed reduction orders: DESIGN.md reading 17)."""
+    B, H, T = 1, 4, 1000
+    dev = torch.device("cuda:0")
+    runs = []
+    for rep in range(2):
+        with gdn.GdnPlan(B=B, H=H, T=T, d_k=64, d_v=64, group=1, chunk=64, flags=gdn.GDN_FLAG_LOG_ALPHA) as p:
+            S = torch.zeros(B, H, 64, 64, device=dev)
+            S_ref = None
+            outs = []
+            for ci in range(4):
+                inp = gin.make_inputs(gin.GdnWorkload("f64s", B, H, T, 64, 64, seed=970 + ci, chunk=64), with_state=False)
+                out = torch.empty(B, T, H, 64, device=dev, dtype=torch.bfloat16)
+                p.forward(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), torch.log(inp.alpha).to(dev), inp.beta.to(dev), S, out, S)
+                torch.cuda.synchronize()
+                outs.append(out.cpu())
+                if rep == 0:
+                    import oracle
+                    o_ref, S_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, S_ref, group=1)
+                    assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S.cpu(), S_ref) <= TOL_BF16
+            runs.append((outs, S.cpu()))
+    assert all(torch.equal(a, b) for a, b in zip(runs[0][0], runs[1][0])) and torch.equal(runs[0][1], runs[1][1])
