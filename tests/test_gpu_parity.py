@@ -718,3 +718,28 @@ def test_fused64_stream_with_carried_state_and_rerun_is_bit_identical():
                     assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S.cpu(), S_ref) <= TOL_BF16
             runs.append((outs, S.cpu()))
     assert all(torch.equal(a, b) for a, b in zip(runs[0][0], runs[1][0])) and torch.equal(runs[0][1], runs[1][1])
+
+
+def test_host_entry_point_pipelined_across_calls():
+    """Five unsegmented host calls issued back to back WITHOUT synchronising in between, each with its own inputs and
+    output buffer, the state carried through ONE host buffer (state_out of call i is state_in of call i + 1): the
+    double-buffered input staging and the stream-ordered state copies must give exactly what the device path gives."""
+    B, H, T, d = 1, 4, 1024, 64
+    dev = torch.device("cuda:0")
+    pin = lambda t: t.contiguous().pin_memory()
+    inps = [gin.make_inputs(gin.GdnWorkload("hostpipe", B, H, T, d, d, seed=80 + i), with_state=False) for i in range(5)]
+    host = [tuple(map(pin, (x.q, x.k, x.v, x.alpha, x.beta))) for x in inps]
+    outs = [torch.full((B, T, H, d), float("nan"), dtype=torch.bfloat16).pin_memory() for _ in inps]
+    hs = pin(0.02 * torch.randn(B, H, d, d, generator=torch.Generator().manual_seed(5)))
+    S0 = hs.clone()
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d) as p:
+        for (q, k, v, a, b), o in zip(host, outs):
+            p.forward_host(q, k, v, a, b, hs, o, hs)
+        torch.cuda.synchronize()
+        S = S0.to(dev)
+        for x, o in zip(inps, outs):
+            od = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+            p.forward(x.q.to(dev), x.k.to(dev), x.v.to(dev), x.alpha.to(dev), x.beta.to(dev), S, od, S)
+            torch.cuda.synchronize()
+            assert torch.equal(o, od.cpu())
+        assert torch.equal(hs, S.cpu())
