@@ -252,7 +252,8 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
     const size_t D = tp.D, BH = tp.BH, NT = tp.NT, NC = tp.NC;
     size_t off = 0;
     auto carve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 1024); return o; };
-    const size_t oG = carve(BH * NC * D * D * 2), oN = carve(BH * NC * D * D * 4), oGam = carve(BH * NC * 4);
+    const bool fused_plan = tc_default_chunk(c) == 128 && !(c.flags & GDN_FLAG_UNFUSED);
+    const size_t oG = carve(BH * NC * D * D * 2), oN = carve(BH * NC * D * D * (fused_plan ? 2 : 4)), oGam = carve(BH * NC * 4);
     const size_t oQt = carve(BH * NT * 128 * D * 2), oOl = carve(BH * NT * 128 * D * 2);
     tp.fused = tp.C == 128 && !(c.flags & GDN_FLAG_UNFUSED);
     const size_t oSc = tp.fused ? 0 : carve(BH * NC * D * D * 2);
@@ -315,7 +316,11 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         const uint32_t box[3] = {64, (uint32_t)D, 1};
         ok = ok && tc::make_tmap(&tp.tmScS, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
-    {   // N_c: fp32 (D, D, BH*NC), box {32, D, 1}
+    if (tp.fused) {   // N_c of the fused kernel: bf16 (D, D, BH*NC), box {64, D, 1} 
+        const uint64_t dims[3] = {D, D, BH * NC}, str[3] = {2, D * 2, D * D * 2};
+        const uint32_t box[3] = {64, (uint32_t)D, 1};
+        ok = ok && tc::make_tmap(&tp.tmN, tp.Nw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
+    } else {          // N_c: fp32 (D, D, BH*NC), box {32, D, 1}
         const uint64_t dims[3] = {D, D, BH * NC}, str[3] = {4, D * 4, D * D * 4};
         const uint32_t box[3] = {32, (uint32_t)D, 1};
         ok = ok && tc::make_tmap(&tp.tmN, tp.Nw, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);

@@ -54,7 +54,7 @@ template <int D>
 struct ChainSmem {
     static constexpr int NB = D / 64;
     static constexpr uint32_t G_BYTES = (uint32_t)D * D * 2;          // NB blocks of [D][64] bf16
-    static constexpr uint32_t N_BYTES = (uint32_t)D * 64 * 4;         // 2 blocks of [D][32] fp32 (this CTA's 64 state columns)
+    static constexpr uint32_t N_BYTES = (uint32_t)D * 64 * 2;         // one block of [D][64] bf16 (this CTA's 64 state columns)
     static constexpr uint32_t GN_BYTES = G_BYTES + N_BYTES;
     static constexpr uint32_t Q_BYTES = 128u * D * 2;                 // NB blocks of [128][64] bf16; block 0 then stages the out tile
     static constexpr uint32_t S_BYTES = (uint32_t)D * 128;            // [D][64] bf16
@@ -151,7 +151,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
 #pragma unroll
                             for (int nb = 0; nb < NB; ++nb) tma_prefetch_3d(tmG, nb * 64, 0, z);
                             tma_prefetch_3d(tmN, ct * 64, 0, z);
-                            tma_prefetch_3d(tmN, ct * 64 + 32, 0, z);
                         }
                     }
                     if (c >= ready) __nanosleep(32);
@@ -169,7 +168,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
 #pragma unroll
                         for (int nb = 0; nb < NB; ++nb) tma_load_3d(gb + nb * (D * 128), tmG, &g_full[gst], nb * 64, 0, z);
                         tma_load_3d(gb + L::G_BYTES, tmN, &g_full[gst], ct * 64, 0, z);
-                        tma_load_3d(gb + L::G_BYTES + D * 128, tmN, &g_full[gst], ct * 64 + 32, 0, z);
                     } else {
                         const int qst = gs % QST;
                         if (gs >= (uint32_t)QST) mbar_wait(&q_empty[qst], ((gs / QST) - 1) & 1u);
@@ -270,14 +268,13 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
                 const float gamma_c = lds_f32(smem_u32(sGamma) + gst * 4);
                 {   // state-independent half, while the MMA runs: S <- gamma_c S + N_c
-                    const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES + half * (D * 128));
+                    const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES);
 #pragma unroll
-                    for (int ch = 0; ch < 8; ++ch) {
-                        const uint4 uu = ld_shared_v4(nbase + swz_chunk_off(mm, ch, 0));
-                        S[4 * ch + 0] = fmaf(gamma_c, S[4 * ch + 0], __uint_as_float(uu.x));
-                        S[4 * ch + 1] = fmaf(gamma_c, S[4 * ch + 1], __uint_as_float(uu.y));
-                        S[4 * ch + 2] = fmaf(gamma_c, S[4 * ch + 2], __uint_as_float(uu.z));
-                        S[4 * ch + 3] = fmaf(gamma_c, S[4 * ch + 3], __uint_as_float(uu.w));
+                    for (int ch = 0; ch < 4; ++ch) {
+                        float f[8];
+                        unpack8(ld_shared_v4(nbase + swz_chunk_off(mm, half * 4 + ch, 0)), f);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) S[8 * ch + e] = fmaf(gamma_c, S[8 * ch + e], f[e]);
                     }
                 }
                 __syncwarp();

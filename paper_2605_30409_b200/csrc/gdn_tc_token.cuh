@@ -621,6 +621,7 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         }
     };
     //   [N | G] at `acc` (lane = summary row m) -> G bf16 as [D][64] blocks at gdst, N fp32 as [D][32] blocks at ndst
+    //   (FUSED: N in bf16 as well, [D][64] blocks like G: half the summary traffic; the chain adds it to its fp32 state)
     auto stage_NG = [&](uint32_t acc, uint32_t gdst, uint32_t ndst) {
 #pragma unroll
         for (int cc = 0; cc < D / 32; ++cc) {
@@ -628,11 +629,15 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
             tmem_ldw2(tmem_addr(acc, lane_base, cc * 32 + cb), tmem_addr(acc, lane_base, D + cc * 32 + cb), nv, gv);
             if (m_ok) {
                 store_roww_bf16(gdst, SBLK, m, cc * 32 + cb, gv);
+                if (FUSED) {
+                    store_roww_bf16(ndst, SBLK, m, cc * 32 + cb, nv);
+                } else {
 #pragma unroll
-                for (int q4 = 0; q4 < CW / 4; ++q4) {
-                    const uint32_t noff = cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4);
-                    st_shared_v4(ndst + noff, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
-                                 __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
+                    for (int q4 = 0; q4 < CW / 4; ++q4) {
+                        const uint32_t noff = cc * SBLK + (uint32_t)m * 128u + (uint32_t)((((cb >> 2) + q4) ^ (m & 7)) << 4);
+                        st_shared_v4(ndst + noff, __float_as_uint(nv[4 * q4]), __float_as_uint(nv[4 * q4 + 1]),
+                                     __float_as_uint(nv[4 * q4 + 2]), __float_as_uint(nv[4 * q4 + 3]));
+                    }
                 }
             }
         }
@@ -654,7 +659,12 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
 #pragma unroll
             for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmG, gsrc + nb * SBLK, nb * 64, 0, z);
         }
-        for (int j = j_lo; j < j_hi; ++j) tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
+        if (FUSED) {
+#pragma unroll
+            for (int nb = 0; nb < NB; ++nb) tma_store_3d(tmN, nsrc + nb * SBLK, nb * 64, 0, z);       // bf16 [D][64] blocks
+        } else {
+            for (int j = j_lo; j < j_hi; ++j) tma_store_3d(tmN, nsrc + j * SBLK, j * 32, 0, z);
+        }
     };
     auto publish_staging = [&]() { fence_proxy_async(); tc_fence_before(); __syncthreads(); };
 
@@ -703,14 +713,9 @@ __device__ __forceinline__ void prepass_tile(const PrepassCtx& cx, const CUtenso
         if (tid == 0) {
             if (!(FUSED && D == 128)) store_QO(sV);
             if (FUSED) tma_store_commit();         // group 1: Qt, Ol (sQ, sV); group 2: G, N (sA, sB, sC)
-            if (FUSED && D == 128) store_NG(sA, sB, tile, 0, 2);
-            else store_NG(sA, sB, tile);
+            store_NG(sA, sB, tile);                // FUSED: N is bf16 and fits sB (d = 128: 32 KB)
             tma_store_commit();
             if (!FUSED) tma_store_wait_read();     // FUSED: the next tile waits where it reuses the staging
-        }
-        if (FUSED && D == 128 && tid == kPrepassFlagTid) {      // N blocks 2, 3 (sC): awaited by this thread before it releases the flag
-            store_NG(sA, sB, tile, 2, 4, false);
-            tma_store_commit();
         }
     } else {
         // first half: drain [PUt | PW] (c2), send Qt / Ol off, then reuse c2 for the second chunk's [N | G]
