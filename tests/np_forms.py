@@ -105,3 +105,67 @@ def affine_chunk_summaries(k, v, alpha, beta, C):
         Ms.append(np.exp(Gam[-1]) * np.eye(dk) - Kt.T @ W)
         Ns.append(Kt.T @ Ut)
     return Ms, Ns
+
+
+def segment_scan(q, k, v, alpha, beta, S0, C, NS, scale=1.0):
+    """Two-level (segment-parallel) scan over the per-chunk affine maps (PAPER.md Eq. 5 L118: S_f = alpha_f P_f S_{f-1}
+    + A_f is affine in the state; the columns are independent, L419-L423), as gdn_tc_fused64.cuh runs it:
+      per chunk c (state-independent):  G_c = Kt^T W, N_c = Kt^T Ut, gamma_c, Qt_c = diag(gamma) Q - P W, Ol_c = P Ut;
+      the chunks are cut into NS segments; segment 0 is scanned from S0; every other segment k from the IDENTITY map:
+          Gacc <- gamma_c Gacc + gacc G_c - G_c Gacc,   B <- gamma_c B - G_c B + N_c,   gacc <- gamma_c gacc
+      (prefix map of chunk c: S_c = gacc_c S_k - Gacc_c S_k + B_c, recorded BEFORE chunk c is applied);
+      level 2: S_{k+1} = gseg_k S_k - Gseg_k S_k + Bseg_k;  outputs: O_c = scale (Qt_c S_c + Ol_c).
+    Returns (out, S_final).  Pins the associativity the kernel relies on against the token loop of the oracle."""
+    T, dk = k.shape
+    dv = v.shape[1]
+    chunks = []
+    for c0 in range(0, T, C):
+        sl = slice(c0, min(c0 + C, T))
+        Q, K, V, b = q[sl], k[sl], v[sl], beta[sl]
+        Gam = np.cumsum(np.log(alpha[sl]))
+        n = len(Gam)
+        D = np.exp(np.minimum(Gam[:, None] - Gam[None, :], 0.0))
+        L = np.tril(b[:, None] * D * (K @ K.T), -1)
+        Tm = np.linalg.inv(np.eye(n) + L)
+        W = Tm @ ((b * np.exp(Gam))[:, None] * K)
+        Ut = Tm @ (b[:, None] * V)
+        Kt = np.exp(Gam[-1] - Gam)[:, None] * K
+        P = np.tril(D) * (Q @ K.T)
+        chunks.append(dict(sl=sl, G=Kt.T @ W, N=Kt.T @ Ut, gamma=np.exp(Gam[-1]), Qt=np.exp(Gam)[:, None] * Q - P @ W, Ol=P @ Ut))
+    NC = len(chunks)
+    LSEG = -(-NC // NS)
+    segs = [list(range(s, min(s + LSEG, NC))) for s in range(0, NC, LSEG)]
+    # level 1: prefix maps of every chunk inside its segment (segment 0 directly on the state)
+    pre = [None] * NC
+    segmap = []
+    S = S0.copy()
+    for kseg, idx in enumerate(segs):
+        if kseg == 0:
+            for c in idx:
+                pre[c] = ("state", S.copy())
+                S = chunks[c]["gamma"] * S - chunks[c]["G"] @ S + chunks[c]["N"]
+            S1 = S
+            continue
+        Gacc, B, gacc = np.zeros((dk, dk)), np.zeros((dk, dv)), 1.0
+        for c in idx:
+            pre[c] = ("map", gacc, Gacc.copy(), B.copy())
+            g, G, N = chunks[c]["gamma"], chunks[c]["G"], chunks[c]["N"]
+            Gacc, B, gacc = g * Gacc + gacc * G - G @ Gacc, g * B - G @ B + N, g * gacc
+        segmap.append((gacc, Gacc, B))
+    # level 2: the segment maps in order
+    S_seg = [None, S1] if len(segs) > 1 else [None]
+    Sk = S1 if len(segs) > 1 else S
+    for gacc, Gacc, B in segmap:
+        Sk = gacc * Sk - Gacc @ Sk + B
+        S_seg.append(Sk)
+    # parallel fix-up and outputs
+    out = np.zeros((T, dv))
+    for kseg, idx in enumerate(segs):
+        for c in idx:
+            if pre[c][0] == "state":
+                Sc = pre[c][1]
+            else:
+                _, gacc, Gacc, B = pre[c]
+                Sc = gacc * S_seg[kseg] - Gacc @ S_seg[kseg] + B
+            out[chunks[c]["sl"]] = scale * (chunks[c]["Qt"] @ Sc + chunks[c]["Ol"])
+    return out, (S_seg[-1] if len(segs) > 1 else S)

@@ -184,6 +184,20 @@ def test_affine_chunk_summaries_reproduce_state():
     np.testing.assert_allclose(S[0, 0], Sc, rtol=0, atol=1e-12)
 
 
+@pytest.mark.parametrize("C,NS,T", [(16, 1, 100), (16, 2, 100), (16, 4, 250), (8, 3, 64), (32, 4, 40)])
+def test_two_level_segment_scan_matches_token_loop(C, NS, T):
+    """SURVEY 8f NEXT-4 (Eq. 5): scanning segments from the identity map, composing the segment maps
+    and fixing the outputs up afterwards gives the token loop (associativity of the affine maps), including a ragged
+    last chunk, a shorter last segment and fewer chunks than segments."""
+    dk, dv = 12, 10
+    q, k, v, a, b, S0 = make(40 + NS, T, dk, dv, amin=0.1)
+    out, S = oracle.gdn_forward(q, k, v, a, b, S0, scale=0.7)
+    o2, S2 = np_forms.segment_scan(stream(q), stream(k), stream(v), a[0, 0].astype(np.float64), b[0, 0].astype(np.float64),
+                                   S0[0, 0], C, NS, scale=0.7)
+    np.testing.assert_allclose(out[0, :, 0], o2, rtol=0, atol=1e-12)
+    np.testing.assert_allclose(S[0, 0], S2, rtol=0, atol=1e-12)
+
+
 # ---- pin 10: joint linearity in (V, S_in) (L122) -------------------------------------------------
 @pytest.mark.parametrize("G", [1, 8])
 def test_linearity_in_v_and_state(G):
