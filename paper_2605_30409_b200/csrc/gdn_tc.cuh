@@ -191,10 +191,13 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
     // segments: chain CTAs (2 NS - 1 per stream) may take up to a quarter of the 4-per-SM CTA slots
     int NS = 1;
     while (NS < 4 && (NS + 1) * 2 <= NC && BH * (2 * (NS + 1) - 1) <= sms) ++NS;
-    const int LSEG = (NC + NS - 1) / NS;
-    NS = (NC + LSEG - 1) / LSEG;
+    // segment 0 (scanned by the CTA that also runs level 2) is about three chunks longer than the others
+    int L1 = NS > 1 ? (NC - 3 + NS - 1) / NS : NC;
+    if (L1 < 1) L1 = 1;
+    int L0 = NS > 1 ? NC - (NS - 1) * L1 : NC;
+    if (L0 < L1) { L1 = (NC + NS - 1) / NS; L0 = L1; NS = (NC + L1 - 1) / L1; }
     F64Params& f = tp.f64;
-    f.NS = NS; f.LSEG = LSEG; f.NCH = BH * (1 + 2 * (NS - 1));
+    f.NS = NS; f.L0 = L0; f.L1 = L1; f.NCH = BH * (1 + 2 * (NS - 1));
     const size_t nchunk = (size_t)BH * NC, nseg = (size_t)BH * NS;
     f.zG = 0; f.zN = (int)nchunk; f.zSc = (int)(2 * nchunk); f.zGA = (int)(3 * nchunk);
     f.zGs = (int)(4 * nchunk); f.zBs = (int)(4 * nchunk + nseg); f.zSk = (int)(4 * nchunk + 2 * nseg);
@@ -219,7 +222,7 @@ inline gdn_status_t tc_plan_init_fused64(TcPlan& tp, const gdn_config_t& c, int 
         if (err) *err = "flag initialisation failed";
         return GDN_ERR_CUDA;
     }
-    f.n_tile_tasks = LSEG * NS * BH; f.n_out_tasks = LSEG * NS * BH;
+    f.n_tile_tasks = L0 * NS * BH; f.n_out_tasks = L0 * NS * BH;
     long long grid = (long long)f.NCH + f.n_tile_tasks;
     if (grid > 4LL * sms) grid = 4LL * sms;
     if (grid < f.NCH + 1) grid = f.NCH + 1;

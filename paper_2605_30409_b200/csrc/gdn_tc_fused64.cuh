@@ -31,9 +31,14 @@
 
 namespace gdn {
 
+struct F64Params;
+__host__ __device__ inline int f64_seg_lo(int L0, int L1, int k) { return k == 0 ? 0 : L0 + (k - 1) * L1; }
+
 struct F64Params {
     TokParams t;                 // alpha, beta, S_in, S_out, out, B, H, T, NC (chunks of 64 per stream), scale, log_alpha
-    int NS, LSEG;                // segments per stream, chunks per segment (the last segment may be shorter)
+    int NS, L0, L1;              // segments per stream; segment 0 has L0 chunks, the others L1 <= L0 (the last one may be
+                                 // shorter): segment 0 is longer by about the latency of publishing a segment map, so that the
+                                 // maps of the other segments are waiting when its scan arrives at level 2
     int NCH;                     // chain CTAs = BH * (1 + 2 (NS - 1))
     int zG, zN, zSc, zGA, zGs, zBs, zSk;   // first [64][64] bf16 slot of each array in the 3-D workspace map
     long long rQt, rOl;          // first row of Qt / Ol in the 2-D workspace map
@@ -50,10 +55,6 @@ struct F64Params {
 
 namespace f64 {
 
-// Chain CTAs release their snapshot flags all at once when they are done (false) or per step, trailing by three steps
-// (true).  A gpu-scope release per step sits on a state warp: per-step release measured 55.4 us, at-the-end 49.5 us (config 2).
-constexpr int kReleaseBatch = 1 << 20;                // ... in batches of this many steps (4: 51.2 us, never: 49.6 us on config 2)
-constexpr bool kStepRelease = false;                 // chain CTAs release their snapshot flags per step (true) or all at the end
 
 
 using namespace tc;
@@ -81,6 +82,17 @@ __device__ __forceinline__ unsigned long long wait_flag(const unsigned long long
     while (!flag_ready(w, epoch)) { __nanosleep(ns); w = ld_relaxed64(f); }
     return w;
 }
+// Waiting that may last long (output tasks waiting for a chain CTA): poll with RELAXED loads and a long sleep, then take
+// the value with one acquire load.  An acquire load invalidates the SM's L1 every time; chain CTAs share the SM.
+__device__ __forceinline__ unsigned long long wait_flag_quiet(const unsigned long long* f, unsigned int epoch) {
+    unsigned long long w;
+    for (;;) {
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w) : "l"(f) : "memory");
+        if (flag_ready(w, epoch)) break;
+        __nanosleep(500);
+    }
+    return ld_acquire64(f);
+}
 __device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_but1() { asm volatile("cp.async.bulk.wait_group 1;" ::: "memory"); }
 
@@ -105,7 +117,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     int bh, type, k;                                  // type 0 = P, 1 = B, 2 = A
     if (unit < BH) { bh = unit; type = 0; k = 0; }
     else { const int u = unit - BH; bh = u / (2 * (NS - 1)); const int r = u % (2 * (NS - 1)); k = 1 + (r >> 1); type = 1 + (r & 1); }
-    const int c_lo = k * fp.LSEG, c_hi = min(c_lo + fp.LSEG, NC);
+    const int c_lo = f64_seg_lo(fp.L0, fp.L1, k), c_hi = min(c_lo + (k == 0 ? fp.L0 : fp.L1), NC);
     const int nchunk = c_hi - c_lo, n = nchunk + (type == 0 ? NS - 1 : 0);
     const int m = 16 * warp + lane;
     const bool act = lane < 16, add_g = type == 2;
@@ -163,9 +175,27 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     auto gam_hist = [&](int e) { return lds_f32(aGam + 16 + (e < 1024 ? e : 1023) * 4); };
     int released = 0;                                 // thread 32: snapshot flags released so far, and gacc before that entry
     float ga_rel = 1.f;
-    float gh1 = 1.f, gh2 = 1.f, gh3 = 1.f;            // gacc before the last three entries (payload of the trailing flags)
     for (int e = 0; e < n; ++e) {
         const int st = e & 1;
+        if (tid == 32) {
+            // Snapshot of the state entry e acts on (independent of the entry's operands: issued before waiting for them).
+            // Its buffer is rewritten at the end of step e + 1: by then the store must have READ it (checked one step
+            // later, cheap).  Flags need COMPLETE stores and a gpu-scope fence, which on a state warp costs more than it
+            // buys during the scan (per-step release 55.4 us, batches of four 51.2, none 49.6 on config 2): a chain CTA
+            // releases its chunk snapshots when its chunks are done.  The segment-0 CTA does so when it ENTERS level 2
+            // (the outputs of segment 0 then run beside level 2) and releases every S_k one step after storing it.
+            tma_store_3d(tmM3, smem + C_OFF_SB + st * kTile, 0, 0, e_snap_z(e));
+            tma_store_commit();
+            asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+            if (type == 0 && e >= nchunk) {
+                asm volatile("cp.async.bulk.wait_group 1;" ::: "memory");
+                __threadfence();
+                for (; released < e; ++released) {
+                    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
+                    ga_rel *= gam_hist(released);
+                }
+            }
+        }
         mbar_wait(&full[st], (uint32_t)(e >> 1) & 1u);
         if (warp == 0) {
             // issued under elect.sync: with a plain `tid == 0` every tcgen05.mma sits in a ~70-cycle "waterfall" loop
@@ -187,26 +217,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
                 issue_load(e + 1, nf0);
                 if (e + 2 < n) { nf0 = ld_relaxed64(e_f0(e + 2)); nf1 = e_f1(e + 2) ? ld_relaxed64(e_f1(e + 2)) : ~0ull; }
             }
-        } else if (tid == 32) {
-            // snapshot of the state entry e acts on.  Its buffer is rewritten at the end of step e + 1: by then the store
-            // must have READ it (checked one step later, cheap).  Its flag needs the store to be COMPLETE, which takes
-            // longer than a step: flags trail by three steps so that the chain never waits for a store's round trip.
-            tma_store_3d(tmM3, smem + C_OFF_SB + st * kTile, 0, 0, e_snap_z(e));
-            tma_store_commit();
-            asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-            if (kStepRelease && e >= 3) {
-                asm volatile("cp.async.bulk.wait_group 3;" ::: "memory");
-                st_release64(e_snap_f(e - 3), flag_word(ep, gh3));
-            }
-            if (!kStepRelease && e >= released + kReleaseBatch + 1) {
-                // a batch of flags: the snapshots before entry e - 1 are complete; one fence, then relaxed stores
-                asm volatile("cp.async.bulk.wait_group 2;" ::: "memory");
-                __threadfence();
-                for (; released < e - 1; ++released) {
-                    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
-                    ga_rel *= gam_hist(released);
-                }
-            }
         }
         const float gamma = lds_f32(aGam + st * 4);
         if (act) {                                    // state-independent half, while the MMA runs
@@ -221,7 +231,6 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
             }
         }
         if (tid == 32 && e < 1024) sts_f32(aGam + 16 + e * 4, gamma);
-        gh3 = gh2; gh2 = gh1; gh1 = gacc;             // gacc before entries e-2, e-1, e (as seen at step e + 1)
         gacc *= gamma;
         mbar_wait(bar_mma, (uint32_t)e & 1u);
         tc_fence_after();
@@ -238,17 +247,10 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     }
     if (tid == 32) {
         tma_store_wait_all();
-        if (kStepRelease) {
-            if (n >= 3) st_release64(e_snap_f(n - 3), flag_word(ep, gh3));
-            if (n >= 2) st_release64(e_snap_f(n - 2), flag_word(ep, gh2));
-            st_release64(e_snap_f(n - 1), flag_word(ep, gh1));
-        } else {
-            // the remaining snapshot flags: one fence, then relaxed stores (payload: gacc before the entry, replayed)
-            __threadfence();
-            for (; released < n; ++released) {
-                asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
-                ga_rel *= gam_hist(released);
-            }
+        __threadfence();                              // the remaining snapshot flags: one fence, then relaxed stores
+        for (; released < n; ++released) {            // (payload: gacc before the entry, replayed from the gamma history)
+            asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e_snap_f(released)), "l"(flag_word(ep, ga_rel)) : "memory");
+            ga_rel *= gam_hist(released);
         }
         if (type != 0) {
             // the map of the whole segment: Gacc / B at its end (the operand buffer holds it in bf16), gamma of the segment
@@ -280,38 +282,38 @@ __device__ __forceinline__ void output_task(uint8_t* smem, uint32_t tmem, uint64
     const bool act = lane < 16;
     const uint32_t aS = smem_u32(smem + t64::OFF_K), aQ = smem_u32(smem + t64::OFF_Q), aO = smem_u32(smem + t64::OFF_V);
     const uint32_t aGA = smem_u32(smem + t64::OFF_PT), aB = smem_u32(smem + t64::OFF_X), aVec = smem_u32(smem + t64::OFF_VEC);
-    uint64_t *bar_ld = &bars[0], *bar_mma = &bars[2];
+    uint64_t *bar_ld = &bars[0], *bar_st = &bars[1], *bar_mma = &bars[2];      // both load barriers complete once per task (as in a tile task)
     const unsigned int ep = fp.epoch;
     const long long ci = (long long)bh * NC + c;
     const bool comp = k > 0;
     if (tid == 0) {
         tma_store_wait_read();                        // the previous task's stores have left the staging buffers
         if (pend_flag) { tma_store_wait_all(); st_release64(pend_flag, pend_val); }
-        wait_flag(fp.f_snap + ci, ep, 200);
-        if (comp) {
-            sts_f32(aVec, flag_payload(wait_flag(fp.f_snapA + ci, ep, 200)));
-            wait_flag(fp.f_segS + (long long)bh * NS + k, ep, 200);
-        }
-        acquire_after_poll();
+        // the tile's own operands first (they do not depend on S_k), then the state operand on a barrier of its own
+        wait_flag_quiet(fp.f_snap + ci, ep);
+        if (comp) sts_f32(aVec, flag_payload(wait_flag_quiet(fp.f_snapA + ci, ep)));
         fence_proxy_async_global();
         const int r0 = (int)(ci * 64);
-        mbar_expect_tx(bar_ld, (comp ? 5u : 3u) * kTile);
+        mbar_expect_tx(bar_ld, (comp ? 4u : 2u) * kTile);
         tma_load_2d(smem + t64::OFF_Q, tmR2, bar_ld, 0, (int)(fp.rQt + r0));
         tma_load_2d(smem + t64::OFF_V, tmR2, bar_ld, 0, (int)(fp.rOl + r0));
         if (comp) {
             tma_load_3d(smem + t64::OFF_PT, tmM3, bar_ld, 0, 0, fp.zGA + (int)ci);
             tma_load_3d(smem + t64::OFF_X, tmM3, bar_ld, 0, 0, fp.zSc + (int)ci);
-            tma_load_3d(smem + t64::OFF_K, tmM3, bar_ld, 0, 0, fp.zSk + bh * NS + k);
-        } else {
-            tma_load_3d(smem + t64::OFF_K, tmM3, bar_ld, 0, 0, fp.zSc + (int)ci);
+            wait_flag_quiet(fp.f_segS + (long long)bh * NS + k, ep);
+            fence_proxy_async_global();
         }
+        mbar_expect_tx(bar_st, kTile);
+        tma_load_3d(smem + t64::OFF_K, tmM3, bar_st, 0, 0, comp ? fp.zSk + bh * NS + k : fp.zSc + (int)ci);
         mbar_wait(bar_ld, pl);
+        mbar_wait(bar_st, pl);
     }
     // Only thread 0 polls (flags, then the load barrier); the others sleep in the CTA barrier instead of spinning on the
     // mbarrier: this CTA shares its SM with chain CTAs whose steps are the critical path.
     __syncthreads();
     auto wait_mma = [&]() { mbar_wait(bar_mma, ph); ph ^= 1; tc_fence_after(); };
     mbar_wait(bar_ld, pl);
+    mbar_wait(bar_st, pl);
     pl ^= 1u;
     if (comp) {
         // S_c = gacc_c S_k - Gacc_c S_k + B_c: one MMA on the bf16 S_k, fp32 combination, S_c (bf16) over S_k
@@ -423,21 +425,24 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         auto decode = [&](int task, bool& tile, int& bh, int& c, int& k) {
             tile = task < fp.n_tile_tasks;
             const int tt = tile ? task : task - fp.n_tile_tasks;
+            int j;
             if (tile) {                               // segments interleaved: (j, k, bh)
-                const int j = tt / (fp.NS * BH), r = tt % (fp.NS * BH);
-                k = r / BH; bh = r % BH; c = k * fp.LSEG + j;
+                j = tt / (fp.NS * BH);
+                const int r = tt % (fp.NS * BH);
+                k = r / BH; bh = r % BH;
             } else {                                  // segment-major: (k, j, bh)
-                k = tt / (fp.LSEG * BH);
-                const int r = tt % (fp.LSEG * BH);
-                bh = r % BH; c = k * fp.LSEG + r / BH;
+                k = tt / (fp.L0 * BH);
+                const int r = tt % (fp.L0 * BH);
+                bh = r % BH; j = r / BH;
             }
-            if (c >= (k + 1) * fp.LSEG) c = p.NC;
+            c = f64_seg_lo(fp.L0, fp.L1, k) + j;
+            if (j >= (k == 0 ? fp.L0 : fp.L1)) c = p.NC;
         };
         unsigned long long* pend_flag = nullptr;      // flag of this CTA's last tile task, released inside the next task
         unsigned long long pend_val = 0ull;
         const uint32_t aRaw = smem_u32(smem + t64::OFF_RAW);
         int raw_sel = 0;                              // raw gate buffer of the current task
-        bool have_cur = false;
+        bool have_cur = false, first_tile = true;
         // static round-robin over the workers: waves of tile tasks complete in task order (the chain CTAs consume them
         // in that order), and the task after this one is known in advance (its inputs are prefetched during this one).
         // (A dynamic queue -- one atomic counter, the next task claimed a task ahead -- measured 15 us slower on config 2.)
@@ -479,6 +484,11 @@ gdn_tok_fused64(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     t64::tile64<true>(smem, tmem, bars, mp, p, bh, c, pl, ph, have_cur ? aRaw + (uint32_t)raw_sel * 512u : 0u, pend_flag, pend_val, &gam_c);
                     pend_flag = fp.f_tile + (long long)bh * p.NC + c;
                     pend_val = flag_word(fp.epoch, gam_c);
+                    if (first_tile) {                 // the chain CTAs are waiting for the first wave: publish it at once
+                        if (tid == 0) { tma_store_wait_all(); st_release64(pend_flag, pend_val); }
+                        pend_flag = nullptr;
+                        first_tile = false;
+                    }
                 } else {
                     output_task(smem, tmem, bars, &tmM3, &tmR2, &tmO, fp, bh, c, k, pl, ph, pend_flag, pend_val);
                     pend_flag = nullptr;
