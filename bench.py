@@ -239,7 +239,7 @@ def run_ours(args):
     set_bytes = wl.B * wl.T * wl.H * (2 * wl.d_k + 2 * wl.d_v) * es
     n_sets = max(2, int(L2_BYTES * 1.5 // set_bytes) + 1)         # rotate so the inputs of a step are cold in L2
     n_sets = min(n_sets, 16)
-    norm = bool(args.normalizer)
+    norm = bool(args.normalizer) or bool(args.full)
     if norm:
         set_bytes += wl.B * wl.T * wl.H * 2 * wl.d_k * es
         n_sets = min(16, max(2, int(L2_BYTES * 1.5 // set_bytes) + 1))
@@ -260,9 +260,28 @@ def run_ours(args):
     info = plan.info
     stream = torch.cuda.current_stream()
 
+    full = None
+    if args.full:
+        # operands of the front end; one packed qkv tensor per input set (the q / k / v views carry the packed token stride)
+        full = []
+        for i in range(n_sets):
+            fi = gin.make_frontend_inputs(wl, seed=rank_seed(wl, rank, i) + 17)
+            dd = {n: fi[n].to(dev) for n in ("qkv", "x", "w_q", "w_k", "cos", "sin", "w_alpha", "b_alpha", "a_log", "w_beta", "b_beta", "gate")}
+            dd["fm"] = gdn.make_featmap_args(dd["qkv"][:, :, 0], dd["qkv"][:, :, 1], dd["w_q"], dd["w_k"], dd["cos"], dd["sin"], 1e-6)
+            dd["ga"] = gdn.make_gate_args(dd["x"], dd["w_alpha"], dd["b_alpha"], dd["a_log"], dd["w_beta"], dd["b_beta"])
+            full.append(dd)
+        plan.close()
+        st3 = 3 * wl.H * wl.d_k
+        plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, flags=flags | gdn.GDN_FLAG_LOG_ALPHA,
+                           q_token_stride=st3, k_token_stride=st3, v_token_stride=st3)
+        info = plan.info
+
     def step(i):
         s = sets[i % n_sets]
-        if norm:
+        if full is not None:
+            f = full[i % n_sets]
+            plan.forward_full(f["fm"], f["qkv"][:, :, 2], f["ga"], None, None, f["gate"], state, zstate, s["out"], state, zstate, stream=stream)
+        elif norm:
             plan.forward_norm(s["q"], s["k"], s["v"], s["q_raw"], s["k_raw"], s["alpha"], s["beta"], state, zstate,
                               s["out"], state, zstate, stream=stream)
         else:
@@ -321,6 +340,8 @@ def run_ours(args):
     if norm:                                       # + 2 d^2 flops and + 4 d bytes per token-head (q_raw, k_raw), + z in/out
         fl += wl.B * wl.H * wl.T * 2 * wl.d_k * wl.d_k
         by += wl.B * wl.H * wl.T * 2 * wl.d_k * es + 2 * wl.B * wl.H * wl.d_k * 4
+    if args.full:                                  # qkv, x and the output gate read once, out written once; alpha / beta never leave the device
+        by = wl.B * wl.H * wl.T * 6 * wl.d_k * es + 2 * wl.B * wl.H * (wl.d_k * wl.d_v + wl.d_k) * 4
     tflops = fl / (ms_per_step * 1e-3) / 1e12
     roof = roofline(wl, info, kernels, ms_per_step, pk, pk_src, by)
     line = {
@@ -336,7 +357,7 @@ def run_ours(args):
         "roofline": roof, "kernels": kernels,
     }
     if norm or args.bidir:
-        line["config"]["variant"] = "+".join(x for x, on in (("normalizer", norm), ("bidir", args.bidir)) if on)
+        line["config"]["variant"] = "+".join(x for x, on in (("full operator (feature map, gates, output gate)", bool(args.full)), ("normalizer", norm), ("bidir", args.bidir)) if on)
     if rank == 0 and world == 1 and not args.no_cpu and not norm and not args.bidir:
         line["cpu_baseline"] = cpu_baseline(wl)
     plan.close()
@@ -407,6 +428,7 @@ def kernel_bytes(name, wl, by_call):
         "gdn_tok_chain": 2 * st,
         "gdn_frm_summaries": th * ((wl.d_k + wl.d_v) * es + 4),
         "gdn_frm_readout": th * (wl.d_k + wl.d_v) * es,
+        "gdn_frontend_kernel": th * 7 * wl.d_k * es,      # q, k read; q_rot, k_rot, q_raw, k_raw written
     }
     if name.startswith("gdn_tok_chain") or name == "gdn_frm_hist_add":
         return 2 * st                              # the scans only carry the state in and out; their summaries are workspace
@@ -444,6 +466,8 @@ def main():
     ap.add_argument("--bidir", action="store_true", help="frame mode: bidirectional in-chunk scan (Alg. 1)")
     ap.add_argument("--paper-shape", action="store_true", help="3 x 880 tokens, 20 heads, d = 128, frame-wise")
     ap.add_argument("--d112", action="store_true", help="with --paper-shape: unpadded head dim 112")
+    ap.add_argument("--full", action="store_true", help="frame mode: the operator at the paper's kernel boundary (Alg. 1): feature map + gates + "
+                    "normalised (--bidir: bidirectional) recurrence + output gate through gdn_forward_chunk_full, from a packed qkv tensor")
     ap.add_argument("--unfused", action="store_true", help="token mode: the three-kernel path (prepass / chain / output) for A/B runs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -211,14 +211,17 @@ gdn_status_t fe_check(gdn_plan_t* p) {
     return GDN_OK;
 }
 
-gdn_status_t featmap_impl(gdn_plan_t* p, const gdn_featmap_args_t* a, void* q_rot, void* k_rot, void* q_raw, void* k_raw, cudaStream_t st, bool mark = true) {
+// validate + fill; returns GDN_OK with `active` = false for an empty problem
+gdn_status_t featmap_fill(gdn_plan_t* p, const gdn_featmap_args_t* a, void* q_rot, void* k_rot, void* q_raw, void* k_raw,
+                          gdn::FeatmapParams& fp, bool& active) {
     const gdn_config_t& c = p->cfg;
+    active = false;
     if (!a || !a->q || !a->k || !a->rms_wq || !a->rms_wk || !a->rope_cos || !a->rope_sin || !q_rot || !k_rot || !q_raw || !k_raw)
         return fail(p, GDN_ERR_INVALID_ARG, "a required feature-map pointer is NULL");
     const void* ptrs[] = {a->q, a->k, a->rms_wq, a->rms_wk, a->rope_cos, a->rope_sin, q_rot, k_rot, q_raw, k_raw};
     for (const void* ptr : ptrs) if (!aligned16(ptr)) return fail(p, GDN_ERR_ALIGNMENT, "tensor pointers must be 16-byte aligned");
     if (c.B == 0 || c.H == 0 || c.T == 0) return GDN_OK;
-    gdn::FeatmapParams fp{};
+    fp = gdn::FeatmapParams{};
     fp.q = static_cast<const __nv_bfloat16*>(a->q); fp.k = static_cast<const __nv_bfloat16*>(a->k);
     fp.wq = a->rms_wq; fp.wk = a->rms_wk; fp.cosT = a->rope_cos; fp.sinT = a->rope_sin;
     fp.q_rot = static_cast<__nv_bfloat16*>(q_rot); fp.k_rot = static_cast<__nv_bfloat16*>(k_rot);
@@ -227,14 +230,8 @@ gdn_status_t featmap_impl(gdn_plan_t* p, const gdn_featmap_args_t* a, void* q_ro
     fp.B = c.B; fp.T = c.T; fp.H = c.H; fp.D = c.d_k;
     fp.rms_eps = a->rms_eps;
     fp.kscale = 1.f / sqrtf((float)c.d_k * (float)c.group);
-    const long long rows = (long long)c.B * c.T * c.H;
-    long long blocks = (rows + 15) / 16;
-    const long long cap = 8LL * (p->sm_count > 0 ? p->sm_count : 148);
-    if (blocks > cap) blocks = cap;
-    gdn::fe::gdn_featmap_kernel<<<(int)blocks, gdn::fe::kFeThreads, 0, st>>>(fp);
-    if (mark) p->prof.mark(st, "gdn_featmap_kernel");
-    cudaError_t e = cudaGetLastError();
-    return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_featmap_kernel launch");
+    active = true;
+    return GDN_OK;
 }
 
 size_t fe_up4(size_t n) { return (n + 3) / 4 * 4; }        // 16-byte aligned sub-buffers
@@ -255,8 +252,9 @@ gdn_status_t fe_gate_buffers(gdn_plan_t* p) {
     return GDN_OK;
 }
 
-gdn_status_t gates_impl(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_out, float* beta_out, cudaStream_t st, bool mark = true) {
+gdn_status_t gates_fill(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_out, float* beta_out, gdn::GateParams& gp, bool& active) {
     const gdn_config_t& c = p->cfg;
+    active = false;
     if (!a || !a->x || !a->w_alpha || !a->b_alpha || !a->a_log || !a->w_beta || !a->b_beta || !alpha_out || !beta_out)
         return fail(p, GDN_ERR_INVALID_ARG, "a required gate pointer is NULL");
     if (!aligned16(a->x) || (a->x_token_stride % 8) != 0) return fail(p, GDN_ERR_ALIGNMENT, "x must be 16-byte aligned with a token stride that is a multiple of 8");
@@ -264,7 +262,7 @@ gdn_status_t gates_impl(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_ou
     gdn_status_t bs = fe_gate_buffers(p);
     if (bs != GDN_OK) return bs;
     const size_t BH = (size_t)c.B * c.H, F = (size_t)(c.T / c.group);
-    gdn::GateParams gp{};
+    gp = gdn::GateParams{};
     gp.x = static_cast<const __nv_bfloat16*>(a->x);
     gp.w_alpha = a->w_alpha; gp.b_alpha = a->b_alpha; gp.a_log = a->a_log; gp.w_beta = a->w_beta; gp.b_beta = a->b_beta;
     gp.alpha_out = alpha_out; gp.beta_out = beta_out;
@@ -273,10 +271,27 @@ gdn_status_t gates_impl(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_ou
     gp.x_ts = tok_stride(a->x_token_stride, c.H, c.d_k);
     gp.B = c.B; gp.T = c.T; gp.H = c.H; gp.D = c.d_k; gp.G = c.group; gp.F = (int)F; gp.NSPL = p->fe_nspl;
     gp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
-    gdn::fe::gdn_gates_kernel<<<dim3((unsigned)(BH * F), (unsigned)p->fe_nspl), gdn::fe::kFeThreads, 0, st>>>(gp);
-    if (mark) p->prof.mark(st, "gdn_gates_kernel");
+    active = true;
+    return GDN_OK;
+}
+
+// ONE launch for whichever parts are active: blocks [0, n_fm) feature map, then B*H*F*NSPL gate blocks
+gdn_status_t launch_frontend(gdn_plan_t* p, const gdn::FeatmapParams* fm, const gdn::GateParams* gp, cudaStream_t st, bool mark) {
+    int n_fm = 0, n_g = 0;
+    if (fm) {
+        const long long rows = (long long)fm->B * fm->T * fm->H, per = 16LL * gdn::fe::kFeRows;
+        long long blocks = (rows + per - 1) / per;
+        const long long cap = 8LL * (p->sm_count > 0 ? p->sm_count : 148);
+        n_fm = (int)(blocks > cap ? cap : blocks);
+    }
+    if (gp) n_g = gp->B * gp->H * gp->F * gp->NSPL;
+    if (n_fm + n_g == 0) return GDN_OK;
+    gdn::GateParams g0{};
+    g0.NSPL = 1;
+    gdn::fe::gdn_frontend_kernel<<<n_fm + n_g, gdn::fe::kFeThreads, 0, st>>>(fm ? *fm : gdn::FeatmapParams{}, gp ? *gp : g0, n_fm);
+    if (mark) p->prof.mark(st, "gdn_frontend_kernel");
     cudaError_t e = cudaGetLastError();
-    return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_gates_kernel launch");
+    return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_frontend_kernel launch");
 }
 
 }  // namespace
@@ -387,16 +402,24 @@ gdn_status_t gdn_feature_map(gdn_plan_t* plan, const gdn_featmap_args_t* args, v
     if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
     gdn_status_t s = fe_check(plan);
     if (s != GDN_OK) return s;
+    gdn::FeatmapParams fp;
+    bool on = false;
+    s = featmap_fill(plan, args, q_rot, k_rot, q_raw, k_raw, fp, on);
+    if (s != GDN_OK || !on) return s;
     plan->prof.begin(static_cast<cudaStream_t>(stream));
-    return featmap_impl(plan, args, q_rot, k_rot, q_raw, k_raw, static_cast<cudaStream_t>(stream));
+    return launch_frontend(plan, &fp, nullptr, static_cast<cudaStream_t>(stream), true);
 }
 
 gdn_status_t gdn_compute_gates(gdn_plan_t* plan, const gdn_gate_args_t* args, float* alpha_out, float* beta_out, gdn_stream_t stream) {
     if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
     gdn_status_t s = fe_check(plan);
     if (s != GDN_OK) return s;
+    gdn::GateParams gp;
+    bool on = false;
+    s = gates_fill(plan, args, alpha_out, beta_out, gp, on);
+    if (s != GDN_OK || !on) return s;
     plan->prof.begin(static_cast<cudaStream_t>(stream));
-    return gates_impl(plan, args, alpha_out, beta_out, static_cast<cudaStream_t>(stream));
+    return launch_frontend(plan, nullptr, &gp, static_cast<cudaStream_t>(stream), true);
 }
 
 gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* fm, const void* v, const gdn_gate_args_t* gates,
@@ -418,16 +441,21 @@ gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* 
         if (cudaMalloc(&plan->fe_feat, 4 * feat * 2) != cudaSuccess) { cudaGetLastError(); return fail(plan, GDN_ERR_NOMEM, "feature buffer allocation failed"); }
     }
     __nv_bfloat16* fb = static_cast<__nv_bfloat16*>(plan->fe_feat);
+    gdn::FeatmapParams fmp;
+    gdn::GateParams gtp;
+    bool fm_on = false, g_on = false;
     if (gates) {
         s = fe_gate_buffers(plan);
         if (s != GDN_OK) return s;
         float* a_buf = plan->fe_gates;
         float* b_buf = plan->fe_gates + fe_up4((size_t)c.B * c.H * (c.T / c.group));
-        s = gates_impl(plan, gates, a_buf, b_buf, st, false);
+        s = gates_fill(plan, gates, a_buf, b_buf, gtp, g_on);
         if (s != GDN_OK) return s;
         alpha = a_buf; beta = b_buf;
     }
-    s = featmap_impl(plan, fm, fb, fb + feat, fb + 2 * feat, fb + 3 * feat, st, false);
+    s = featmap_fill(plan, fm, fb, fb + feat, fb + 2 * feat, fb + 3 * feat, fmp, fm_on);
+    if (s != GDN_OK) return s;
+    s = launch_frontend(plan, fm_on ? &fmp : nullptr, g_on ? &gtp : nullptr, st, false);
     if (s != GDN_OK) return s;
     return forward_impl(plan, fb, fb + feat, v, fb + 2 * feat, fb + 3 * feat, alpha, beta, S_in, z_in, out, S_out, z_out, st, true,
                         out_gate, true);

@@ -2,11 +2,11 @@
 // qkv, beta, decay alpha, normalization weights, RoPE tables", L325): both are HBM-bound element-wise / reduction passes
 // (no contraction worth a tensor core), written for coalesced 16-byte accesses.
 //
-//   gdn_featmap_kernel   Eq. 12 (L552) + key rescale (L554): per (token, head) row of D channels
+//   featmap_body         Eq. 12 (L552) + key rescale (L554): per (token, head) row of D channels
 //                            y = ReLU(RMSNorm(x) * w),  raw = y,  rot = rho(y) on adjacent channel pairs,
 //                            keys additionally * 1/sqrt(D N).  q and k are read ONCE and all four feature tensors the
 //                            recurrence needs (q_rot, k_rot for the KV memory; q_raw, k_raw for the normaliser) leave.
-//   gdn_gates_kernel     Eq. 13-15 (L562-L572): beta_n = sigmoid(W_beta . x_n + b_beta) per token,
+//   gates_body           Eq. 13-15 (L562-L572): beta_n = sigmoid(W_beta . x_n + b_beta) per token,
 //                            alpha_f = exp(-e^{A_log} softplus(W_alpha . mean_n x_n + b_alpha)) per frame.  The mean
 //                            commutes with the projection, so the frame sum of the per-token dots is accumulated in a
 //                            FIXED order (per 16-lane group, then over groups, then over the splits of a frame by the
@@ -62,76 +62,85 @@ __device__ __forceinline__ float group16_sum(float v) {
 
 constexpr int kFeThreads = 256;            // 16 rows of 16 lanes; a lane owns 8 consecutive channels (D <= 128)
 
-__global__ void __launch_bounds__(kFeThreads)
-gdn_featmap_kernel(const FeatmapParams p) {
+constexpr int kFeRows = 2;                 // rows / tokens a 16-lane group has in flight per iteration (independent loads)
+
+// Feature map of rows r0 + g + 16 j (j < kFeRows) of [B*T*H] (row = one token of one head), grid-stride over row groups.
+__device__ __forceinline__ void featmap_body(const FeatmapParams& p, int block, int nblocks) {
     const int g = threadIdx.x >> 4, l = threadIdx.x & 15;
     const long long rows = (long long)p.B * p.T * p.H;
     const int c0 = l * 8;
     const bool on = c0 < p.D;
     const float inv_d = 1.f / (float)p.D;
-    for (long long r0 = (long long)blockIdx.x * 16; r0 < rows; r0 += (long long)gridDim.x * 16) {     // uniform trip count: the
-        const bool valid = r0 + g < rows;                                                             // shuffles need the whole warp
-        const long long r = valid ? r0 + g : rows - 1;
-        const int h = (int)(r % p.H);
-        const long long bt = r / p.H;
-        const int t = (int)(bt % p.T);
-        float xq[8], xk[8];
+    constexpr int R = kFeRows;
+    for (long long r0 = (long long)block * 16 * R; r0 < rows; r0 += (long long)nblocks * 16 * R) {   // uniform trip count: the
+        float xq[R][8], xk[R][8];                                                                     // shuffles need the whole warp
+        long long rr[R];
+        bool valid[R];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { xq[i] = 0.f; xk[i] = 0.f; }
-        if (on) {
-            unpack8f(__ldg(reinterpret_cast<const uint4*>(p.q + bt * p.q_ts + (long long)h * p.D + c0)), xq);
-            unpack8f(__ldg(reinterpret_cast<const uint4*>(p.k + bt * p.k_ts + (long long)h * p.D + c0)), xk);
-        }
-        float sq = 0.f, sk = 0.f;
+        for (int j = 0; j < R; ++j) {
+            valid[j] = r0 + g + 16 * j < rows;
+            rr[j] = valid[j] ? r0 + g + 16 * j : rows - 1;
+            const int h = (int)(rr[j] % p.H);
+            const long long bt = rr[j] / p.H;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { sq = fmaf(xq[i], xq[i], sq); sk = fmaf(xk[i], xk[i], sk); }
-        sq = group16_sum(sq);
-        sk = group16_sum(sk);
-        if (!on || !valid) continue;
-        const float rq = rsqrtf(sq * inv_d + p.rms_eps), rk = rsqrtf(sk * inv_d + p.rms_eps);
-        const float4 wq0 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0));
-        const float4 wq1 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0 + 4));
-        const float4 wk0 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0));
-        const float4 wk1 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0 + 4));
-        const float wqv[8] = {wq0.x, wq0.y, wq0.z, wq0.w, wq1.x, wq1.y, wq1.z, wq1.w};
-        const float wkv[8] = {wk0.x, wk0.y, wk0.z, wk0.w, wk1.x, wk1.y, wk1.z, wk1.w};
-        const float4 cs = __ldg(reinterpret_cast<const float4*>(p.cosT + (long long)t * (p.D / 2) + c0 / 2));
-        const float4 sn = __ldg(reinterpret_cast<const float4*>(p.sinT + (long long)t * (p.D / 2) + c0 / 2));
-        const float cv[4] = {cs.x, cs.y, cs.z, cs.w}, sv[4] = {sn.x, sn.y, sn.z, sn.w};
-        float qr[8], kr[8], qo[8], ko[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            qr[i] = fmaxf(xq[i] * rq * wqv[i], 0.f);
-            kr[i] = fmaxf(xk[i] * rk * wkv[i], 0.f) * p.kscale;
+            for (int i = 0; i < 8; ++i) { xq[j][i] = 0.f; xk[j][i] = 0.f; }
+            if (on) {
+                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.q + bt * p.q_ts + (long long)h * p.D + c0)), xq[j]);
+                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.k + bt * p.k_ts + (long long)h * p.D + c0)), xk[j]);
+            }
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            qo[2 * i] = qr[2 * i] * cv[i] - qr[2 * i + 1] * sv[i];
-            qo[2 * i + 1] = qr[2 * i] * sv[i] + qr[2 * i + 1] * cv[i];
-            ko[2 * i] = kr[2 * i] * cv[i] - kr[2 * i + 1] * sv[i];
-            ko[2 * i + 1] = kr[2 * i] * sv[i] + kr[2 * i + 1] * cv[i];
+        for (int j = 0; j < R; ++j) {
+            float sq = 0.f, sk = 0.f;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { sq = fmaf(xq[j][i], xq[j][i], sq); sk = fmaf(xk[j][i], xk[j][i], sk); }
+            sq = group16_sum(sq);
+            sk = group16_sum(sk);
+            if (!on || !valid[j]) continue;
+            const int h = (int)(rr[j] % p.H);
+            const int t = (int)((rr[j] / p.H) % p.T);
+            const float rq = rsqrtf(sq * inv_d + p.rms_eps), rk = rsqrtf(sk * inv_d + p.rms_eps);
+            const float4 wq0 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0));
+            const float4 wq1 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0 + 4));
+            const float4 wk0 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0));
+            const float4 wk1 = __ldg(reinterpret_cast<const float4*>(p.wk + (long long)h * p.D + c0 + 4));
+            const float wqv[8] = {wq0.x, wq0.y, wq0.z, wq0.w, wq1.x, wq1.y, wq1.z, wq1.w};
+            const float wkv[8] = {wk0.x, wk0.y, wk0.z, wk0.w, wk1.x, wk1.y, wk1.z, wk1.w};
+            const float4 cs = __ldg(reinterpret_cast<const float4*>(p.cosT + (long long)t * (p.D / 2) + c0 / 2));
+            const float4 sn = __ldg(reinterpret_cast<const float4*>(p.sinT + (long long)t * (p.D / 2) + c0 / 2));
+            const float cv[4] = {cs.x, cs.y, cs.z, cs.w}, sv[4] = {sn.x, sn.y, sn.z, sn.w};
+            float qr[8], kr[8], qo[8], ko[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                qr[i] = fmaxf(xq[j][i] * rq * wqv[i], 0.f);
+                kr[i] = fmaxf(xk[j][i] * rk * wkv[i], 0.f) * p.kscale;
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                qo[2 * i] = qr[2 * i] * cv[i] - qr[2 * i + 1] * sv[i];
+                qo[2 * i + 1] = qr[2 * i] * sv[i] + qr[2 * i + 1] * cv[i];
+                ko[2 * i] = kr[2 * i] * cv[i] - kr[2 * i + 1] * sv[i];
+                ko[2 * i + 1] = kr[2 * i] * sv[i] + kr[2 * i + 1] * cv[i];
+            }
+            const long long o = rr[j] * p.D + c0;
+            *reinterpret_cast<uint4*>(p.q_raw + o) = pack8f(qr);
+            *reinterpret_cast<uint4*>(p.k_raw + o) = pack8f(kr);
+            *reinterpret_cast<uint4*>(p.q_rot + o) = pack8f(qo);
+            *reinterpret_cast<uint4*>(p.k_rot + o) = pack8f(ko);
         }
-        const long long o = r * p.D + c0;
-        *reinterpret_cast<uint4*>(p.q_raw + o) = pack8f(qr);
-        *reinterpret_cast<uint4*>(p.k_raw + o) = pack8f(kr);
-        *reinterpret_cast<uint4*>(p.q_rot + o) = pack8f(qo);
-        *reinterpret_cast<uint4*>(p.k_rot + o) = pack8f(ko);
     }
 }
 
-// grid = (B*H*F, NSPL).  Split s of frame (b, h, f) owns the tokens n = s*16*per + ... : group g of the CTA takes tokens
-// base + g, base + g + 16, ... in order, so every partial sum has a fixed association.
-__global__ void __launch_bounds__(kFeThreads)
-gdn_gates_kernel(const GateParams p) {
-    __shared__ float s_sum[16];
-    __shared__ unsigned int s_last;
+// Split s of frame (b, h, f) owns the tokens [s*per, (s+1)*per): group g of the CTA takes tokens base + g, base + g + 16, ...
+// in order, so every partial sum has a fixed association.
+__device__ __forceinline__ void gates_body(const GateParams& p, int bhf, int s, float* s_sum, unsigned int* s_last) {
     const int g = threadIdx.x >> 4, l = threadIdx.x & 15;
-    const int bhf = blockIdx.x, s = blockIdx.y;
     const int f = bhf % p.F, bh = bhf / p.F, b = bh / p.H, h = bh % p.H;
     const int per = (p.G + p.NSPL - 1) / p.NSPL;               // tokens per split
     const int n_lo = s * per, n_hi = min(n_lo + per, p.G);
     const int c0 = l * 8;
     const bool on = c0 < p.D;
+    constexpr int R = kFeRows;
     float wa[8], wb[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) { wa[i] = 0.f; wb[i] = 0.f; }
@@ -140,22 +149,29 @@ gdn_gates_kernel(const GateParams p) {
         for (int i = 0; i < 8; ++i) { wa[i] = __ldg(p.w_alpha + (long long)h * p.D + c0 + i); wb[i] = __ldg(p.w_beta + (long long)h * p.D + c0 + i); }
     }
     const float bb = __ldg(p.b_beta + h);
-    float acc = 0.f;                                           // sum of W_alpha . x_n over this group's tokens
-    for (int n0 = n_lo; n0 < n_hi; n0 += 16) {                 // uniform trip count: the shuffles need the whole warp
-        const int n = n0 + g;
-        const bool valid = n < n_hi;
-        const long long t = (long long)f * p.G + (valid ? n : n_lo);
-        float x[8];
+    float acc = 0.f;                                           // sum of W_alpha . x_n over this group's tokens, in token order
+    for (int n0 = n_lo; n0 < n_hi; n0 += 16 * R) {             // uniform trip count: the shuffles need the whole warp
+        float x[R][8];
+        bool valid[R];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = 0.f;
-        if (on && valid) unpack8f(__ldg(reinterpret_cast<const uint4*>(p.x + ((long long)b * p.T + t) * p.x_ts + (long long)h * p.D + c0)), x);
-        float da = 0.f, db = 0.f;
+        for (int j = 0; j < R; ++j) {
+            const int n = n0 + g + 16 * j;
+            valid[j] = n < n_hi;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { da = fmaf(wa[i], x[i], da); db = fmaf(wb[i], x[i], db); }
-        da = group16_sum(da);
-        db = group16_sum(db);
-        acc += da;                                             // da = 0 for a tail group (x = 0)
-        if (l == 0 && valid) p.beta_out[(long long)bh * p.T + t] = 1.f / (1.f + __expf(-(db + bb)));      // Eq. 15
+            for (int i = 0; i < 8; ++i) x[j][i] = 0.f;
+            if (on && valid[j])
+                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.x + ((long long)b * p.T + (long long)f * p.G + n) * p.x_ts + (long long)h * p.D + c0)), x[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < R; ++j) {
+            float da = 0.f, db = 0.f;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { da = fmaf(wa[i], x[j][i], da); db = fmaf(wb[i], x[j][i], db); }
+            da = group16_sum(da);
+            db = group16_sum(db);
+            acc += da;                                         // da = 0 for a tail slot (x = 0)
+            if (l == 0 && valid[j]) p.beta_out[(long long)bh * p.T + (long long)f * p.G + n0 + g + 16 * j] = 1.f / (1.f + __expf(-(db + bb)));      // Eq. 15
+        }
     }
     if (l == 0) s_sum[g] = acc;
     __syncthreads();
@@ -165,8 +181,8 @@ gdn_gates_kernel(const GateParams p) {
         for (int i = 0; i < 16; ++i) tot += s_sum[i];
         p.part[(long long)bhf * p.NSPL + s] = tot;
         __threadfence();
-        s_last = atomicAdd(p.counters + bhf, 1u) == (unsigned int)(p.NSPL - 1) ? 1u : 0u;
-        if (s_last) {
+        *s_last = atomicAdd(p.counters + bhf, 1u) == (unsigned int)(p.NSPL - 1) ? 1u : 0u;
+        if (*s_last) {
             __threadfence();
             float sum = 0.f;
             for (int i = 0; i < p.NSPL; ++i) sum += __ldcg(p.part + (long long)bhf * p.NSPL + i);
@@ -177,6 +193,23 @@ gdn_gates_kernel(const GateParams p) {
             p.counters[bhf] = 0u;
         }
     }
+}
+
+// ONE launch for the whole front end: blocks [0, n_fm) run the feature map, the rest the gates (either part may be empty).
+// The recurrence's first kernel is launched as a programmatic dependent of this one.
+__global__ void __launch_bounds__(kFeThreads, 4)
+gdn_frontend_kernel(const FeatmapParams fm, const GateParams gp, const int n_fm) {
+    __shared__ float s_sum[16];
+    __shared__ unsigned int s_last;
+    if ((int)blockIdx.x < n_fm) {
+        featmap_body(fm, (int)blockIdx.x, n_fm);
+    } else {
+        const int idx = (int)blockIdx.x - n_fm;
+        gates_body(gp, idx / gp.NSPL, idx % gp.NSPL, s_sum, &s_last);
+    }
+    // only now: dependents launched earlier would sit on the SMs (Phase A's CTAs take most of an SM's shared memory)
+    // while blocks of this grid are still waiting to be scheduled
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
 }  // namespace fe

@@ -445,7 +445,7 @@ inline cudaError_t tc_launch_fused64(TcPlan& tp, const TokParams& p, cudaStream_
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
                                    const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
-                                   cudaEvent_t before_readout = nullptr) {
+                                   cudaEvent_t before_readout = nullptr, bool pdl_first = false) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -461,9 +461,14 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     const int sms = tp.sm_count > 0 ? tp.sm_count : 148;
     const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
     if (prof) prof->begin(st);
-    gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tmK, tmV, fp);
-    if (prof) prof->mark(st, "gdn_frm_summaries");
     cudaError_t le;
+    if (pdl_first) {       // the front-end kernel precedes in the stream: its tail overlaps this kernel's prologue
+        le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
+        if (le != cudaSuccess) return le;
+    } else {
+        gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tmK, tmV, fp);
+    }
+    if (prof) prof->mark(st, "gdn_frm_summaries");
     const int nchain = tp.BH * (D / 64);
     if (tp.bidir && tp.F > 1) {
         // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero
@@ -554,8 +559,9 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
             den_ready = tp.zev1;
         }
-        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready)
-                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready);
+        const bool pdl_first = na && na->dense_qk;
+        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, pdl_first)
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, pdl_first);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

@@ -138,6 +138,7 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    pdl_wait();                                    // no-op unless launched as a dependent of the front-end kernel (gdn_forward_chunk_full)
     pdl_launch_dependents();
 
     if (warp == 5) {
