@@ -258,7 +258,8 @@ def run_ours(args):
     plan = gdn.GdnPlan(B=wl.B, H=wl.H, T=wl.T, d_k=wl.d_k, d_v=wl.d_v, group=wl.group, chunk=wl.chunk, flags=flags,
                        io_dtype=gdn.GDN_BF16 if wl.dtype == torch.bfloat16 else gdn.GDN_FP32)
     info = plan.info
-    stream = torch.cuda.current_stream()
+    stream = torch.cuda.Stream(device=dev)         # a stream of its own (the library replays CUDA graphs on non-default streams)
+    stream.wait_stream(torch.cuda.current_stream())
 
     full = None
     if args.full:

@@ -79,6 +79,11 @@ struct gdn_plan {
     void* fe_feat = nullptr;      // q_rot | k_rot | q_raw | k_raw, dense [B,T,H,D] bf16 each
     float* fe_gates = nullptr;    // alpha [B,H,F] | beta [B,H,T] | partial frame sums | counters
     int fe_nspl = 1;
+    // CUDA graphs of the multi-launch frame-wise calls, one per tuple of argument pointers (see run_graphed)
+    struct GraphEntry { std::vector<const void*> key; cudaGraphExec_t exec = nullptr; unsigned long long used = 0; };
+    std::vector<GraphEntry> graphs;
+    unsigned long long graph_tick = 0;
+    bool graph_warm = false;      // the first call of a plan is issued directly (kernel attributes, lazy allocations)
     Staging host;
     gdn::TcPlan tc;               // tensor-core path state (tensor maps, workspace carving)
     gdn::Profiler prof;           // optional per-kernel CUDA events (bench roofline)
@@ -197,6 +202,54 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
     return GDN_OK;
 }
 
+
+
+// The frame-wise paths are up to eleven launches on two streams per call; at the paper's production chunk (8 MB of
+// input) the host cannot issue them as fast as the GPU retires them.  So a call is captured ONCE per tuple of argument
+// pointers into a CUDA graph (fork / join with the normaliser's stream and the programmatic launch edges included) and
+// replayed afterwards: one graph launch per call.  Not used when per-kernel profiling is on, when the caller is itself
+// capturing `st` (the launches then simply go into the caller's graph), or on the legacy default stream.
+constexpr size_t kMaxGraphs = 32;
+template <typename Issue>
+gdn_status_t run_graphed(gdn_plan_t* p, std::vector<const void*> key, cudaStream_t st, Issue&& issue) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (p->prof.enabled() || st == nullptr || cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return issue();
+    }
+    if (!p->graph_warm) { p->graph_warm = true; return issue(); }
+    for (auto& g : p->graphs)
+        if (g.key == key) {
+            g.used = ++p->graph_tick;
+            cudaError_t e = cudaGraphLaunch(g.exec, st);
+            return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "graph launch");
+        }
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return issue(); }
+    const gdn_status_t is = issue();
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ee = cudaStreamEndCapture(st, &graph);
+    if (is != GDN_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return is; }
+    if (ee != cudaSuccess || !graph) { cudaGetLastError(); return issue(); }       // not capturable here: issue directly
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ie = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ie != cudaSuccess || !exec) { cudaGetLastError(); return issue(); }
+    if (p->graphs.size() >= kMaxGraphs) {                                            // evict the least recently used
+        size_t lru = 0;
+        for (size_t i = 1; i < p->graphs.size(); ++i) if (p->graphs[i].used < p->graphs[lru].used) lru = i;
+        cudaGraphExecDestroy(p->graphs[lru].exec);
+        p->graphs.erase(p->graphs.begin() + (long)lru);
+    }
+    gdn_plan::GraphEntry ge;
+    ge.key = std::move(key); ge.exec = exec; ge.used = ++p->graph_tick;
+    p->graphs.push_back(std::move(ge));
+    const cudaError_t le = cudaGraphLaunch(exec, st);
+    return le == cudaSuccess ? GDN_OK : cuda_fail(p, le, "graph launch");
+}
+
+inline uint32_t __float_as_uint_host(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+
+bool graphable(const gdn_plan_t* p) { return p->path == GDN_PATH_TC_FRAME && p->cfg.T > 0 && p->cfg.B > 0 && p->cfg.H > 0; }
 
 // ---- front end ----------------------------------------------------------------------------------------
 gdn_status_t fe_check(gdn_plan_t* p) {
@@ -381,8 +434,10 @@ gdn_status_t gdn_forward_chunk(gdn_plan_t* plan, const void* q, const void* k, c
     if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
     if (plan->cfg.flags & GDN_FLAG_NORMALIZER)
         return fail(plan, GDN_ERR_INVALID_ARG, "plan carries GDN_FLAG_NORMALIZER: call gdn_forward_chunk_norm");
-    return forward_impl(plan, q, k, v, nullptr, nullptr, alpha, beta, state_in, nullptr, out, state_out, nullptr,
-                        static_cast<cudaStream_t>(stream), false);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    auto issue = [&]() { return forward_impl(plan, q, k, v, nullptr, nullptr, alpha, beta, state_in, nullptr, out, state_out, nullptr, st, false); };
+    if (!graphable(plan)) return issue();
+    return run_graphed(plan, {(const void*)1, q, k, v, alpha, beta, state_in, out, state_out}, st, issue);
 }
 
 gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan, const void* q_rot, const void* k_rot, const void* v,
@@ -392,8 +447,10 @@ gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan, const void* q_rot, const v
     if (!plan) return fail(nullptr, GDN_ERR_INVALID_ARG, "plan is NULL");
     if (!(plan->cfg.flags & GDN_FLAG_NORMALIZER))
         return fail(plan, GDN_ERR_INVALID_ARG, "plan was not created with GDN_FLAG_NORMALIZER");
-    return forward_impl(plan, q_rot, k_rot, v, q_raw, k_raw, alpha, beta, S_in, z_in, out, S_out, z_out,
-                        static_cast<cudaStream_t>(stream), true);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    auto issue = [&]() { return forward_impl(plan, q_rot, k_rot, v, q_raw, k_raw, alpha, beta, S_in, z_in, out, S_out, z_out, st, true); };
+    if (!graphable(plan)) return issue();
+    return run_graphed(plan, {(const void*)2, q_rot, k_rot, v, q_raw, k_raw, alpha, beta, S_in, z_in, out, S_out, z_out}, st, issue);
 }
 
 
@@ -455,10 +512,19 @@ gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* 
     }
     s = featmap_fill(plan, fm, fb, fb + feat, fb + 2 * feat, fb + 3 * feat, fmp, fm_on);
     if (s != GDN_OK) return s;
-    s = launch_frontend(plan, fm_on ? &fmp : nullptr, g_on ? &gtp : nullptr, st, false);
-    if (s != GDN_OK) return s;
-    return forward_impl(plan, fb, fb + feat, v, fb + 2 * feat, fb + 3 * feat, alpha, beta, S_in, z_in, out, S_out, z_out, st, true,
-                        out_gate, true);
+    auto issue = [&]() {
+        gdn_status_t r = launch_frontend(plan, fm_on ? &fmp : nullptr, g_on ? &gtp : nullptr, st, false);
+        if (r != GDN_OK) return r;
+        return forward_impl(plan, fb, fb + feat, v, fb + 2 * feat, fb + 3 * feat, alpha, beta, S_in, z_in, out, S_out, z_out, st, true,
+                            out_gate, true);
+    };
+    std::vector<const void*> key = {(const void*)3, fm->q, fm->k, fm->rms_wq, fm->rms_wk, fm->rope_cos, fm->rope_sin, v, alpha, beta, out_gate,
+                                    S_in, z_in, out, S_out, z_out};
+    key.push_back(reinterpret_cast<const void*>((uintptr_t)__float_as_uint_host(fm->rms_eps)));
+    if (gates) for (const void* g : {gates->x, (const void*)gates->w_alpha, (const void*)gates->b_alpha, (const void*)gates->a_log,
+                                     (const void*)gates->w_beta, (const void*)gates->b_beta, reinterpret_cast<const void*>((uintptr_t)gates->x_token_stride)})
+        key.push_back(g);
+    return run_graphed(plan, std::move(key), st, issue);
 }
 
 gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const void* k_host, const void* v_host,
@@ -581,6 +647,7 @@ gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan, const void* q_host, const 
 }
 
 gdn_status_t gdn_destroy(gdn_plan_t* plan) {
+    if (plan) { for (auto& g : plan->graphs) if (g.exec) cudaGraphExecDestroy(g.exec); plan->graphs.clear(); }
     if (plan) { if (plan->fe_feat) cudaFree(plan->fe_feat); if (plan->fe_gates) cudaFree(plan->fe_gates); plan->fe_feat = nullptr; plan->fe_gates = nullptr; }
     if (!plan) return GDN_OK;
     gdn::tc_plan_free(plan->tc);
