@@ -103,7 +103,8 @@ constexpr uint32_t C_OFF_GAM = C_OFF_SB + 2 * kTile;  // gamma of the entry in e
 constexpr uint32_t C_OFF_GH = C_OFF_GAM + 16;         // gamma of every entry done (replayed for the flag payloads), up to 1024 entries
 
 // ---------------------------------------------------------------------------------------------------
-// chain CTA.  Thread (warp w, lane l < 16) owns state row m = 16 w + l (the TMEM lanes of an M = 64 accumulator).
+// chain CTA.  Warp w owns state rows 16 w .. 16 w + 15 (the TMEM lanes of an M = 64 accumulator), spread over all of its
+// 32 threads in the 16x256b fragment layout: 32 state values per thread, no idle lanes.
 // The CTA walks a list of ENTRIES (G, N, gamma): the chunks of its segment and, for P, the maps of the segments 1..NS-1
 // behind them (level 2).  Before entry e the bf16 operand buffer holds the state that entry e acts on; it is stored as
 // the snapshot of that entry.  The chores of a step are spread over three warps so that none of them delays its warp's share
@@ -119,8 +120,8 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     else { const int u = unit - BH; bh = u / (2 * (NS - 1)); const int r = u % (2 * (NS - 1)); k = 1 + (r >> 1); type = 1 + (r & 1); }
     const int c_lo = f64_seg_lo(fp.L0, fp.L1, k), c_hi = min(c_lo + (k == 0 ? fp.L0 : fp.L1), NC);
     const int nchunk = c_hi - c_lo, n = nchunk + (type == 0 ? NS - 1 : 0);
-    const int m = 16 * warp + lane;
-    const bool act = lane < 16, add_g = type == 2;
+    const int r0 = 16 * warp + (lane >> 2), r1 = r0 + 8, qd = lane & 3;
+    const bool add_g = type == 2;
     const uint32_t aSt = smem_u32(smem), aSb = smem_u32(smem + C_OFF_SB), aGam = smem_u32(smem + C_OFF_GAM);
     uint64_t *full = &bars[0], *bar_mma = &bars[2];
     const unsigned int ep = fp.epoch;
@@ -133,22 +134,30 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
     auto e_snap_z = [&](int e) { return e < nchunk ? (add_g ? fp.zGA : fp.zSc) + (int)cb + c_lo + e : fp.zSk + (int)sb + (e - nchunk + 1); };
     auto e_snap_f = [&](int e) { return e < nchunk ? (add_g ? fp.f_snapA : fp.f_snap) + cb + c_lo + e : fp.f_segS + sb + (e - nchunk + 1); };
 
-    float S[64];
+    // S[4j], S[4j+1] = state (r0, 8j + 2qd + {0,1});  S[4j+2], S[4j+3] = the same columns of row r1 (tmem_ld_16x64's layout)
+    float S[32];
 #pragma unroll
-    for (int j = 0; j < 64; ++j) S[j] = 0.f;
-    if (type == 0 && act && p.S_in) {
-        const float4* src = reinterpret_cast<const float4*>(p.S_in + ((long long)bh * 64 + m) * 64);
+    for (int j = 0; j < 32; ++j) S[j] = 0.f;
+    if (type == 0 && p.S_in) {
+        const float* s0 = p.S_in + ((long long)bh * 64 + r0) * 64 + 2 * qd;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) { const float4 f = __ldcg(src + q); S[4 * q] = f.x; S[4 * q + 1] = f.y; S[4 * q + 2] = f.z; S[4 * q + 3] = f.w; }
+        for (int j = 0; j < 8; ++j) {
+            const float2 a = __ldcg(reinterpret_cast<const float2*>(s0 + 8 * j)), b = __ldcg(reinterpret_cast<const float2*>(s0 + 8 * 64 + 8 * j));
+            S[4 * j] = a.x; S[4 * j + 1] = a.y; S[4 * j + 2] = b.x; S[4 * j + 3] = b.y;
+        }
     }
-    float gacc = 1.f;                                 // gamma accumulated over the entries done so far
-    auto publish = [&](int buf) {                     // bf16 copy of the state rows -> MN-major B operand `buf`
-        if (act) {
-            const uint32_t base = aSb + buf * kTile;
+    // byte offset, inside a swizzled bf16 [64][64] tile, of this thread's column pair in 8-column block j of row r0 / r1;
+    // the eight rows of a warp's access hit eight different 16-byte slots: no bank conflicts
+    uint32_t o0[8], o1[8];
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-                st_shared_v4(base + swz_chunk_off(m, c, 0), pack_bf16(S[8 * c], S[8 * c + 1]), pack_bf16(S[8 * c + 2], S[8 * c + 3]),
-                             pack_bf16(S[8 * c + 4], S[8 * c + 5]), pack_bf16(S[8 * c + 6], S[8 * c + 7]));
+    for (int j = 0; j < 8; ++j) { o0[j] = swz_chunk_off(r0, j, 0) + 4 * qd; o1[j] = swz_chunk_off(r1, j, 0) + 4 * qd; }
+    float gacc = 1.f;                                 // gamma accumulated over the entries done so far
+    auto publish = [&](int buf) {                     // bf16 copy of the state -> MN-major B operand `buf`
+        const uint32_t base = aSb + buf * kTile;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            sts_b32(base + o0[j], pack_bf16(S[4 * j], S[4 * j + 1]));
+            sts_b32(base + o1[j], pack_bf16(S[4 * j + 2], S[4 * j + 3]));
         }
         fence_proxy_async();
     };
@@ -219,27 +228,27 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
             }
         }
         const float gamma = lds_f32(aGam + st * 4);
-        if (act) {                                    // state-independent half, while the MMA runs
+        {                                             // state-independent half, while the MMA runs
             const uint32_t src = aSt + st * C_STAGE + (add_g ? 0u : kTile);
             const float w = add_g ? gacc : 1.f;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                float f[8];
-                unpack8(ld_shared_v4(src + swz_chunk_off(m, c, 0)), f);
-#pragma unroll
-                for (int j = 0; j < 8; ++j) S[8 * c + j] = fmaf(gamma, S[8 * c + j], w * f[j]);
+            for (int j = 0; j < 8; ++j) {
+                const uint32_t a = lds_b32(src + o0[j]), b = lds_b32(src + o1[j]);
+                S[4 * j] = fmaf(gamma, S[4 * j], w * bf16lo(a));
+                S[4 * j + 1] = fmaf(gamma, S[4 * j + 1], w * bf16hi(a));
+                S[4 * j + 2] = fmaf(gamma, S[4 * j + 2], w * bf16lo(b));
+                S[4 * j + 3] = fmaf(gamma, S[4 * j + 3], w * bf16hi(b));
             }
         }
         if (tid == 32 && e < 1024) sts_f32(aGam + 16 + e * 4, gamma);
         gacc *= gamma;
         mbar_wait(bar_mma, (uint32_t)e & 1u);
         tc_fence_after();
+        {
+            float v[32];
+            tmem_ld_16x64(tmem_addr(tmem, warp * 32, 0), v);
 #pragma unroll
-        for (int hc = 0; hc < 4; ++hc) {
-            float v[16];
-            tmem_ld16(tmem_addr(tmem, warp * 32, hc * 16), v);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) S[hc * 16 + j] -= v[j];
+            for (int j = 0; j < 32; ++j) S[j] -= v[j];
         }
         tc_fence_before();
         publish((e + 1) & 1);
@@ -260,10 +269,13 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, uint32_t tmem, uint64_
             st_release64((add_g ? fp.f_segA : fp.f_segB) + sb + k, flag_word(ep, gacc));
         }
     }
-    if (type == 0 && act && p.S_out) {
-        float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * 64 + m) * 64);
+    if (type == 0 && p.S_out) {
+        float* d0 = p.S_out + ((long long)bh * 64 + r0) * 64 + 2 * qd;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) dst[q] = make_float4(S[4 * q], S[4 * q + 1], S[4 * q + 2], S[4 * q + 3]);
+        for (int j = 0; j < 8; ++j) {
+            *reinterpret_cast<float2*>(d0 + 8 * j) = make_float2(S[4 * j], S[4 * j + 1]);
+            *reinterpret_cast<float2*>(d0 + 8 * 64 + 8 * j) = make_float2(S[4 * j + 2], S[4 * j + 3]);
+        }
     }
 }
 

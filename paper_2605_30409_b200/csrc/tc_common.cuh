@@ -236,6 +236,24 @@ __device__ __forceinline__ void tmem_ldw2(uint32_t ta, uint32_t tb, float (&va)[
 __device__ __forceinline__ void tmem_ldw2(uint32_t ta, uint32_t tb, float (&va)[16], float (&vb)[16]) { tmem_ld16x2(ta, tb, va, vb); }
 
 // TMEM address = (lane << 16) | column
+// 16 TMEM lanes x 64 fp32 columns spread over ALL 32 threads of the warp (shape .16x256b, eight 8-column blocks): thread t
+// gets, for block j, v[4j], v[4j+1] = row t/4, columns 8j + 2(t%4) + {0,1} and v[4j+2], v[4j+3] = row t/4 + 8, same columns
+// (the C-fragment layout of mma.m16n8).  An M = 64 accumulator keeps its rows in lanes 0..15 of each quadrant: with this
+// shape no thread of the warp idles in its epilogue.
+__device__ __forceinline__ void tmem_ld_16x64(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.16x256b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];\n\t"
+        "tcgen05.wait::ld.sync.aligned;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ uint32_t lds_b32(uint32_t a) { uint32_t v; asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ float bf16lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
 __device__ __forceinline__ uint32_t tmem_addr(uint32_t base, uint32_t lane, uint32_t col) { return base + (lane << 16) + col; }
 
 // ----------------------------------------------------------------------------------------- descriptors
