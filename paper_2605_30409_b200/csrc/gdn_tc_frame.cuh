@@ -144,9 +144,28 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     if (warp == 5) {
         // ===== TMA producer =====
         if (elect_one()) {
+            // The ring holds what fits in shared memory (three tiles); the DRAM latency of a tile (~3500 cycles measured from
+            // issue to arrival with the ring alone) is taken earlier, by an L2 prefetch kPF tiles ahead of the load.
+            constexpr int kPF = 3;
+            auto prefetch = [&](int i) {
+                const int n0 = (tile_lo + i) * 128;
+                if (j == 0) {                     // the column CTAs of a frame read the same K: one of them prefetches it
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) tma_prefetch_5d(&tmK, nb * 64, h, n0, f, b);
+                }
+                if (zp) return;
+                if (NC == 1) {
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) tma_prefetch_5d(&tmV, nb * 64, h, n0, f, b);
+                } else {
+                    tma_prefetch_5d(&tmV, j * 64, h, n0, f, b);
+                }
+            };
+            for (int i = STAGES; i < min(ntiles, STAGES + kPF); ++i) prefetch(i);
             for (int i = 0; i < ntiles; ++i) {
                 const int st = i % STAGES;
                 if (i >= STAGES) mbar_wait(&bar_empty[st], (uint32_t)((i / STAGES) - 1) & 1u);
+                if (i + kPF < ntiles && i >= STAGES) prefetch(i + kPF);
                 uint8_t* base = smem + st * L::STAGE;
                 mbar_expect_tx(&bar_full[st], zp ? L::KTILE : L::STAGE);
                 const int n0 = (tile_lo + i) * 128;
@@ -198,18 +217,20 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
             mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
             const uint32_t src = smem_u32(smem + st * L::STAGE) + (uint32_t)row * 128u;
             const uint32_t dst = smem_u32(sSc + sb * L::KTILE) + (uint32_t)row * 128u;
+            const Bf16Scale bs = bf16_scale(bt);
 #pragma unroll
             for (int blk = 0; blk < NB; ++blk) {
+                // the scale is per row, so the copy keeps every 16-byte chunk where the swizzle put it; rotating
+                // the chunk order by the row index keeps the 8 lanes of a quarter-warp on distinct banks.  All eight
+                // loads of a block are issued before the first use (the asm loads are not reordered by the compiler:
+                // one load at a time left the warp, alone on its scheduler, waiting out every shared-memory latency).
+                uint4 x[8];
 #pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    // the scale is per row, so the copy keeps every 16-byte chunk where the swizzle put it; rotating
-                    // the chunk order by the row index keeps the 8 lanes of a quarter-warp on distinct banks
-                    const uint32_t off = blk * kBlk + (uint32_t)(((c + row) & 7) << 4);
-                    float x[8];
-                    unpack8(ld_shared_v4(src + off), x);
-                    st_shared_v4(dst + off, pack_bf16(x[0] * bt, x[1] * bt), pack_bf16(x[2] * bt, x[3] * bt),
-                                 pack_bf16(x[4] * bt, x[5] * bt), pack_bf16(x[6] * bt, x[7] * bt));
-                }
+                for (int c = 0; c < 8; ++c) x[c] = ld_shared_v4(src + blk * kBlk + (uint32_t)(((c + row) & 7) << 4));
+#pragma unroll
+                for (int c = 0; c < 8; ++c)
+                    st_shared_v4(dst + blk * kBlk + (uint32_t)(((c + row) & 7) << 4), bf16x2_scale(x[c].x, bs), bf16x2_scale(x[c].y, bs),
+                                 bf16x2_scale(x[c].z, bs), bf16x2_scale(x[c].w, bs));
             }
             fence_proxy_async();
             __syncwarp();

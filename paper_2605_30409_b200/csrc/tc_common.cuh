@@ -361,6 +361,22 @@ __device__ __forceinline__ void unpack8(const uint4& u, float (&f)[8]) {
 }
 
 // ---------------------------------------------------------- small shared-memory stores, warp-level MMA
+// Row scaling of bf16 data without leaving bf16x2: the fp32 factor s is split into two bf16 terms (s = hi + lo + O(2^-17 s)),
+// x * s = fma(x, hi, x * lo) with one rounding of the sum: the correctly rounded bf16 product of x and the fp32 factor up to
+// 2^-17 relative before the final rounding, in two packed instructions per pair (unpack, two FMULs and a pack cost five).
+struct Bf16Scale { uint32_t hi2, lo2; };
+__device__ __forceinline__ Bf16Scale bf16_scale(float s) {
+    const __nv_bfloat16 h = __float2bfloat16_rn(s);
+    const __nv_bfloat16 l = __float2bfloat16_rn(s - __bfloat162float(h));
+    const uint32_t hu = __bfloat16_as_ushort(h), lu = __bfloat16_as_ushort(l);
+    return Bf16Scale{hu | (hu << 16), lu | (lu << 16)};
+}
+__device__ __forceinline__ uint32_t bf16x2_scale(uint32_t x, const Bf16Scale& s) {
+    uint32_t t, r;
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(t) : "r"(x), "r"(s.lo2));
+    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(s.hi2), "r"(t));
+    return r;
+}
 __device__ __forceinline__ void sts_b16(uint32_t a, unsigned short v) { asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory"); }
 
 __device__ __forceinline__ void sts_b32(uint32_t a, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
