@@ -462,12 +462,11 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
     if (prof) prof->begin(st);
     cudaError_t le;
-    if (pdl_first) {       // the front-end kernel precedes in the stream: its tail overlaps this kernel's prologue
-        le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
-        if (le != cudaSuccess) return le;
-    } else {
-        gdn_frm_summaries<D><<<tp.BH * tp.F * tp.NSPLIT * sum_nc<D>(), kSumThreads, smem1, st>>>(tmK, tmV, fp);
-    }
+    // Launched as a programmatic dependent of whatever precedes it in the stream (the front-end kernel, the readout of the
+    // previous call): the kernel waits for that grid before its first global access, only its prologue overlaps.
+    (void)pdl_first;
+    le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_summaries");
     const int nchain = tp.BH * (D / 64);
     if (tp.bidir && tp.F > 1) {

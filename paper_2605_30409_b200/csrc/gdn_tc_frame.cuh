@@ -451,14 +451,26 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    pdl_wait();                                    // the chain's state snapshots are complete
+    pdl_launch_dependents();                       // the next kernel in the stream (Phase A of the next call) may set itself up
+    if (warp != 5) pdl_wait();                     // the chain's state snapshots (and the z pass's den) are complete
 
     if (warp == 5) {
-        // ===== TMA producer: Q tiles through the ring, S_f whenever the frame changes =====
+        // ===== TMA producer: Q tiles through the ring, S_f whenever the frame changes.  Q does not come from the previous
+        //       kernel: the ring is filled before waiting for it =====
         if (elect_one()) {
+            auto load_q = [&](int t, int i) {
+                const int bhf = t / p.TPF, tile = t % p.TPF;
+                const int f = bhf % p.F, bh = bhf / p.F;
+                const int st = i % QST;
+                mbar_expect_tx(&q_full[st], L::Q_BYTES);
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+            };
+            for (int i = 0; i < QST && t_lo + i < t_hi; ++i) load_q(t_lo + i, i);
+            pdl_wait();
             int cur = -1, ns = 0;
             for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
-                const int bhf = t / p.TPF, tile = t % p.TPF;
+                const int bhf = t / p.TPF;
                 const int f = bhf % p.F, bh = bhf / p.F;
                 if (bhf != cur) {
                     const int sb = ns & 1;
@@ -468,11 +480,10 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     for (int nb = 0; nb < NB; ++nb) tma_load_3d(sS + sb * L::S_BYTES + nb * (D * 128), &tmSc, &s_full[sb], nb * 64, 0, bh * p.NSc + f + 1);
                     cur = bhf; ++ns;
                 }
-                const int st = i % QST;
-                if (i >= QST) mbar_wait(&q_empty[st], (uint32_t)((i / QST) - 1) & 1u);
-                mbar_expect_tx(&q_full[st], L::Q_BYTES);
-#pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+                if (i >= QST) {
+                    mbar_wait(&q_empty[i % QST], (uint32_t)((i / QST) - 1) & 1u);
+                    load_q(t, i);
+                }
             }
         }
     } else if (warp == 4) {

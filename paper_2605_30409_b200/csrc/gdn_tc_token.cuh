@@ -826,7 +826,11 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     pdl_launch_dependents();
-    pdl_wait();                                    // the summaries of the previous kernel are complete
+    // Only the summaries (G, N, gamma) come from the previous kernel: the TMA producer waits for it before its first load and
+    // the state rows before they read gamma.  The carried state S_in is older than that (the previous call's kernels are
+    // complete before this call's first kernel passes its own wait), so its load and the first operand copy overlap the
+    // previous kernel's tail.
+    if (warp >= 4) pdl_wait();
 
     auto ent = [&](int c) { return p.rev ? p.NCa - 1 - c : c; };      // summary entry of step c / snapshot slot of state c
     auto issue_loads = [&](int c) {
@@ -869,7 +873,7 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
                              pack_bf16(S[8 * ch + 4], S[8 * ch + 5]), pack_bf16(S[8 * ch + 6], S[8 * ch + 7]));
         }
     };
-    if (worker) publish_smem(0);
+    if (worker) { publish_smem(0); pdl_wait(); }
     fence_proxy_async();
     tc_fence_before();
     __syncthreads();
