@@ -328,7 +328,7 @@ gdn_status_t gates_fill(gdn_plan_t* p, const gdn_gate_args_t* a, float* alpha_ou
     return GDN_OK;
 }
 
-// ONE launch for whichever parts are active: blocks [0, n_fm) feature map, then B*H*F*NSPL gate blocks
+// ONE launch for whichever parts are active: B*H*F*NSPL gate blocks, then the feature-map blocks
 gdn_status_t launch_frontend(gdn_plan_t* p, const gdn::FeatmapParams* fm, const gdn::GateParams* gp, cudaStream_t st, bool mark) {
     int n_fm = 0, n_g = 0;
     if (fm) {
@@ -341,7 +341,7 @@ gdn_status_t launch_frontend(gdn_plan_t* p, const gdn::FeatmapParams* fm, const 
     if (n_fm + n_g == 0) return GDN_OK;
     gdn::GateParams g0{};
     g0.NSPL = 1;
-    gdn::fe::gdn_frontend_kernel<<<n_fm + n_g, gdn::fe::kFeThreads, 0, st>>>(fm ? *fm : gdn::FeatmapParams{}, gp ? *gp : g0, n_fm);
+    gdn::fe::gdn_frontend_kernel<<<n_fm + n_g, gdn::fe::kFeThreads, 0, st>>>(fm ? *fm : gdn::FeatmapParams{}, gp ? *gp : g0, n_g);
     if (mark) p->prof.mark(st, "gdn_frontend_kernel");
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? GDN_OK : cuda_fail(p, e, "gdn_frontend_kernel launch");
