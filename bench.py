@@ -431,7 +431,7 @@ def kernel_bytes(name, wl, by_call):
         "gdn_frm_readout": th * (wl.d_k + wl.d_v) * es,
         "gdn_frontend_kernel": th * 7 * wl.d_k * es,      # q, k read; q_rot, k_rot, q_raw, k_raw written
     }
-    if name.startswith("gdn_tok_chain") or name == "gdn_frm_hist_add":
+    if name.startswith("gdn_tok_chain"):
         return 2 * st                              # the scans only carry the state in and out; their summaries are workspace
     return table.get(name, by_call)               # single-kernel paths: the whole call
 

@@ -204,7 +204,7 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
 
 
 
-// The frame-wise paths are up to eleven launches on two streams per call; at the paper's production chunk (8 MB of
+// The frame-wise paths are up to seven launches on two streams per call; at the paper's production chunk (8 MB of
 // input) the host cannot issue them as fast as the GPU retires them.  So a call is captured ONCE per tuple of argument
 // pointers into a CUDA graph (fork / join with the normaliser's stream and the programmatic launch edges included) and
 // replayed afterwards: one graph launch per call.  Not used when per-kernel profiling is on, when the caller is itself
@@ -414,7 +414,6 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
                 if (ts != GDN_OK) { gdn::tc_plan_free(p->tc); delete p; return fail(nullptr, ts, msg); }
             }
             // frame path: + S^hist kernel with the bidirectional scan (F > 1); the normaliser runs all of it twice
-            if (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_BIDIR) && c.T / c.group > 1) launches += 1;
             p->path = path; p->chunk = chunk; p->launches = (c.flags & GDN_FLAG_NORMALIZER) ? 2 * launches : launches;
             p->workspace_bytes = p->tc.workspace_bytes;
         }

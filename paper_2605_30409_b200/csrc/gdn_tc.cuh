@@ -56,6 +56,7 @@ struct TcPlan {
     // bidirectional in-chunk scan: reverse-scan snapshots S<_f, bf16 [BH][F][D][D]
     bool bidir = false;
     __nv_bfloat16* ScR = nullptr;
+    unsigned int* hist_cnt = nullptr;
     CUtensorMap tmScR;
     const void *cqr = nullptr, *ckr = nullptr;
     CUtensorMap tmQr, tmKr;
@@ -127,6 +128,7 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     const size_t oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
     tp.bidir = (c.flags & GDN_FLAG_BIDIR) != 0;
     const size_t oScR = tp.bidir ? carve(BH * F * D * D * 2) : 0;
+    const size_t oHc = tp.bidir ? carve(BH * 2 * 4) : 0;        // (forward, reverse) arrival counters per (b, h, column tile)
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -142,6 +144,10 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
     if (norm) tp.den = reinterpret_cast<float*>(w + oDen);
     if (tp.bidir) tp.ScR = reinterpret_cast<__nv_bfloat16*>(w + oScR);
+    if (tp.bidir) {
+        tp.hist_cnt = reinterpret_cast<unsigned int*>(w + oHc);
+        if (cudaMemset(tp.hist_cnt, 0, BH * 2 * 4) != cudaSuccess) { cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
+    }
     if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "counter initialisation failed";
@@ -468,21 +474,21 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_summaries");
-    const int nchain = tp.BH * (D / 64);
+    const int nchain = tp.BH * (cp.col_tiles ? cp.col_tiles : D / 64);
     if (tp.bidir && tp.F > 1) {
         // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero
         // state; then S^hist = S> + S< in place in the forward snapshots
         TokParams rp = cp;
         rp.rev = 1; rp.NCa = tp.F; rp.NC = tp.F - 1; rp.NSc = tp.F; rp.S_in = nullptr; rp.S_out = nullptr;
         rp.z_vec_in = nullptr; rp.z_vec_out = nullptr;              // z< starts from zero as well and is not carried
-        le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScR, cp, rp, nchain);
+        TokParams fwd = cp;
+        fwd.hist_cnt = rp.hist_cnt = tp.hist_cnt;
+        fwd.hist_dst = rp.hist_dst = tp.Sc;
+        fwd.hist_src = rp.hist_src = tp.ScR;
+        fwd.hist_F = rp.hist_F = tp.F;
+        le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScR, fwd, rp, nchain);
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_tok_chain_bidir");
-        const long long total8 = (long long)tp.BH * tp.F * D * D / 8;
-        const int blocks = (int)((total8 + 255) / 256 < 4 * sms ? (total8 + 255) / 256 : 4 * sms);
-        le = launch_pdl(gdn_frm_hist_add, dim3(blocks), dim3(256), 0, st, tp.Sc, (const __nv_bfloat16*)tp.ScR, tp.F, D * D / 8, total8);
-        if (le != cudaSuccess) return le;
-        if (prof) prof->mark(st, "gdn_frm_hist_add");
     } else {
         le = launch_pdl(tok::gdn_tok_chain<D>, dim3(nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, cp);
         if (le != cudaSuccess) return le;
@@ -550,6 +556,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             zc.Gw = zt.Gw; zc.Nw = zt.Nw; zc.gam = zt.gam; zc.Sc = zt.Sc;
             zc.S_in = nullptr; zc.S_out = nullptr;
             zc.zvec = 1; zc.z_vec_in = na->z_in; zc.z_vec_out = na->z_out;      // z <-> column 0 of the state, in the chain kernel
+            zc.col_tiles = 1;                        // ... so only the first 64-column tile is run (the readout uses column 0 only)
             e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr)
                              : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr);
             if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);

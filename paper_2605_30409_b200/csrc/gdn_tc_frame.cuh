@@ -11,6 +11,8 @@
 //                                data, no separate reduction launch.
 //   Phase B  gdn_tok_chain     : S_f = alpha_f S_{f-1} - G_f S_{f-1} + N_f  -- the same one-MMA-per-step chain
 //                                kernel as the token-wise path (Eq. 5: S_f = alpha_f (I - Gram_f) S_{f-1} + A_f)
+//   (bidirectional scan, Alg. 1 l.9-21: forward and reverse scan in ONE launch, gdn_tok_chain_bidir; the CTA of a pair that
+//    finishes last adds S<_f into the forward snapshot S>_f in place, so Phase C reads S^hist with no second output pass, L122)
 //   Phase C  gdn_frm_readout   : O_f = scale * Q_f S_f  (every token of frame f reads the post-update state, Eq. 22)
 //                                persistent CTAs over contiguous tile ranges: TMA ring for Q, S_f reloaded only when
 //                                the frame changes, two TMEM accumulators, bf16 tiles leave by TMA store.
@@ -373,31 +375,6 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, NW);
-}
-
-// ---------------------------------------------------------------------------------------------------
-// Bidirectional in-chunk scan (Alg. 1 l.19-21): S^hist_f = S>_f + S<_f.  The forward snapshot of frame f (slot f + 1
-// of Sc, bf16) takes the reverse scan's S<_f (slot f of ScR) in place, so Phase C reads the summed history with no
-// second output pass.  8 bf16 per thread and step.
-// ---------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-gdn_frm_hist_add(__nv_bfloat16* Sc, const __nv_bfloat16* ScR, int F, int DD8, long long total8) {
-    pdl_launch_dependents();
-    pdl_wait();                                    // both scans are complete
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total8; e += (long long)gridDim.x * blockDim.x) {
-        const long long bhf = e / DD8;
-        const int within = (int)(e % DD8), f = (int)(bhf % F);
-        const long long bh = bhf / F;
-        uint4* dst = reinterpret_cast<uint4*>(Sc) + (bh * (F + 1) + f + 1) * DD8 + within;
-        const uint4 r = __ldcg(reinterpret_cast<const uint4*>(ScR) + bhf * DD8 + within);
-        const uint4 a = __ldcg(dst);
-        float x[8], y[8];
-        unpack8(a, x); unpack8(r, y);
-        uint4 o;
-        o.x = pack_bf16(x[0] + y[0], x[1] + y[1]); o.y = pack_bf16(x[2] + y[2], x[3] + y[3]);
-        o.z = pack_bf16(x[4] + y[4], x[5] + y[5]); o.w = pack_bf16(x[6] + y[6], x[7] + y[7]);
-        *dst = o;
-    }
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -49,9 +49,17 @@ struct TokParams {
     int zvec;
     const float* z_vec_in;
     float* z_vec_out;
+    int col_tiles;               // chain kernel: 64-column tiles of the state that are run (0 = all D / 64; the z pass runs tile 0 only)
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
+    // chain kernel, bidirectional frame path (Alg. 1 l.19-21): S^hist_f = S>_f + S<_f.  The forward and the reverse CTA of a
+    // (b, h, column tile) count themselves in hist_cnt; the one that finishes last adds the reverse snapshots hist_src
+    // [BH][hist_F][D][D] into the forward ones hist_dst [BH][hist_F + 1][D][D] (slot f + 1) for its 64 columns.  NULL = off.
+    unsigned int* hist_cnt;
+    __nv_bfloat16* hist_dst;
+    const __nv_bfloat16* hist_src;
+    int hist_F;
 };
 
 
@@ -806,7 +814,7 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + STAGES + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    constexpr int NT_COL = D / 64;
+    const int NT_COL = p.col_tiles ? p.col_tiles : D / 64;
     const int ct = cta % NT_COL, bh = cta / NT_COL;
     const int n0 = ct * 64;
     const bool worker = warp < 4;
@@ -913,7 +921,10 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
                 if (c + STAGES < p.NC) issue_loads(c + STAGES);
             }
         }
-        if (lane == 0) tma_store_wait_read();        // the snapshots have left shared memory; their writes complete with the kernel
+        if (lane == 0) {
+            if (p.hist_cnt) { tma_store_wait_all(); __threadfence(); }     // the snapshots are in global memory (read again below)
+            else tma_store_wait_read();              // the snapshots have left shared memory; their writes complete with the kernel
+        }
     } else {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
         uint32_t ph_mma = 0;
@@ -959,6 +970,48 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
 #pragma unroll
             for (int i = 0; i < 16; ++i)
                 if (n0 + 4 * i < p.dr) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+        }
+    }
+    if (p.hist_cnt) {
+        // sum of the two scans' snapshots by whichever CTA of the (forward, reverse) pair finishes last: no separate launch
+        // (the element-wise kernel this replaces took 4-5 us per call, most of it launch and drain)
+        __shared__ unsigned int s_last;
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned int prev = atomicAdd(p.hist_cnt + cta, 1u);
+            s_last = prev == 1u ? 1u : 0u;
+            if (prev == 1u) p.hist_cnt[cta] = 0u;    // ready for the next call (stream order)
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int total = p.hist_F * D * 8;      // 16-byte pieces of this CTA's 64 columns
+            constexpr int UN = 8;                    // pieces per thread and pass: all 2 UN loads in flight before the first use
+            for (int base = tid; base < total; base += UN * kChainThreads) {
+                uint4* dst[UN];
+                uint4 a[UN], r[UN];
+#pragma unroll
+                for (int u = 0; u < UN; ++u) {
+                    const int idx = base + u * kChainThreads;
+                    const bool ok = idx < total;
+                    const int f = ok ? idx / (D * 8) : 0, row = (idx >> 3) % D, c = idx & 7;
+                    dst[u] = ok ? reinterpret_cast<uint4*>(p.hist_dst + (((long long)bh * (p.hist_F + 1) + f + 1) * D + row) * D + n0 + c * 8) : nullptr;
+                    if (ok) {
+                        r[u] = __ldcg(reinterpret_cast<const uint4*>(p.hist_src + (((long long)bh * p.hist_F + f) * D + row) * D + n0 + c * 8));
+                        a[u] = __ldcg(dst[u]);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < UN; ++u) {
+                    if (!dst[u]) continue;
+                    float x[8], y[8];
+                    unpack8(a[u], x); unpack8(r[u], y);
+                    uint4 o;
+                    o.x = pack_bf16(x[0] + y[0], x[1] + y[1]); o.y = pack_bf16(x[2] + y[2], x[3] + y[3]);
+                    o.z = pack_bf16(x[4] + y[4], x[5] + y[5]); o.w = pack_bf16(x[6] + y[6], x[7] + y[7]);
+                    *dst[u] = o;
+                }
+            }
         }
     }
     tc_fence_before();
