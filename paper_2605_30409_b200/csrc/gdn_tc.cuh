@@ -43,6 +43,8 @@ struct TcPlan {
     // per-call activation maps, cached on the pointers they were built for
     const void *cq = nullptr, *ck = nullptr, *cv = nullptr, *co = nullptr;
     CUtensorMap tmQ, tmK, tmV, tmO;
+    CUtensorMap tmGt;                                // output gate (Eq. 23), same tiling as tmO
+    const void* cgate = nullptr;
     // fused single-kernel token path (C = 128): per-tile ready flags and the call epoch
     bool fused = false;
     unsigned int* flags = nullptr;
@@ -495,7 +497,7 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
         if (prof) prof->mark(st, "gdn_tok_chain");
     }
     if (before_readout) { le = cudaStreamWaitEvent(st, before_readout, 0); if (le != cudaSuccess) return le; }   // den of the z pass
-    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp);
+    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp.gate ? tp.tmGt : tp.tmO, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
     return cudaGetLastError();
@@ -563,6 +565,10 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             fp.den = tp.den; fp.den_mode = 2; fp.eps = c.eps;
             fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
+            if (na->gate && na->gate != tp.cgate) {
+                if (!tc::make_act_tmap(&tp.tmGt, na->gate, c.B, c.T, c.H, c.d_v, c.group, fp.g_ts, 128, err)) { tp.cgate = nullptr; return GDN_ERR_CUDA; }
+                tp.cgate = na->gate;
+            }
             den_ready = tp.zev1;
         }
         const bool pdl_first = na && na->dense_qk;

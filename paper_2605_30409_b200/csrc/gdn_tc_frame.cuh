@@ -398,7 +398,7 @@ struct ReadSmem {
 template <int D>
 __global__ void __launch_bounds__(kReadThreads, 1)
 gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmSc,
-                const __grid_constant__ CUtensorMap tmO, const FrmParams p) {
+                const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUtensorMap tmGt, const FrmParams p) {
     using L = ReadSmem<D>;
     constexpr int NB = L::NB, QST = L::QST;
     extern __shared__ uint8_t smem_raw[];
@@ -412,14 +412,15 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* s_empty = s_full + 2;           // [2]   the last MMA that reads this state has completed
     uint64_t* acc_full = s_empty + 2;         // [2]
     uint64_t* acc_empty = acc_full + 2;       // [2]   drained by the 4 epilogue warps
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+    uint64_t* g_full = acc_empty + 2;         // [2]   output-gate tile landed in the staging buffer
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(g_full + 2);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long nt = p.total_tiles;
     const int t_lo = (int)(nt * blockIdx.x / gridDim.x), t_hi = (int)(nt * (blockIdx.x + 1) / gridDim.x);
     if (tid == 0) {
         for (int s = 0; s < QST; ++s) { mbar_init(&q_full[s], 1); mbar_init(&q_empty[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], 1); mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], 1); mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); mbar_init(&g_full[s], 1); }
         mbar_fence_init();
     }
     if (tid == 160) { tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmSc); tma_prefetch_desc(&tmO); }
@@ -490,6 +491,20 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else {
         // ===== epilogue: TMEM -> registers -> scale (/ normaliser) -> bf16 -> swizzled staging -> TMA store =====
         const int row = tid;
+        // Output gate (Eq. 23): the gate tile of a token tile has the layout of the output tile, so it is brought by TMA INTO
+        // the staging buffer the output tile is about to be written to; each thread reads a 16-byte piece of the gate, scales
+        // its accumulator piece and writes the result over it.  (One global load per piece and thread, issued when needed,
+        // put a full memory latency on every tile: +6 us on the paper's chunk.)  The tile after the next is requested as soon
+        // as the store that last used its buffer has read it.
+        const bool gated = p.gate != nullptr;
+        auto load_gate = [&](int t, int i) {
+            const int bhf = t / p.TPF, tile = t % p.TPF;
+            const int f = bhf % p.F, bh = bhf / p.F;
+            mbar_expect_tx(&g_full[i & 1], L::Q_BYTES);
+#pragma unroll
+            for (int nb = 0; nb < NB; ++nb) tma_load_5d(sO + (i & 1) * L::Q_BYTES + nb * kBlk, &tmGt, &g_full[i & 1], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+        };
+        if (gated && tid == 0 && t_lo < t_hi) load_gate(t_lo, 0);
         for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
             const int bhf = t / p.TPF, tile = t % p.TPF;
             const int f = bhf % p.F, bh = bhf / p.F;
@@ -498,8 +513,6 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const long long tok = ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.H + (bh % p.H);   // index into den [B][T][H]
             float mul = p.scale;
             if (p.den_mode == 2 && n < p.G) mul = p.scale / (__ldg(p.den + tok) + p.eps);          // Eq. 22: eps after the dot product, no clamp
-            const __nv_bfloat16* grow = (p.gate && n < p.G)
-                ? p.gate + ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.g_ts + (long long)(bh % p.H) * p.dr : nullptr;
             if (p.den_mode == 1) {
                 // z pass: only column 0 of Q_raw S^z is the normaliser q_raw . z_f; nothing goes to `out`
                 mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
@@ -513,10 +526,18 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 continue;
             }
             // the store that read staging buffer `a` two tiles ago must have finished reading it
-            if (tid == 0) tma_store_wait_read_but1();
+            if (tid == 0) {
+                if (gated) {
+                    tma_store_wait_read();           // ... and the previous tile's store its own: that buffer takes the next gate tile
+                    if (t + 1 < t_hi) load_gate(t + 1, i + 1);
+                } else {
+                    tma_store_wait_read_but1();
+                }
+            }
             mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
             tc_fence_after();
             asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (gated) mbar_wait(&g_full[a], (uint32_t)(i >> 1) & 1u);
             const uint32_t stg = smem_u32(sO + a * L::Q_BYTES);
 #pragma unroll
             for (int cc = 0; cc < D / 32; ++cc) {
@@ -532,9 +553,9 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     float m[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) m[e] = mul;
-                    if (grow && cc * 32 + q4 * 8 < p.dr) {
+                    if (gated) {
                         float gv[8];
-                        unpack8(__ldg(reinterpret_cast<const uint4*>(grow + cc * 32 + q4 * 8)), gv);
+                        unpack8(ld_shared_v4(stg + swz_chunk_off(row, cc * 4 + q4, kBlk)), gv);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) m[e] *= gv[e];
                     }
