@@ -354,7 +354,7 @@ def run_ours(args):
         "tflops": tflops, "pct_bf16_peak": 100 * tflops / pk["bf16_tflops"], "peaks": pk_src,
         "flops": flops_report(wl, info.chunk, ms_per_step, by, pk),
         "hbm_gbs_algorithmic": by / (ms_per_step * 1e-3) / 1e9,
-        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * info.launches_per_call,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps * (info.launches_per_call + (1 if args.full else 0)),      # --full: + the front-end kernel
         "roofline": roof, "kernels": kernels,
     }
     if norm or args.bidir:

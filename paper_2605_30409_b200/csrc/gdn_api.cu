@@ -256,6 +256,8 @@ gdn_status_t fe_check(gdn_plan_t* p) {
     const gdn_config_t& c = p->cfg;
     if (c.io_dtype != GDN_BF16 || c.d_k != c.d_v || c.d_k % 8 != 0 || c.d_k > 128)
         return fail(p, GDN_ERR_UNSUPPORTED, "the front end needs a bf16 plan with d_k = d_v a multiple of 8, at most 128");
+    if ((long long)c.B * c.T * c.H >= (1LL << 31) - 64 * 1024)
+        return fail(p, GDN_ERR_UNSUPPORTED, "the front end indexes (token, head) rows with 32 bits: B*T*H must stay below 2^31");
     gdn_status_t ds = check_device(p);
     if (ds != GDN_OK) return ds;
     int cur = -1;

@@ -67,21 +67,24 @@ constexpr int kFeRows = 2;                 // rows / tokens a 16-lane group has 
 // Feature map of rows r0 + g + 16 j (j < kFeRows) of [B*T*H] (row = one token of one head), grid-stride over row groups.
 __device__ __forceinline__ void featmap_body(const FeatmapParams& p, int block, int nblocks) {
     const int g = threadIdx.x >> 4, l = threadIdx.x & 15;
-    const long long rows = (long long)p.B * p.T * p.H;
-    const int c0 = l * 8;
+    const int rows = p.B * p.T * p.H;           // < 2^31 (checked by the host): 32-bit index arithmetic, the 64-bit
+    const int c0 = l * 8;                       // divisions by H and T were a third of this kernel's instructions
     const bool on = c0 < p.D;
     const float inv_d = 1.f / (float)p.D;
     constexpr int R = kFeRows;
-    for (long long r0 = (long long)block * 16 * R; r0 < rows; r0 += (long long)nblocks * 16 * R) {   // uniform trip count: the
-        float xq[R][8], xk[R][8];                                                                     // shuffles need the whole warp
-        long long rr[R];
+    for (int r0 = block * 16 * R; r0 < rows; r0 += nblocks * 16 * R) {   // uniform trip count: the shuffles need the whole warp
+        float xq[R][8], xk[R][8];
+        int rr[R], hh[R], tt[R];
         bool valid[R];
 #pragma unroll
         for (int j = 0; j < R; ++j) {
             valid[j] = r0 + g + 16 * j < rows;
             rr[j] = valid[j] ? r0 + g + 16 * j : rows - 1;
-            const int h = (int)(rr[j] % p.H);
-            const long long bt = rr[j] / p.H;
+            const unsigned int btu = (unsigned int)rr[j] / (unsigned int)p.H;
+            const int h = rr[j] - (int)btu * p.H;
+            const long long bt = btu;
+            hh[j] = h;
+            tt[j] = (int)(btu % (unsigned int)p.T);
 #pragma unroll
             for (int i = 0; i < 8; ++i) { xq[j][i] = 0.f; xk[j][i] = 0.f; }
             if (on) {
@@ -97,8 +100,7 @@ __device__ __forceinline__ void featmap_body(const FeatmapParams& p, int block, 
             sq = group16_sum(sq);
             sk = group16_sum(sk);
             if (!on || !valid[j]) continue;
-            const int h = (int)(rr[j] % p.H);
-            const int t = (int)((rr[j] / p.H) % p.T);
+            const int h = hh[j], t = tt[j];
             const float rq = rsqrtf(sq * inv_d + p.rms_eps), rk = rsqrtf(sk * inv_d + p.rms_eps);
             const float4 wq0 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0));
             const float4 wq1 = __ldg(reinterpret_cast<const float4*>(p.wq + (long long)h * p.D + c0 + 4));
@@ -122,7 +124,7 @@ __device__ __forceinline__ void featmap_body(const FeatmapParams& p, int block, 
                 ko[2 * i] = kr[2 * i] * cv[i] - kr[2 * i + 1] * sv[i];
                 ko[2 * i + 1] = kr[2 * i] * sv[i] + kr[2 * i + 1] * cv[i];
             }
-            const long long o = rr[j] * p.D + c0;
+            const long long o = (long long)rr[j] * p.D + c0;
             *reinterpret_cast<uint4*>(p.q_raw + o) = pack8f(qr);
             *reinterpret_cast<uint4*>(p.k_raw + o) = pack8f(kr);
             *reinterpret_cast<uint4*>(p.q_rot + o) = pack8f(qo);
