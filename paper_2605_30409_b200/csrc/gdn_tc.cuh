@@ -51,7 +51,6 @@ struct TcPlan {
     unsigned int epoch = 0;
     int HPR = 0, NWC = 0, grid = 0;
     // normaliser on the frame path: z as column 0 of the chain kernel's state, den = q_raw . z per token
-    float* den = nullptr;
     TcPlan* zplan = nullptr;                   // the z pass runs concurrently on its own workspace, stream and events
     cudaStream_t zs = nullptr;
     cudaEvent_t zev0 = nullptr, zev1 = nullptr;
@@ -127,7 +126,6 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     const size_t oP = carve(NS > 1 ? BH * F * NS * D * 2 * D * 4 : 16), oG = carve(BH * F * D * D * 2), oN = carve(BH * F * D * D * 4);
     const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
     const bool norm = (c.flags & GDN_FLAG_NORMALIZER) != 0;
-    const size_t oDen = norm ? carve((size_t)c.B * c.T * c.H * 4) : 0;
     tp.bidir = (c.flags & GDN_FLAG_BIDIR) != 0;
     const size_t oScR = tp.bidir ? carve(BH * F * D * D * 2) : 0;
     const size_t oHc = tp.bidir ? carve(BH * 2 * 4) : 0;        // (forward, reverse) arrival counters per (b, h, column tile)
@@ -144,7 +142,6 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.gam = reinterpret_cast<float*>(w + oGam);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
-    if (norm) tp.den = reinterpret_cast<float*>(w + oDen);
     if (tp.bidir) tp.ScR = reinterpret_cast<__nv_bfloat16*>(w + oScR);
     if (tp.bidir) {
         tp.hist_cnt = reinterpret_cast<unsigned int*>(w + oHc);
@@ -453,7 +450,7 @@ inline cudaError_t tc_launch_fused64(TcPlan& tp, const TokParams& p, cudaStream_
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
                                    const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
-                                   cudaEvent_t before_readout = nullptr, bool pdl_first = false) {
+                                   cudaEvent_t before_readout = nullptr, bool readout = true, const CUtensorMap* tmQr = nullptr) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -472,7 +469,6 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     cudaError_t le;
     // Launched as a programmatic dependent of whatever precedes it in the stream (the front-end kernel, the readout of the
     // previous call): the kernel waits for that grid before its first global access, only its prologue overlaps.
-    (void)pdl_first;
     le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_summaries");
@@ -496,8 +492,10 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_tok_chain");
     }
-    if (before_readout) { le = cudaStreamWaitEvent(st, before_readout, 0); if (le != cudaSuccess) return le; }   // den of the z pass
-    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp.gate ? tp.tmGt : tp.tmO, fp);
+    if (!readout) return cudaGetLastError();       // the z pass ends with its scan: the matrix pass's readout takes z_f from its snapshots
+    if (before_readout) { le = cudaStreamWaitEvent(st, before_readout, 0); if (le != cudaSuccess) return le; }   // the z pass's scan
+    le = launch_pdl(gdn_frm_readout<D>, dim3(grid3), dim3(kReadThreads), smem3, st, tmQ, tp.tmSc, tp.tmO, fp.gate ? tp.tmGt : tp.tmO,
+                    tmQr ? *tmQr : tmQ, fp);
     if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_frm_readout");
     return cudaGetLastError();
@@ -537,9 +535,10 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         cudaError_t e = cudaSuccess;
         cudaEvent_t den_ready = nullptr;
         if (na) {
-            // z pass (Eq. 20-21 through the same three kernels): K_raw summaries with the constant block as V, the scan on
-            // a [D][D] state whose column 0 is z, q_raw . z_f per token -> den.  It shares nothing with the matrix pass
-            // until the division in Phase C, so it runs beside it on its own stream and workspace.
+            // z pass (Eq. 20-21 through the same Phase A and scan kernels): K_raw summaries with the constant block as V, the
+            // scan on a [D][D] state whose column 0 is z (first 64-column tile only).  It shares nothing with the matrix pass
+            // until the division in Phase C, so it runs beside it on its own stream and workspace; Phase C of the matrix pass
+            // takes z_f from its snapshots and forms q_raw . z_f itself.
             TcPlan& zt = *tp.zplan;
             if (na->q_raw != tp.cqr || na->k_raw != tp.ckr) {
                 bool ok = tc::make_act_tmap(&tp.tmQr, na->q_raw, c.B, c.T, c.H, c.d_k, c.group, ts(na->dense_qk ? 0 : c.q_token_stride, c.d_k), 128, err) &&
@@ -547,23 +546,22 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
                 if (!ok) { tp.cqr = tp.ckr = nullptr; return GDN_ERR_CUDA; }
                 tp.cqr = na->q_raw; tp.ckr = na->k_raw;
             }
-            zt.tmO = tp.tmO;                         // unused by the z pass (den_mode 1 stores no tile)
             e = cudaEventRecord(tp.zev0, st);         // after everything queued on the caller's stream so far
             if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
             if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             FrmParams zf = fp;
             zf.part = zt.part; zf.counters = zt.flags; zf.Gw = zt.Gw; zf.Nw = zt.Nw; zf.gam = zt.gam;
-            zf.zpass = 1; zf.den = tp.den; zf.den_mode = 1; zf.scale = 1.f;
+            zf.zpass = 1; zf.scale = 1.f;
             TokParams zc = cp;
             zc.Gw = zt.Gw; zc.Nw = zt.Nw; zc.gam = zt.gam; zc.Sc = zt.Sc;
             zc.S_in = nullptr; zc.S_out = nullptr;
             zc.zvec = 1; zc.z_vec_in = na->z_in; zc.z_vec_out = na->z_out;      // z <-> column 0 of the state, in the chain kernel
             zc.col_tiles = 1;                        // ... so only the first 64-column tile is run (the readout uses column 0 only)
-            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr)
-                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmQr, zf, zc, tp.zs, nullptr);
+            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false)
+                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false);
             if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
             if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
-            fp.den = tp.den; fp.den_mode = 2; fp.eps = c.eps;
+            fp.den_mode = 1; fp.eps = c.eps; fp.z_sc = zt.Sc;
             fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
             if (na->gate && na->gate != tp.cgate) {
                 if (!tc::make_act_tmap(&tp.tmGt, na->gate, c.B, c.T, c.H, c.d_v, c.group, fp.g_ts, 128, err)) { tp.cgate = nullptr; return GDN_ERR_CUDA; }
@@ -571,9 +569,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             }
             den_ready = tp.zev1;
         }
-        const bool pdl_first = na && na->dense_qk;
-        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, pdl_first)
-                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, pdl_first);
+        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr)
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

@@ -41,13 +41,15 @@ struct FrmParams {
     long long o_ts;
     float scale;
     int log_alpha;
-    // normaliser (Eq. 20-22): the vector state z is run through the SAME kernels as column 0 of a matrix state
-    // ("the z path is the matrix path with v = 1", SURVEY pin 13): zpass = 1 replaces V by a constant block whose
-    // column 0 is one, so N_f[:, 0] = K^T beta = b_f and Gram is that of the un-rotated keys.
+    // normaliser (Eq. 20-22): the vector state z is run through the SAME Phase A and scan kernels as column 0 of a
+    // matrix state ("the z path is the matrix path with v = 1", SURVEY pin 13): zpass = 1 replaces V by a constant block whose
+    // column 0 is one, so N_f[:, 0] = K^T beta = b_f and Gram is that of the un-rotated keys.  The readout of the MATRIX pass
+    // forms den = q_raw . z_f itself (den_mode 1): z_f is column 0 of the z pass's state snapshots z_sc, the q_raw tile of a
+    // token tile rides in the last slot of the Q ring, and out = scale Q S / (den + eps).
     int zpass;
-    float* den;                  // [B][T][H] fp32: q_raw . z_f per token
-    int den_mode;                // readout: 0 = plain, 1 = write den (column 0 of Q_raw S^z), 2 = out = scale Q S / (den + eps)
+    int den_mode;                // readout: 0 = plain, 1 = normalised
     float eps;
+    const __nv_bfloat16* z_sc;   // [BH][NSc][D][D] bf16 snapshots of the z pass (slot f + 1 = the state frame f reads)
     // output gate (Eq. 23, the Hadamard product G (.) Y): multiplied in the readout's epilogue, before the
     // bf16 rounding of the tile.  gate [B][T][H][dr] bf16, token stride g_ts; NULL = no gate.
     const __nv_bfloat16* gate;
@@ -392,15 +394,21 @@ struct ReadSmem {
     static constexpr uint32_t OFF_S = QST * Q_BYTES;
     static constexpr uint32_t OFF_O = OFF_S + 2 * S_BYTES;            // 2 x out staging [128][D] bf16
     static constexpr uint32_t OFF_BAR = OFF_O + 2 * Q_BYTES;
-    static constexpr uint32_t TOTAL = OFF_BAR + 512 + 1024;
+    static constexpr uint32_t OFF_Z = OFF_BAR + 512;                  // fp32 z_f [D] (normalised readout)
+    static constexpr uint32_t TOTAL = OFF_Z + 512 + 1024;
 };
 
 template <int D>
 __global__ void __launch_bounds__(kReadThreads, 1)
 gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmSc,
-                const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUtensorMap tmGt, const FrmParams p) {
+                const __grid_constant__ CUtensorMap tmO, const __grid_constant__ CUtensorMap tmGt,
+                const __grid_constant__ CUtensorMap tmQr, const FrmParams p) {
     using L = ReadSmem<D>;
     constexpr int NB = L::NB, QST = L::QST;
+    // normalised readout: the last ring slot holds the q_raw tile of the tile being finished, the Q ring is one slot shorter
+    const bool norm = p.den_mode == 1;
+    const int qst = norm ? QST - 1 : QST;
+    uint8_t* sQr = nullptr;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* sS = smem + L::OFF_S;
@@ -413,7 +421,10 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* acc_full = s_empty + 2;         // [2]
     uint64_t* acc_empty = acc_full + 2;       // [2]   drained by the 4 epilogue warps
     uint64_t* g_full = acc_empty + 2;         // [2]   output-gate tile landed in the staging buffer
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(g_full + 2);
+    uint64_t* qr_full = g_full + 2;           // q_raw tile landed
+    uint64_t* qr_empty = qr_full + 1;         // ... and has been read by the 4 epilogue warps
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(qr_empty + 1);
+    sQr = smem + (QST - 1) * L::Q_BYTES;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long nt = p.total_tiles;
@@ -421,6 +432,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (tid == 0) {
         for (int s = 0; s < QST; ++s) { mbar_init(&q_full[s], 1); mbar_init(&q_empty[s], 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], 1); mbar_init(&acc_full[s], 1); mbar_init(&acc_empty[s], 4); mbar_init(&g_full[s], 1); }
+        mbar_init(qr_full, 1); mbar_init(qr_empty, 4);
         mbar_fence_init();
     }
     if (tid == 160) { tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmSc); tma_prefetch_desc(&tmO); }
@@ -430,7 +442,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     pdl_launch_dependents();                       // the next kernel in the stream (Phase A of the next call) may set itself up
-    if (warp != 5) pdl_wait();                     // the chain's state snapshots (and the z pass's den) are complete
+    if (warp != 5) pdl_wait();                     // the chain's state snapshots are complete
 
     if (warp == 5) {
         // ===== TMA producer: Q tiles through the ring, S_f whenever the frame changes.  Q does not come from the previous
@@ -439,12 +451,20 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             auto load_q = [&](int t, int i) {
                 const int bhf = t / p.TPF, tile = t % p.TPF;
                 const int f = bhf % p.F, bh = bhf / p.F;
-                const int st = i % QST;
+                const int st = i % qst;
                 mbar_expect_tx(&q_full[st], L::Q_BYTES);
 #pragma unroll
                 for (int nb = 0; nb < NB; ++nb) tma_load_5d(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
             };
-            for (int i = 0; i < QST && t_lo + i < t_hi; ++i) load_q(t_lo + i, i);
+            auto load_qr = [&](int t) {
+                const int bhf = t / p.TPF, tile = t % p.TPF;
+                const int f = bhf % p.F, bh = bhf / p.F;
+                mbar_expect_tx(qr_full, L::Q_BYTES);
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(sQr + nb * kBlk, &tmQr, qr_full, nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+            };
+            for (int i = 0; i < qst && t_lo + i < t_hi; ++i) load_q(t_lo + i, i);
+            if (norm && t_lo < t_hi) load_qr(t_lo);
             pdl_wait();
             int cur = -1, ns = 0;
             for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
@@ -458,9 +478,13 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     for (int nb = 0; nb < NB; ++nb) tma_load_3d(sS + sb * L::S_BYTES + nb * (D * 128), &tmSc, &s_full[sb], nb * 64, 0, bh * p.NSc + f + 1);
                     cur = bhf; ++ns;
                 }
-                if (i >= QST) {
-                    mbar_wait(&q_empty[i % QST], (uint32_t)((i / QST) - 1) & 1u);
+                if (i >= qst) {
+                    mbar_wait(&q_empty[i % qst], (uint32_t)((i / qst) - 1) & 1u);
                     load_q(t, i);
+                }
+                if (norm && i >= 1) {
+                    mbar_wait(qr_empty, (uint32_t)(i - 1) & 1u);             // the epilogue has formed den of the previous tile
+                    load_qr(t);
                 }
             }
         }
@@ -476,8 +500,8 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mbar_wait(&s_full[ns & 1], (uint32_t)(ns >> 1) & 1u);
                     cur = bhf; ++ns;
                 }
-                const int st = i % QST, a = i & 1;
-                mbar_wait(&q_full[st], (uint32_t)(i / QST) & 1u);
+                const int st = i % qst, a = i & 1;
+                mbar_wait(&q_full[st], (uint32_t)(i / qst) & 1u);
                 if (i >= 2) mbar_wait(&acc_empty[a], (uint32_t)((i >> 1) - 1) & 1u);
                 tc_fence_after();
                 const uint32_t aQ = smem_u32(smem + st * L::Q_BYTES), aS = smem_u32(sS + ((ns - 1) & 1) * L::S_BYTES);
@@ -491,6 +515,8 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else {
         // ===== epilogue: TMEM -> registers -> scale (/ normaliser) -> bf16 -> swizzled staging -> TMA store =====
         const int row = tid;
+        int z_cur = -1, z_nxt_bhf = -1;
+        unsigned short z_nxt = 0;
         // Output gate (Eq. 23): the gate tile of a token tile has the layout of the output tile, so it is brought by TMA INTO
         // the staging buffer the output tile is about to be written to; each thread reads a 16-byte piece of the gate, scales
         // its accumulator piece and writes the result over it.  (One global load per piece and thread, issued when needed,
@@ -510,20 +536,45 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const int f = bhf % p.F, bh = bhf / p.F;
             const int a = i & 1;
             const int n = tile * 128 + row;                      // token inside the frame
-            const long long tok = ((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.H + (bh % p.H);   // index into den [B][T][H]
             float mul = p.scale;
-            if (p.den_mode == 2 && n < p.G) mul = p.scale / (__ldg(p.den + tok) + p.eps);          // Eq. 22: eps after the dot product, no clamp
-            if (p.den_mode == 1) {
-                // z pass: only column 0 of Q_raw S^z is the normaliser q_raw . z_f; nothing goes to `out`
-                mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
-                tc_fence_after();
-                float v[8];
-                tmem_ld8(tmem_addr(tmem + a * D, warp * 32, 0), v);
-                tc_fence_before();
+            if (norm) {
+                // Eq. 20-22: den = q_raw . z_f (fp32 accumulation; eps after the dot product, no clamp).  z_f: column 0 of the z
+                // pass's snapshot, fetched when the frame changes; q_raw row: this thread's row of the staged tile.
+                const uint32_t zb = smem_u32(smem + L::OFF_Z);
+                auto z_of = [&](int bhf_) {                      // element `row` of z of frame-head bhf_ (bf16 bits)
+                    const int f_ = bhf_ % p.F, bh_ = bhf_ / p.F;
+                    return (row < D) ? __ldcg(reinterpret_cast<const unsigned short*>(p.z_sc) + (((long long)bh_ * p.NSc + f_ + 1) * D + row) * D) : (unsigned short)0;
+                };
+                if (bhf != z_cur) {                              // uniform over the 128 epilogue threads
+                    if (z_nxt_bhf != bhf) z_nxt = z_of(bhf);     // (first tile of the CTA: nothing was requested ahead)
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    if (row < D) sts_f32(zb + row * 4, __uint_as_float((uint32_t)z_nxt << 16));
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    z_cur = bhf;
+                }
+                if (t + 1 < t_hi && (t + 1) / p.TPF != bhf) {    // the next tile is in another frame: its z is requested a tile ahead
+                    z_nxt_bhf = (t + 1) / p.TPF;
+                    z_nxt = z_of(z_nxt_bhf);
+                }
+                mbar_wait(qr_full, (uint32_t)i & 1u);
+                const uint32_t qr = smem_u32(sQr);
+                uint4 qv[D / 8];
+#pragma unroll
+                for (int c = 0; c < D / 8; ++c) qv[c] = ld_shared_v4(qr + swz_chunk_off(row, c, kBlk));
+                float den = 0.f;
+#pragma unroll
+                for (int c = 0; c < D / 8; ++c) {
+                    float x[8];
+                    unpack8(qv[c], x);
+                    const float4 z0 = lds_f4(zb + c * 32), z1 = lds_f4(zb + c * 32 + 16);
+                    den = fmaf(x[0], z0.x, den); den = fmaf(x[1], z0.y, den); den = fmaf(x[2], z0.z, den); den = fmaf(x[3], z0.w, den);
+                    den = fmaf(x[4], z1.x, den); den = fmaf(x[5], z1.y, den); den = fmaf(x[6], z1.z, den); den = fmaf(x[7], z1.w, den);
+                }
+                // The slot is released only now, behind the arithmetic that consumed the loaded registers: an arrive issued
+                // right after the loads overtook them (measured: the next tile's q_raw landed in rows still being read).
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[a]);
-                if (n < p.G) p.den[tok] = v[0];
-                continue;
+                if (lane == 0) mbar_arrive(qr_empty);
+                if (n < p.G) mul = p.scale / (den + p.eps);
             }
             // the store that read staging buffer `a` two tiles ago must have finished reading it
             if (tid == 0) {
