@@ -204,7 +204,7 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
 
 
 
-// The frame-wise paths are up to seven launches on two streams per call; at the paper's production chunk (8 MB of
+// The frame-wise paths are up to six launches on two streams per call; at the paper's production chunk (8 MB of
 // input) the host cannot issue them as fast as the GPU retires them.  So a call is captured ONCE per tuple of argument
 // pointers into a CUDA graph (fork / join with the normaliser's stream and the programmatic launch edges included) and
 // replayed afterwards: one graph launch per call.  Not used when per-kernel profiling is on, when the caller is itself
