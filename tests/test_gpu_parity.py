@@ -221,7 +221,8 @@ def test_normalizer_readout(G):
 
 
 @pytest.mark.parametrize("d", [64, 128])
-@pytest.mark.parametrize("B,H,G,F", [(1, 2, 352, 2), (2, 3, 880, 3), (1, 20, 256, 1)])
+@pytest.mark.parametrize("B,H,G,F", [(1, 2, 352, 2), (2, 3, 880, 3), (1, 20, 256, 1),
+                                     (1, 20, 880, 3)])      # 420 tiles on 148 readout CTAs: several tiles and frame changes per CTA
 def test_normalizer_readout_tensor_core_frame_path(d, B, H, G, F):
     """Paper Eq. 20-22 on the tcgen05 frame path (bf16): the z recurrence runs through the same three kernels as
     column 0 of a matrix state; out = scale q S / (q_raw . z + eps).  z updated in place."""
