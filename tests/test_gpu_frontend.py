@@ -169,3 +169,35 @@ def test_graph_replay_on_a_user_stream_matches_direct_calls():
     assert all(torch.isfinite(o.float()).all() for o in results["graph"])
     for a, b in zip(results["direct"], results["graph"]):
         assert torch.equal(a, b)
+
+
+def test_full_operator_is_bit_repeatable_over_many_calls():
+    """The paper's production chunk through gdn_forward_chunk_full, 30 times from the same inputs and state: every
+    output, state and z must be bit-identical to the first call's.  The readout CTAs run several tiles each (ring slots,
+    staging buffers and the q_raw slot are reused), Phase A reduces in a fixed order, the scans hand their history sum to
+    whichever CTA of a pair finishes last: any reuse-before-read or order dependence shows up as a differing bit."""
+    B, H, G, F, D = 1, 20, 880, 3, 128
+    T = G * F
+    wl = gin.GdnWorkload("repeat", B, H, T, D, D, group=G, seed=700)
+    fi = gin.make_frontend_inputs(wl)
+    d = {n: fi[n].to(DEV) for n in fi}
+    out = torch.empty(B, T, H, D, device=DEV, dtype=torch.bfloat16)
+    st3 = 3 * H * D
+    first = None
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=D, d_v=D, group=G, flags=gdn.GDN_FLAG_NORMALIZER | gdn.GDN_FLAG_BIDIR,
+                     q_token_stride=st3, k_token_stride=st3, v_token_stride=st3) as p:
+        fm = gdn.make_featmap_args(d["qkv"][:, :, 0], d["qkv"][:, :, 1], d["w_q"], d["w_k"], d["cos"], d["sin"], 1e-6)
+        ga = gdn.make_gate_args(d["x"], d["w_alpha"], d["b_alpha"], d["a_log"], d["w_beta"], d["b_beta"])
+        for i in range(30):
+            S = d["state"].clone()
+            z = d["z_in"].clone()
+            out.fill_(float("nan"))
+            p.forward_full(fm, d["qkv"][:, :, 2], ga, None, None, d["gate"], S, z, out, S, z)
+            torch.cuda.synchronize()
+            got = (out.clone(), S, z)
+            if first is None:
+                first = got
+                assert torch.isfinite(out.float()).all()
+            else:
+                for a, b in zip(first, got):
+                    assert torch.equal(a, b), f"call {i} differs from call 0"
