@@ -130,9 +130,9 @@ gdn_status_t gdn_forward_chunk(gdn_plan_t* plan,
  *   (Eq. 20-21), out_n = scale * q_rot_n S_g / (q_raw_n . z_g + eps) (Eq. 22).
  *   z_in [B,H,d_k] fp32 or NULL; z_out [B,H,d_k] fp32 (may alias z_in).  Other arguments as above.
  *   q_raw has the layout of q_rot (q_token_stride) and k_raw the layout of k_rot (k_token_stride).
- *   Frame-wise bf16 plans (group > 1, d_k = d_v in {64,128}) run it on the tensor-core path: the z recurrence goes
- *   through the same three kernels as column 0 of a matrix state (the z path is the matrix path with v = 1),
- *   leaving q_raw . z_f per token in the plan's workspace, then the matrix pass divides in its epilogue.
+ *   Frame-wise bf16 plans (group > 1, d_k = d_v in {64,112,128}) run it on the tensor-core path: the z recurrence goes
+ *   through the same summary and scan kernels as column 0 of a matrix state (the z path is the matrix path with v = 1);
+ *   the readout of the matrix pass takes z_f from that scan, forms q_raw . z_f per token and divides in its epilogue.
  *   Everything else (token-wise, fp32, d = 32) runs on the fp32 CUDA-core kernel.
  */
 gdn_status_t gdn_forward_chunk_norm(gdn_plan_t* plan,
