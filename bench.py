@@ -428,6 +428,7 @@ def kernel_bytes(name, wl, by_call):
         "gdn_tok_output": th * wl.d_v * es,
         "gdn_tok_chain": 2 * st,
         "gdn_frm_summaries": th * ((wl.d_k + wl.d_v) * es + 4),
+        "gdn_frm_summaries_dual": th * ((2 * wl.d_k + wl.d_v) * es + 4),      # k, k_raw, v, beta
         "gdn_frm_readout": th * (wl.d_k + wl.d_v) * es,
         "gdn_frontend_kernel": th * 7 * wl.d_k * es,      # q, k read; q_rot, k_rot, q_raw, k_raw written
     }

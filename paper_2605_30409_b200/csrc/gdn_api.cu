@@ -415,8 +415,9 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
                 gdn_status_t ts = gdn::tc_plan_init(p->tc, c, p->sm_count, &msg);
                 if (ts != GDN_OK) { gdn::tc_plan_free(p->tc); delete p; return fail(nullptr, ts, msg); }
             }
-            // frame path with the normaliser: Phase A and the scan run twice (matrix and z pass), the readout once
-            p->path = path; p->chunk = chunk; p->launches = (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_NORMALIZER)) ? 2 * launches - 1 : launches;
+            // frame path with the normaliser: Phase A and the scan run twice (matrix and z pass), the readout once; at d = 128
+            // without a token split one launch does Phase A of both passes
+            p->path = path; p->chunk = chunk; p->launches = (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_NORMALIZER)) ? 2 * launches - 1 - ((p->tc.D == 128 && p->tc.NSPLIT == 1) ? 1 : 0) : launches;
             p->workspace_bytes = p->tc.workspace_bytes;
         }
     }

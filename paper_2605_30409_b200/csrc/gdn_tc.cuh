@@ -45,6 +45,8 @@ struct TcPlan {
     CUtensorMap tmQ, tmK, tmV, tmO;
     CUtensorMap tmGt;                                // output gate (Eq. 23), same tiling as tmO
     const void* cgate = nullptr;
+    CUtensorMap tmK64, tmV64, tmKr64;                // 64-token boxes of k, v, k_raw: the dual Phase A of the normalised frame path
+    const void *ck64 = nullptr, *cv64 = nullptr, *ckr64 = nullptr;
     // fused single-kernel token path (C = 128): per-tile ready flags and the call epoch
     bool fused = false;
     unsigned int* flags = nullptr;
@@ -450,7 +452,8 @@ inline cudaError_t tc_launch_fused64(TcPlan& tp, const TokParams& p, cudaStream_
 template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
                                    const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
-                                   cudaEvent_t before_readout = nullptr, bool readout = true, const CUtensorMap* tmQr = nullptr) {
+                                   cudaEvent_t before_readout = nullptr, bool readout = true, const CUtensorMap* tmQr = nullptr,
+                                   bool phase_a = true) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -465,13 +468,15 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     }
     const int sms = tp.sm_count > 0 ? tp.sm_count : 148;
     const int grid3 = fp.total_tiles < sms ? fp.total_tiles : sms;
-    if (prof) prof->begin(st);
     cudaError_t le;
-    // Launched as a programmatic dependent of whatever precedes it in the stream (the front-end kernel, the readout of the
-    // previous call): the kernel waits for that grid before its first global access, only its prologue overlaps.
-    le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
-    if (le != cudaSuccess) return le;
-    if (prof) prof->mark(st, "gdn_frm_summaries");
+    if (phase_a) {
+        if (prof) prof->begin(st);
+        // Launched as a programmatic dependent of whatever precedes it in the stream (the front-end kernel, the readout of the
+        // previous call): the kernel waits for that grid before its first global access, only its prologue overlaps.
+        le = launch_pdl(gdn_frm_summaries<D>, dim3(tp.BH * tp.F * tp.NSPLIT * sum_nc<D>()), dim3(kSumThreads), smem1, st, tmK, tmV, fp);
+        if (le != cudaSuccess) return le;
+    }
+    if (prof && phase_a) prof->mark(st, "gdn_frm_summaries");
     const int nchain = tp.BH * (cp.col_tiles ? cp.col_tiles : D / 64);
     if (tp.bidir && tp.F > 1) {
         // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero
@@ -534,6 +539,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dr = c.d_k;
         cudaError_t e = cudaSuccess;
         cudaEvent_t den_ready = nullptr;
+        bool dual = false;
         if (na) {
             // z pass (Eq. 20-21 through the same Phase A and scan kernels): K_raw summaries with the constant block as V, the
             // scan on a [D][D] state whose column 0 is z (first 64-column tile only).  It shares nothing with the matrix pass
@@ -546,9 +552,6 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
                 if (!ok) { tp.cqr = tp.ckr = nullptr; return GDN_ERR_CUDA; }
                 tp.cqr = na->q_raw; tp.ckr = na->k_raw;
             }
-            e = cudaEventRecord(tp.zev0, st);         // after everything queued on the caller's stream so far
-            if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
-            if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             FrmParams zf = fp;
             zf.part = zt.part; zf.counters = zt.flags; zf.Gw = zt.Gw; zf.Nw = zt.Nw; zf.gam = zt.gam;
             zf.zpass = 1; zf.scale = 1.f;
@@ -557,8 +560,35 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             zc.S_in = nullptr; zc.S_out = nullptr;
             zc.zvec = 1; zc.z_vec_in = na->z_in; zc.z_vec_out = na->z_out;      // z <-> column 0 of the state, in the chain kernel
             zc.col_tiles = 1;                        // ... so only the first 64-column tile is run (the readout uses column 0 only)
-            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false)
-                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false);
+            // d = 128 without a token split: Phase A of both passes in ONE launch (gdn_frm_summaries_dual), then the z scan
+            // beside the matrix scan
+            dual = tp.D == 128 && tp.NSPLIT == 1 && zt.NSPLIT == 1;
+            if (dual) {
+                if (k != tp.ck64 || v != tp.cv64 || na->k_raw != tp.ckr64) {
+                    const bool dense = na->dense_qk;
+                    bool ok = tc::make_act_tmap(&tp.tmK64, k, c.B, c.T, c.H, c.d_k, c.group, ts(dense ? 0 : c.k_token_stride, c.d_k), 64, err) &&
+                              tc::make_act_tmap(&tp.tmV64, v, c.B, c.T, c.H, c.d_v, c.group, ts(c.v_token_stride, c.d_v), 64, err) &&
+                              tc::make_act_tmap(&tp.tmKr64, na->k_raw, c.B, c.T, c.H, c.d_k, c.group, ts(dense ? 0 : c.k_token_stride, c.d_k), 64, err);
+                    if (!ok) { tp.ck64 = tp.cv64 = tp.ckr64 = nullptr; return GDN_ERR_CUDA; }
+                    tp.ck64 = k; tp.cv64 = v; tp.ckr64 = na->k_raw;
+                }
+                const size_t smemD = frm::DualSmem<128>::TOTAL;
+                if (!(tp.attr_mask & 32u)) {
+                    e = set_smem(frm::gdn_frm_summaries_dual<128>, smemD);
+                    if (e != cudaSuccess) { if (err) *err = std::string("dual Phase A attribute: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+                    tp.attr_mask |= 32u;
+                }
+                if (prof) prof->begin(st);
+                e = launch_pdl(frm::gdn_frm_summaries_dual<128>, dim3(tp.BH * tp.F * 2), dim3(frm::kSumThreads), smemD, st, tp.tmK64, tp.tmV64,
+                               tp.tmKr64, fp, zf);
+                if (e != cudaSuccess) { if (err) *err = std::string("dual Phase A launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+                if (prof) prof->mark(st, "gdn_frm_summaries_dual");
+            }
+            e = cudaEventRecord(tp.zev0, st);         // after everything queued on the caller's stream so far
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
+            if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false, nullptr, !dual)
+                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false, nullptr, !dual);
             if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
             if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
             fp.den_mode = 1; fp.eps = c.eps; fp.z_sc = zt.Sc;
@@ -569,8 +599,8 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             }
             den_ready = tp.zev1;
         }
-        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr)
-                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr);
+        e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr, !dual)
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr, !dual);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

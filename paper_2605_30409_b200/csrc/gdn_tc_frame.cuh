@@ -380,6 +380,227 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Phase A of BOTH passes of the normalised frame path in one launch (d = 128, no token split): CTA (b,h,f,j) streams
+// 64-token tiles of K, V block j and K_raw once and keeps two accumulators,
+//     [Gram | A](:, block j)       = (diag(beta) K)^T     [K block j     | V block j]       (matrix pass, Eq. 4-5)
+//     [Gram_raw | b](:, block j)   = (diag(beta) K_raw)^T [K_raw block j | 1-column block]  (z pass, Eq. 20-21: b = K_raw^T beta)
+// Launched one after the other, the two passes' Phase A grids (120 CTAs of 230 KB each at the paper's chunk) cannot be
+// resident together and the second waits for SMs; here the second pass costs one more tile load and copy per tile.  The
+// constant block is a 16-token slice addressed by every MMA of the tile through its own LBO (any distance is a legal LBO).
+// ---------------------------------------------------------------------------------------------------
+constexpr uint32_t kHBlk = 8192;       // one [64 tokens][64 features] bf16 block
+
+template <int D>
+struct DualSmem {
+    static constexpr int NB = D / 64;
+    static constexpr uint32_t KT = NB * kHBlk;                        // [64 tokens][D] bf16
+    static constexpr uint32_t STAGE = KT + kHBlk + KT;                // K | V block j | K_raw
+    static constexpr int STAGES = 4;                                  // the ring is latency-bound: (load + copies + MMAs) / stages per tile
+    static constexpr int SCB = 2;                                     // diag(beta) K copies
+    static constexpr int SCR = 1;                                     // diag(beta) K_raw copies (one: what a fourth stage leaves room for)
+    static constexpr uint32_t OFF_SCK = STAGES * STAGE;
+    static constexpr uint32_t OFF_SCR = OFF_SCK + SCB * KT;
+    static constexpr uint32_t OFF_ONE = OFF_SCR + SCR * KT;           // [16 tokens][64]: column 0 = 1 (block j = 0 only)
+    static constexpr uint32_t OFF_BAR = OFF_ONE + 2048;
+    static constexpr uint32_t TOTAL = OFF_BAR + 512 + 1024;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kSumThreads, 1)
+gdn_frm_summaries_dual(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                       const __grid_constant__ CUtensorMap tmKr, const FrmParams p, const FrmParams pz) {
+    static_assert(D == 128, "dual Phase A: d = 128 (two column CTAs per frame)");
+    using L = DualSmem<D>;
+    constexpr int NB = L::NB, NC = 2, STAGES = L::STAGES, SCB = L::SCB, SCR = L::SCR;
+    constexpr int NW = 2 * D / NC;                // accumulator columns per pass: [Gram cols | A cols]
+    constexpr int HW = D / NC;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::OFF_BAR);
+    uint64_t* bar_full = bars;                    // [STAGES]
+    uint64_t* bar_empty = bar_full + STAGES;      // [STAGES]
+    uint64_t* bar_scK = bar_empty + STAGES;       // [SCB] diag(beta) K written (4 warps)
+    uint64_t* bar_frK = bar_scK + SCB;            // [SCB] the MMAs that read it have completed
+    uint64_t* bar_scR = bar_frK + SCB;            // [SCR] the same for K_raw
+    uint64_t* bar_frR = bar_scR + SCR;
+    uint64_t* bar_done = bar_frR + SCR;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bar_done + 1);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int j = blockIdx.x % NC;
+    const int bhf = blockIdx.x / NC;
+    const int f = bhf % p.F, bh = bhf / p.F;
+    const int b = bh / p.H, h = bh % p.H;
+    const int ntiles = (p.G + 63) / 64;           // 64-token tiles of the frame
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(&bar_full[s], 1); mbar_init(&bar_empty[s], 1); }
+        for (int s = 0; s < SCB; ++s) { mbar_init(&bar_scK[s], 4); mbar_init(&bar_frK[s], 1); }
+        for (int s = 0; s < SCR; ++s) { mbar_init(&bar_scR[s], 4); mbar_init(&bar_frR[s], 1); }
+        mbar_init(bar_done, 1);
+        mbar_fence_init();
+    }
+    if (tid == 160) { tma_prefetch_desc(&tmK); tma_prefetch_desc(&tmV); tma_prefetch_desc(&tmKr); }
+    if (warp == 0) tmem_alloc(tmem_slot, 2 * NW);
+    if (tid < 16) {
+        const uint32_t one = smem_u32(smem + L::OFF_ONE);
+#pragma unroll
+        for (int c = 0; c < 8; ++c) st_shared_v4(one + swz_chunk_off(tid, c, 0), (c == 0 && j == 0) ? 0x00003F80u : 0u, 0u, 0u, 0u);
+        fence_proxy_async();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    pdl_wait();                                    // (the front-end kernel of gdn_forward_chunk_full precedes)
+    pdl_launch_dependents();
+
+    if (warp == 5) {
+        // ===== TMA producer =====
+        if (elect_one()) {
+            constexpr int kPF = 4;                 // L2 prefetch distance (64-token tiles) ahead of the ring
+            auto prefetch = [&](int i) {
+                const int n0 = i * 64;
+                if (j == 0) {
+#pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) { tma_prefetch_5d(&tmK, nb * 64, h, n0, f, b); tma_prefetch_5d(&tmKr, nb * 64, h, n0, f, b); }
+                }
+                tma_prefetch_5d(&tmV, j * 64, h, n0, f, b);
+            };
+            for (int i = STAGES; i < min(ntiles, STAGES + kPF); ++i) prefetch(i);
+            for (int i = 0; i < ntiles; ++i) {
+                const int st = i % STAGES;
+                if (i >= STAGES) mbar_wait(&bar_empty[st], (uint32_t)((i / STAGES) - 1) & 1u);
+                if (i + kPF < ntiles && i >= STAGES) prefetch(i + kPF);
+                uint8_t* base = smem + st * L::STAGE;
+                mbar_expect_tx(&bar_full[st], L::STAGE);
+                const int n0 = i * 64;
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + nb * kHBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
+                tma_load_5d(base + L::KT, &tmV, &bar_full[st], j * 64, h, n0, f, b);
+#pragma unroll
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + L::KT + kHBlk + nb * kHBlk, &tmKr, &bar_full[st], nb * 64, h, n0, f, b);
+            }
+        }
+    }
+    else if (warp == 4) {
+        // ===== MMA issuer: four 16-token steps per pass and tile =====
+        if (elect_one()) {
+            const uint32_t id = umma_idesc(D, NW, true, true);
+            const uint32_t one = smem_u32(smem + L::OFF_ONE);
+            for (int i = 0; i < ntiles; ++i) {
+                const int st = i % STAGES, sb = i % SCB, sr = i % SCR;
+                mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
+                const uint32_t base = smem_u32(smem + st * L::STAGE);
+                mbar_wait(&bar_scK[sb], (uint32_t)(i / SCB) & 1u);
+                tc_fence_after();
+                {   // matrix pass: B = [K block j | V block j]
+                    const uint32_t a = smem_u32(smem + L::OFF_SCK + sb * L::KT), bq = base + (uint32_t)j * kHBlk;
+#pragma unroll
+                    for (int s = 0; s < 4; ++s)
+                        umma_bf16(tmem, desc_mnmajor(a + s * 2048, kHBlk), desc_mnmajor(bq + s * 2048, (uint32_t)(NB - j) * kHBlk), id,
+                                  (i > 0 || s > 0) ? 1u : 0u);
+                    umma_commit(&bar_frK[sb]);
+                }
+                mbar_wait(&bar_scR[sr], (uint32_t)(i / SCR) & 1u);
+                tc_fence_after();
+                {   // z pass: B = [K_raw block j | the constant slice, the same 16 rows for every step]
+                    const uint32_t a = smem_u32(smem + L::OFF_SCR + sr * L::KT), br = base + L::KT + kHBlk + (uint32_t)j * kHBlk;
+#pragma unroll
+                    for (int s = 0; s < 4; ++s)
+                        umma_bf16(tmem + NW, desc_mnmajor(a + s * 2048, kHBlk), desc_mnmajor(br + s * 2048, one - (br + s * 2048)), id,
+                                  (i > 0 || s > 0) ? 1u : 0u);
+                    umma_commit(&bar_frR[sr]);
+                }
+                umma_commit(&bar_empty[st]);
+            }
+            umma_commit(bar_done);
+        }
+    } else {
+        // ===== diag(beta) copies of K and K_raw: thread t -> token row t % 64 of feature block t / 64 =====
+        const int r = tid & 63, blk = tid >> 6;
+        const float* beta_f = p.beta + (long long)bh * p.T + (long long)f * p.G;
+        auto load_beta = [&](int i) { const int n = i * 64 + r; return (i < ntiles && n < p.G) ? __ldg(beta_f + n) : 0.f; };
+        auto scaled_copy = [&](uint32_t src, uint32_t dst, const Bf16Scale& bs) {
+            uint4 x[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) x[c] = ld_shared_v4(src + (uint32_t)(((c + r) & 7) << 4));
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                st_shared_v4(dst + (uint32_t)(((c + r) & 7) << 4), bf16x2_scale(x[c].x, bs), bf16x2_scale(x[c].y, bs),
+                             bf16x2_scale(x[c].z, bs), bf16x2_scale(x[c].w, bs));
+            fence_proxy_async();
+            __syncwarp();
+        };
+        float b_next = load_beta(0);
+        for (int i = 0; i < ntiles; ++i) {
+            const int st = i % STAGES, sb = i % SCB, sr = i % SCR;
+            const Bf16Scale bs = bf16_scale(b_next);
+            b_next = load_beta(i + 1);
+            const uint32_t stage = smem_u32(smem + st * L::STAGE), off = (uint32_t)blk * kHBlk + (uint32_t)r * 128u;
+            if (i >= SCB) mbar_wait(&bar_frK[sb], (uint32_t)((i / SCB) - 1) & 1u);
+            mbar_wait(&bar_full[st], (uint32_t)(i / STAGES) & 1u);
+            scaled_copy(stage + off, smem_u32(smem + L::OFF_SCK + sb * L::KT) + off, bs);
+            if (lane == 0) mbar_arrive(&bar_scK[sb]);
+            if (i >= SCR) mbar_wait(&bar_frR[sr], (uint32_t)((i / SCR) - 1) & 1u);
+            scaled_copy(stage + L::KT + kHBlk + off, smem_u32(smem + L::OFF_SCR + sr * L::KT) + off, bs);
+            if (lane == 0) mbar_arrive(&bar_scR[sr]);
+        }
+    }
+
+    // ---- epilogue (warps 0-3; thread = summary row m): G_f = alpha_f Gram (bf16), N_f = A (fp32) of both passes, staged in the
+    //      idle ring and copied out in whole row segments (see gdn_frm_summaries) ----
+    if (warp < 4) {
+        const int m = tid;
+        float a_f = p.alpha[bhf];
+        if (p.log_alpha) a_f = expf(a_f);
+        mbar_wait(bar_done, 0);
+        tc_fence_after();
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            const FrmParams& q = pass ? pz : p;
+            const uint32_t stgG = smem_u32(smem) + (uint32_t)pass * (D * 128 + D * 256), stgN = stgG + D * 128;
+#pragma unroll 1
+            for (int cc = 0; cc < NW / 32; ++cc) {
+                float v[32];
+                tmem_ld32(tmem_addr(tmem + pass * NW, warp * 32, cc * 32), v);
+                if (cc < HW / 32) {
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4)
+                        st_shared_v4(stgG + m * 128 + (uint32_t)(((cc * 4 + q4) ^ (m & 7)) << 4), pack_bf16(a_f * v[8 * q4], a_f * v[8 * q4 + 1]),
+                                     pack_bf16(a_f * v[8 * q4 + 2], a_f * v[8 * q4 + 3]), pack_bf16(a_f * v[8 * q4 + 4], a_f * v[8 * q4 + 5]),
+                                     pack_bf16(a_f * v[8 * q4 + 6], a_f * v[8 * q4 + 7]));
+                } else {
+#pragma unroll
+                    for (int q4 = 0; q4 < 8; ++q4)
+                        st_shared_v4(stgN + m * 256 + (uint32_t)((((cc - HW / 32) * 8 + q4) ^ (m & 7)) << 4), __float_as_uint(v[4 * q4]),
+                                     __float_as_uint(v[4 * q4 + 1]), __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
+                }
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            __nv_bfloat16* gbase = q.Gw + (long long)bhf * D * D + j * HW;
+            float* nbase = q.Nw + (long long)bhf * D * D + j * HW;
+#pragma unroll 4
+            for (int idx = tid; idx < D * 8; idx += 128) {
+                const int row = idx >> 3, c = idx & 7;
+                const uint4 u = ld_shared_v4(stgG + row * 128 + (uint32_t)((c ^ (row & 7)) << 4));
+                st_global_v4(gbase + (long long)row * D + c * 8, u.x, u.y, u.z, u.w);
+            }
+#pragma unroll 4
+            for (int idx = tid; idx < D * 16; idx += 128) {
+                const int row = idx >> 4, c = idx & 15;
+                const uint4 u = ld_shared_v4(stgN + row * 256 + (uint32_t)((c ^ (row & 7)) << 4));
+                st_global_v4(nbase + (long long)row * D + c * 4, u.x, u.y, u.z, u.w);
+            }
+            if (tid == 0 && j == 0) q.gam[bhf] = a_f;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, 2 * NW);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Phase C.  grid = min(#SM, tiles), block = 192.   O = scale * Q_f S_f   (S_f = snapshot slot f + 1)
 //   CTA c runs the contiguous tile range [c n / grid, (c+1) n / grid) of the (b,h,f,tile) order.
 // ---------------------------------------------------------------------------------------------------
