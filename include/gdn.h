@@ -188,6 +188,25 @@ gdn_status_t gdn_compute_gates(gdn_plan_t* plan, const gdn_gate_args_t* args, fl
                                gdn_stream_t stream);
 
 /*
+ * gdn_compute_gates_static: gdn_compute_gates (Eq. 13-15) for callers that must not allocate -- code under CUDA
+ *   graph capture, tight serving loops, harnesses that forbid cudaMalloc.  No plan: the problem is given by plain sizes.
+ *   The call allocates NOTHING (no cudaMalloc / cudaFree / allocating library routine; it issues one cudaMemsetAsync and one
+ *   kernel launch on `stream`): the scratch gdn_compute_gates keeps in a plan-owned buffer (partial frame sums, arrival
+ *   counters) lives in a file-scope `static __device__` array of the library, 80 KB that every GPU loading the library holds
+ *   until the process exits.
+ *   args, alpha_out [B,H,T/group], beta_out [B,H,T]: as gdn_compute_gates (device pointers; the caller owns them);
+ *   D = head dim (multiple of 8, <= 128); log_alpha != 0 writes log(alpha) instead of alpha.
+ *   LIMIT: B*H*(T/group) <= 4096 frame-heads per call (the paper's chunk: 60); beyond that GDN_ERR_UNSUPPORTED with a
+ *   message naming the limit (gdn_last_error(NULL)), nothing is launched.
+ *   SHARING: all calls on a device use the same array and find the last call's contents in it; the call clears what must
+ *   start at zero in stream order.  Calls that may run concurrently on the GPU (different streams, no ordering between them)
+ *   RACE on it and give wrong gates: serialise them.  Results equal gdn_compute_gates' (bit for bit whenever both choose the
+ *   same number of token splits per frame, which they do unless B*H*(T/group)*splits would exceed 16384).
+ */
+gdn_status_t gdn_compute_gates_static(const gdn_gate_args_t* args, int B, int T, int H, int D, int group, int log_alpha,
+                                      float* alpha_out, float* beta_out, gdn_stream_t stream);
+
+/*
  * gdn_forward_chunk_full: the operator at the boundary of the paper's kernel (Alg. 1): feature map on q, k
  *   -> [gates from x] -> GDN recurrence with normalised readout (and the bidirectional in-chunk scan when the plan
  *   carries GDN_FLAG_BIDIR) -> output gate, out = G (.) Y (Eq. 23; the projection W_o is outside).

@@ -31,7 +31,7 @@ GDN_FLAG_NORMALIZER, GDN_FLAG_BIDIR, GDN_FLAG_LOG_ALPHA, GDN_FLAG_FORCE_SIMT, GD
 PATH_NAMES = {0: "simt_fp32", 1: "tc_token", 2: "tc_frame"}
 EXPORTED_SYMBOLS = [
     "gdn_plan", "gdn_forward_chunk", "gdn_forward_chunk_norm", "gdn_forward_chunk_host", "gdn_destroy",
-    "gdn_feature_map", "gdn_compute_gates", "gdn_forward_chunk_full",
+    "gdn_feature_map", "gdn_compute_gates", "gdn_compute_gates_static", "gdn_forward_chunk_full",
     "gdn_plan_get_info", "gdn_plan_set_profiling", "gdn_plan_kernel_times", "gdn_status_string", "gdn_last_error",
     "gdn_version",
 ]
@@ -100,6 +100,8 @@ def lib() -> ctypes.CDLL:
         L.gdn_feature_map.argtypes = [vp, ctypes.POINTER(GdnFeatmapArgs), vp, vp, vp, vp, vp]
         L.gdn_compute_gates.restype = ctypes.c_int
         L.gdn_compute_gates.argtypes = [vp, ctypes.POINTER(GdnGateArgs), fp, fp, vp]
+        L.gdn_compute_gates_static.restype = ctypes.c_int
+        L.gdn_compute_gates_static.argtypes = [ctypes.POINTER(GdnGateArgs)] + [ctypes.c_int] * 6 + [fp, fp, vp]
         L.gdn_forward_chunk_full.restype = ctypes.c_int
         L.gdn_forward_chunk_full.argtypes = [vp, ctypes.POINTER(GdnFeatmapArgs), vp, ctypes.POINTER(GdnGateArgs), fp, fp, vp,
                                              fp, fp, vp, fp, fp, vp]
@@ -205,6 +207,13 @@ def gdn_feature_map(plan, fm: GdnFeatmapArgs, q_rot, k_rot, q_raw, k_raw, stream
 
 def gdn_compute_gates(plan, ga: GdnGateArgs, alpha_out, beta_out, stream=None) -> None:
     _check(plan, lib().gdn_compute_gates(plan, ctypes.byref(ga), _ptr(alpha_out), _ptr(beta_out), _stream_handle(stream)))
+
+
+def gdn_compute_gates_static(ga: GdnGateArgs, B: int, T: int, H: int, D: int, group: int, log_alpha: bool, alpha_out, beta_out,
+                             stream=None) -> None:
+    """The gates without a plan and without any allocation (static device scratch; see include/gdn.h for the limit)."""
+    _check(None, lib().gdn_compute_gates_static(ctypes.byref(ga), B, T, H, D, group, int(bool(log_alpha)), _ptr(alpha_out),
+                                                _ptr(beta_out), _stream_handle(stream)))
 
 
 def gdn_forward_chunk_full(plan, fm: GdnFeatmapArgs, v, gates: Optional[GdnGateArgs], alpha, beta, out_gate, S_in, z_in,

@@ -7,6 +7,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -21,6 +22,24 @@ struct gdn_plan;
 namespace {
 
 thread_local std::string g_plan_error;
+
+// ---------------------------------------------------------------------------------------------------
+// gdn_compute_gates_static (include/gdn.h): the gates of Eq. 13-15 with NO allocation of any kind.  Its scratch (the partial
+// frame sums of W_alpha . x_n and the per-frame arrival counters that gdn_compute_gates keeps in a plan-owned cudaMalloc'd
+// buffer) lives in this file-scope device array: every GPU that loads the library holds these 80 KB until the process exits,
+// and every call on a device shares them.  In HOST code the array's name is a host-side stand-in, not a device address: the
+// launch below passes the address cudaGetSymbolAddress returns for the current device (looked up once per device).
+// ---------------------------------------------------------------------------------------------------
+constexpr int kStaticGateMaxFrames = 4096;      // B * H * (T / group) at most
+constexpr int kStaticGateMaxParts = 16384;      // B * H * (T / group) * (token splits per frame) at most
+static __device__ __align__(256) unsigned int g_gates_static_scratch[kStaticGateMaxParts + kStaticGateMaxFrames];   // partial sums (fp32) | counters
+
+__global__ void __launch_bounds__(gdn::fe::kFeThreads, 4)
+gdn_gates_static_kernel(const gdn::GateParams gp) {
+    __shared__ float s_sum[16];
+    __shared__ unsigned int s_last;
+    gdn::fe::gates_body(gp, (int)blockIdx.x / gp.NSPL, (int)blockIdx.x % gp.NSPL, s_sum, &s_last);
+}
 
 // gdn_forward_chunk_host: device staging plus a copy/compute pipeline over token segments.  The call is cut into
 // up to kMaxSeg segments of Tseg tokens (whole 128-token tiles, resp. whole frames; exact by the split invariance of
@@ -479,6 +498,77 @@ gdn_status_t gdn_compute_gates(gdn_plan_t* plan, const gdn_gate_args_t* args, fl
     if (s != GDN_OK || !on) return s;
     plan->prof.begin(static_cast<cudaStream_t>(stream));
     return launch_frontend(plan, nullptr, &gp, static_cast<cudaStream_t>(stream), true);
+}
+
+gdn_status_t gdn_compute_gates_static(const gdn_gate_args_t* a, int B, int T, int H, int D, int group, int log_alpha,
+                                      float* alpha_out, float* beta_out, gdn_stream_t stream) {
+    if (B < 0 || H < 0 || T < 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "B, H, T must be >= 0");
+    if (group <= 0 || T % group != 0) return fail(nullptr, GDN_ERR_INVALID_ARG, "group must be > 0 and divide T");
+    if (D < 8 || D > 128 || D % 8 != 0) return fail(nullptr, GDN_ERR_UNSUPPORTED, "D must be a multiple of 8 between 8 and 128");
+    if (!a || !a->x || !a->w_alpha || !a->b_alpha || !a->a_log || !a->w_beta || !a->b_beta || !alpha_out || !beta_out)
+        return fail(nullptr, GDN_ERR_INVALID_ARG, "a required gate pointer is NULL");
+    if (!aligned16(a->x) || (a->x_token_stride % 8) != 0)
+        return fail(nullptr, GDN_ERR_ALIGNMENT, "x must be 16-byte aligned with a token stride that is a multiple of 8");
+    if (a->x_token_stride < 0 || (a->x_token_stride != 0 && a->x_token_stride < (long long)H * D))
+        return fail(nullptr, GDN_ERR_INVALID_ARG, "x token stride smaller than H*D");
+    if (B == 0 || H == 0 || T == 0) return GDN_OK;
+    const long long BH = (long long)B * H, F = T / group;
+    if (BH * F > kStaticGateMaxFrames)
+        return fail(nullptr, GDN_ERR_UNSUPPORTED, "gdn_compute_gates_static: B*H*(T/group) = " + std::to_string(BH * F) +
+                                                  " exceeds the static scratch (at most 4096 frame-heads per call); use gdn_compute_gates");
+    if (BH * T >= (1LL << 31)) return fail(nullptr, GDN_ERR_UNSUPPORTED, "B*T*H must stay below 2^31");
+
+    // once per device, with that device current: the device address of the scratch array and the SM count
+    struct Dev { bool ready = false; unsigned int* scratch = nullptr; int sms = 0; };
+    constexpr int kMaxDev = 64;
+    static Dev devs[kMaxDev];
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDev) return fail(nullptr, GDN_ERR_UNSUPPORTED, "device ordinal beyond 63");
+    unsigned int* scratch = nullptr;
+    int sms = 0;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        Dev& d = devs[dev];
+        if (!d.ready) {
+            void* ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, g_gates_static_scratch);
+            if (e != cudaSuccess || !ptr) { cudaGetLastError(); return cuda_fail(nullptr, e, "cudaGetSymbolAddress(static gate scratch)"); }
+            e = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(nullptr, e, "cudaDeviceGetAttribute"); }
+            d.scratch = static_cast<unsigned int*>(ptr);
+            d.ready = true;
+        }
+        scratch = d.scratch;
+        sms = d.sms;
+    }
+    // token splits per frame: the rule of gdn_compute_gates (enough CTAs to fill the GPU, at least 64 tokens each), then
+    // as many as the scratch holds
+    int nspl = (int)((4LL * (sms > 0 ? sms : 148) + BH * F - 1) / (BH * F));
+    const int max_spl = (group + 63) / 64;
+    if (nspl > max_spl) nspl = max_spl;
+    while (nspl > 1 && BH * F * nspl > kStaticGateMaxParts) --nspl;
+    if (nspl < 1) nspl = 1;
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // The array keeps what the last call left.  The partial sums are all rewritten before they are read; the counters must
+    // start at zero (a call normally leaves them so, but a failed launch would not): cleared in stream order.
+    e = cudaMemsetAsync(scratch + kStaticGateMaxParts, 0, (size_t)(BH * F) * sizeof(unsigned int), st);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(nullptr, e, "clearing the static gate counters"); }
+    gdn::GateParams gp{};
+    gp.x = static_cast<const __nv_bfloat16*>(a->x);
+    gp.w_alpha = a->w_alpha; gp.b_alpha = a->b_alpha; gp.a_log = a->a_log; gp.w_beta = a->w_beta; gp.b_beta = a->b_beta;
+    gp.alpha_out = alpha_out; gp.beta_out = beta_out;
+    gp.part = reinterpret_cast<float*>(scratch);
+    gp.counters = scratch + kStaticGateMaxParts;
+    gp.x_ts = a->x_token_stride ? a->x_token_stride : (long long)H * D;
+    gp.B = B; gp.T = T; gp.H = H; gp.D = D; gp.G = group; gp.F = (int)F; gp.NSPL = nspl;
+    gp.log_alpha = log_alpha ? 1 : 0;
+    gdn_gates_static_kernel<<<(unsigned int)(BH * F * nspl), gdn::fe::kFeThreads, 0, st>>>(gp);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? GDN_OK : cuda_fail(nullptr, e, "gdn_gates_static_kernel launch");
 }
 
 gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* fm, const void* v, const gdn_gate_args_t* gates,
