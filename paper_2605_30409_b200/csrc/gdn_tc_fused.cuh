@@ -266,6 +266,15 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
             for (int c = 0; c < NT; ++c, ++gs) {
                 const int gst = gs % GST;
                 mbar_wait(&g_full[gst], (gs / GST) & 1u);
+                // N_c's 64-column block of this CTA has been read for the only time (no other CTA loads these lines; the next
+                // call rewrites them): dropped from L2 without a write-back to DRAM (config 3: DRAM writes 170 -> 123 MB, the
+                // call 178.4 -> 176.3 us).  G_c and Qt_c are read by both column CTAs of a head; dropping them from the last
+                // reader (a counter per tile, 4 discards per output-epilogue thread and step) brought the writes down to
+                // 57 MB but cost time where the chain is the bound (config 5: 180 -> 210 us): not done.
+                if (half == 0 && m_ok) {
+                    const char* nl = reinterpret_cast<const char*>(p.Nw) + ((((long long)bh * p.NC + c) * D + m) * D + ct * 64) * 2;
+                    asm volatile("discard.global.L2 [%0], 128;" ::"l"(nl) : "memory");
+                }
                 const float gamma_c = lds_f32(smem_u32(sGamma) + gst * 4);
                 {   // state-independent half, while the MMA runs: S <- gamma_c S + N_c
                     const uint32_t nbase = smem_u32(sG + gst * L::GN_BYTES + L::G_BYTES);
