@@ -26,7 +26,7 @@
  *     nothing throws across the ABI.  A plan is bound to the device current at gdn_plan() time and
  *     must not be used from two host threads at once.  Two calls on the same plan must be issued to
  *     the same stream or be externally ordered (they share the plan's workspace).
- *   - Frame-wise tensor-core calls (up to six launches on two streams) issued on a NON-default stream are captured
+ *   - Frame-wise tensor-core calls (three to five launches) issued on a NON-default stream are captured
  *     once per tuple of argument pointers into a CUDA graph and replayed on later calls with the same pointers (one
  *     graph launch per call; the plan keeps up to 32 graphs).  Results are bit-identical to direct launches.  Calls on
  *     the legacy default stream, calls made while the caller is capturing `stream`, and calls with per-kernel profiling

@@ -223,7 +223,7 @@ gdn_status_t forward_impl(gdn_plan_t* p, const void* q, const void* k, const voi
 
 
 
-// The frame-wise paths are up to six launches on two streams per call; at the paper's production chunk (8 MB of
+// The frame-wise paths are three to five launches per call (two streams where the normaliser runs as a pass of its own); at the paper's production chunk (8 MB of
 // input) the host cannot issue them as fast as the GPU retires them.  So a call is captured ONCE per tuple of argument
 // pointers into a CUDA graph (fork / join with the normaliser's stream and the programmatic launch edges included) and
 // replayed afterwards: one graph launch per call.  Not used when per-kernel profiling is on, when the caller is itself
@@ -435,8 +435,8 @@ gdn_status_t gdn_plan(const gdn_config_t* cfg, gdn_plan_t** plan_out) {
                 if (ts != GDN_OK) { gdn::tc_plan_free(p->tc); delete p; return fail(nullptr, ts, msg); }
             }
             // frame path with the normaliser: Phase A and the scan run twice (matrix and z pass), the readout once; at d = 128
-            // without a token split one launch does Phase A of both passes
-            p->path = path; p->chunk = chunk; p->launches = (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_NORMALIZER)) ? 2 * launches - 1 - ((p->tc.D == 128 && p->tc.NSPLIT == 1) ? 1 : 0) : launches;
+            // without a token split one launch does Phase A of both passes and one launch their scans
+            p->path = path; p->chunk = chunk; p->launches = (path == GDN_PATH_TC_FRAME && (c.flags & GDN_FLAG_NORMALIZER)) ? ((p->tc.D == 128 && p->tc.NSPLIT == 1) ? launches : 2 * launches - 1) : launches;
             p->workspace_bytes = p->tc.workspace_bytes;
         }
     }

@@ -453,7 +453,7 @@ template <int D>
 inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmQ,
                                    const FrmParams& fp, const TokParams& cp, cudaStream_t st, Profiler* prof,
                                    cudaEvent_t before_readout = nullptr, bool readout = true, const CUtensorMap* tmQr = nullptr,
-                                   bool phase_a = true) {
+                                   bool phase_a = true, TcPlan* zt = nullptr, const TokParams* zc = nullptr) {
     using namespace frm;
     const size_t smem1 = SumSmem<D>::TOTAL;
     const size_t smem2 = tok::ChainSmem<D>::TOTAL;
@@ -462,6 +462,7 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
         cudaError_t e = set_smem(gdn_frm_summaries<D>, smem1);
         if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain<D>, smem2);
         if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain_bidir<D>, smem2);
+        if (e == cudaSuccess) e = set_smem(tok::gdn_tok_chain_multi<D>, smem2);
         if (e == cudaSuccess) e = set_smem(gdn_frm_readout<D>, smem3);
         if (e != cudaSuccess) return e;
         tp.attr_mask |= 16u;
@@ -478,17 +479,39 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     }
     if (prof && phase_a) prof->mark(st, "gdn_frm_summaries");
     const int nchain = tp.BH * (cp.col_tiles ? cp.col_tiles : D / 64);
-    if (tp.bidir && tp.F > 1) {
-        // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero
-        // state; then S^hist = S> + S< in place in the forward snapshots
-        TokParams rp = cp;
-        rp.rev = 1; rp.NCa = tp.F; rp.NC = tp.F - 1; rp.NSc = tp.F; rp.S_in = nullptr; rp.S_out = nullptr;
-        rp.z_vec_in = nullptr; rp.z_vec_out = nullptr;              // z< starts from zero as well and is not carried
-        TokParams fwd = cp;
-        fwd.hist_cnt = rp.hist_cnt = tp.hist_cnt;
-        fwd.hist_dst = rp.hist_dst = tp.Sc;
-        fwd.hist_src = rp.hist_src = tp.ScR;
-        fwd.hist_F = rp.hist_F = tp.F;
+    const bool both = tp.bidir && tp.F > 1;
+    // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero state; the CTA of
+    // a (forward, reverse) pair that finishes last forms S^hist = S> + S< in place in the forward snapshots
+    auto scan_pair = [&](TcPlan& t, const TokParams& base, TokParams& fwd, TokParams& rev) {
+        fwd = base;
+        rev = base;
+        rev.rev = 1; rev.NCa = t.F; rev.NC = t.F - 1; rev.NSc = t.F; rev.S_in = nullptr; rev.S_out = nullptr;
+        rev.z_vec_in = nullptr; rev.z_vec_out = nullptr;            // z< starts from zero as well and is not carried
+        fwd.hist_cnt = rev.hist_cnt = t.hist_cnt;
+        fwd.hist_dst = rev.hist_dst = t.Sc;
+        fwd.hist_src = rev.hist_src = t.ScR;
+        fwd.hist_F = rev.hist_F = t.F;
+    };
+    if (zt && zc) {
+        // normalised path with the dual Phase A: the scans of both passes in one launch
+        tok::ChainSets cs{};
+        const int nz = tp.BH * (zc->col_tiles ? zc->col_tiles : D / 64);
+        if (both) {
+            scan_pair(tp, cp, cs.p[0], cs.p[1]);
+            scan_pair(*zt, *zc, cs.p[2], cs.p[3]);
+            cs.n[0] = cs.n[1] = nchain; cs.n[2] = cs.n[3] = nz;
+        } else {
+            cs.p[0] = cp; cs.p[2] = *zc;
+            cs.n[0] = nchain; cs.n[1] = 0; cs.n[2] = nz; cs.n[3] = 0;
+        }
+        const int total = cs.n[0] + cs.n[1] + cs.n[2] + cs.n[3];
+        le = launch_pdl(tok::gdn_tok_chain_multi<D>, dim3(total), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS,
+                        both ? tp.tmScR : tp.tmScS, zt->tmG, zt->tmN, zt->tmScS, both ? zt->tmScR : zt->tmScS, cs);
+        if (le != cudaSuccess) return le;
+        if (prof) prof->mark(st, "gdn_tok_chain_multi");
+    } else if (both) {
+        TokParams fwd, rp;
+        scan_pair(tp, cp, fwd, rp);
         le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScR, fwd, rp, nchain);
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_tok_chain_bidir");
@@ -540,6 +563,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         cudaError_t e = cudaSuccess;
         cudaEvent_t den_ready = nullptr;
         bool dual = false;
+        TokParams zscan{};
         if (na) {
             // z pass (Eq. 20-21 through the same Phase A and scan kernels): K_raw summaries with the constant block as V, the
             // scan on a [D][D] state whose column 0 is z (first 64-column tile only).  It shares nothing with the matrix pass
@@ -584,23 +608,28 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
                 if (e != cudaSuccess) { if (err) *err = std::string("dual Phase A launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
                 if (prof) prof->mark(st, "gdn_frm_summaries_dual");
             }
-            e = cudaEventRecord(tp.zev0, st);         // after everything queued on the caller's stream so far
-            if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
-            if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
-            e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false, nullptr, !dual)
-                             : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false, nullptr, !dual);
-            if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
-            if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+            if (!dual) {
+                e = cudaEventRecord(tp.zev0, st);     // after everything queued on the caller's stream so far
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(tp.zs, tp.zev0, 0);
+                if (e != cudaSuccess) { if (err) *err = std::string("z pass fork: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+                e = (tp.D == 64) ? tc_launch_frame<64>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false)
+                                 : tc_launch_frame<128>(zt, tp.tmKr, tp.tmKr, tp.tmKr, zf, zc, tp.zs, nullptr, nullptr, false);
+                if (e == cudaSuccess) e = cudaEventRecord(tp.zev1, tp.zs);
+                if (e != cudaSuccess) { if (err) *err = std::string("normaliser pass: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
+                den_ready = tp.zev1;
+            } else {
+                zscan = zc;                          // the z scan rides in the matrix pass's scan launch (tc_launch_frame below)
+            }
             fp.den_mode = 1; fp.eps = c.eps; fp.z_sc = zt.Sc;
             fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
             if (na->gate && na->gate != tp.cgate) {
                 if (!tc::make_act_tmap(&tp.tmGt, na->gate, c.B, c.T, c.H, c.d_v, c.group, fp.g_ts, 128, err)) { tp.cgate = nullptr; return GDN_ERR_CUDA; }
                 tp.cgate = na->gate;
             }
-            den_ready = tp.zev1;
         }
         e = (tp.D == 64) ? tc_launch_frame<64>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr, !dual)
-                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr, !dual);
+                         : tc_launch_frame<128>(tp, tp.tmK, tp.tmV, tp.tmQ, fp, cp, st, prof, den_ready, true, na ? &tp.tmQr : nullptr, !dual,
+                                                dual ? tp.zplan : nullptr, dual ? &zscan : nullptr);
         if (e != cudaSuccess) { if (err) *err = std::string("frame tensor-core launch: ") + cudaGetErrorString(e); return GDN_ERR_CUDA; }
         return GDN_OK;
     }

@@ -1037,6 +1037,27 @@ gdn_tok_chain_bidir(const __grid_constant__ CUtensorMap tmG, const __grid_consta
     else chain_body<D>(&tmG, &tmN, &tmScR, pr, (int)blockIdx.x - n_fwd);
 }
 
+// Every scan of the normalised frame path in ONE launch: the matrix pass (forward, and reverse with GDN_FLAG_BIDIR) and the z
+// pass (the same two, on its own summaries and snapshots, first column tile only).  They are independent of one another; as
+// separate launches on two streams the readout behind them had two dependencies and could not be a programmatic dependent.
+// Set s takes the next n[s] CTAs (n[s] = 0: absent).
+struct ChainSets { TokParams p[4]; int n[4]; };
+
+template <int D>
+__global__ void __launch_bounds__(kChainThreads, 1)
+gdn_tok_chain_multi(const __grid_constant__ CUtensorMap tmG, const __grid_constant__ CUtensorMap tmN,
+                    const __grid_constant__ CUtensorMap tmScF, const __grid_constant__ CUtensorMap tmScR,
+                    const __grid_constant__ CUtensorMap tmGz, const __grid_constant__ CUtensorMap tmNz,
+                    const __grid_constant__ CUtensorMap tmSczF, const __grid_constant__ CUtensorMap tmSczR, const ChainSets cs) {
+    int cta = (int)blockIdx.x, s = 0;
+    while (s < 3 && cta >= cs.n[s]) { cta -= cs.n[s]; ++s; }
+    const TokParams p = cs.p[s];
+    const CUtensorMap* g = s < 2 ? &tmG : &tmGz;
+    const CUtensorMap* n = s < 2 ? &tmN : &tmNz;
+    const CUtensorMap* sc = s == 0 ? &tmScF : (s == 1 ? &tmScR : (s == 2 ? &tmSczF : &tmSczR));
+    chain_body<D>(g, n, sc, p, cta);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Kernel 3: output.  grid = BH * NT, block = 128.   O = scale (Qt S_c + Ol)
 //   tmQt: bf16 (D cols, BH*NT*128 rows) box {64, 128}       -> A operand (K-major)
