@@ -58,9 +58,6 @@ struct TcPlan {
     cudaEvent_t zev0 = nullptr, zev1 = nullptr;
     // bidirectional in-chunk scan: reverse-scan snapshots S<_f, bf16 [BH][F][D][D]
     bool bidir = false;
-    __nv_bfloat16* ScR = nullptr;
-    unsigned int* hist_cnt = nullptr;
-    CUtensorMap tmScR;
     const void *cqr = nullptr, *ckr = nullptr;
     CUtensorMap tmQr, tmKr;
 };
@@ -129,8 +126,6 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     const size_t oGam = carve(BH * F * 4), oSc = carve(BH * (F + 1) * D * D * 2), oCnt = carve(BH * F * 4);
     const bool norm = (c.flags & GDN_FLAG_NORMALIZER) != 0;
     tp.bidir = (c.flags & GDN_FLAG_BIDIR) != 0;
-    const size_t oScR = tp.bidir ? carve(BH * F * D * D * 2) : 0;
-    const size_t oHc = tp.bidir ? carve(BH * 2 * 4) : 0;        // (forward, reverse) arrival counters per (b, h, column tile)
     if (cudaMalloc(&tp.workspace, off) != cudaSuccess) {
         cudaGetLastError();
         if (err) *err = "workspace allocation of " + std::to_string(off) + " bytes failed";
@@ -144,11 +139,6 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
     tp.gam = reinterpret_cast<float*>(w + oGam);
     tp.Sc = reinterpret_cast<__nv_bfloat16*>(w + oSc);
     tp.flags = reinterpret_cast<unsigned int*>(w + oCnt);          // per-frame split counters (self-resetting)
-    if (tp.bidir) tp.ScR = reinterpret_cast<__nv_bfloat16*>(w + oScR);
-    if (tp.bidir) {
-        tp.hist_cnt = reinterpret_cast<unsigned int*>(w + oHc);
-        if (cudaMemset(tp.hist_cnt, 0, BH * 2 * 4) != cudaSuccess) { cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr; return GDN_ERR_CUDA; }
-    }
     if (cudaMemset(tp.flags, 0, BH * F * 4) != cudaSuccess) {
         cudaGetLastError(); cudaFree(tp.workspace); tp.workspace = nullptr;
         if (err) *err = "counter initialisation failed";
@@ -162,7 +152,6 @@ inline gdn_status_t tc_plan_init_frame(TcPlan& tp, const gdn_config_t& c, int sm
         const uint64_t dimsS[3] = {D, D, BH * (F + 1)};
         ok = ok && tc::make_tmap(&tp.tmSc, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
         ok = ok && tc::make_tmap(&tp.tmScS, tp.Sc, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dimsS, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
-        if (tp.bidir) ok = ok && tc::make_tmap(&tp.tmScR, tp.ScR, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, err);
     }
     {
         const uint64_t dims[3] = {D, D, BH * F}, str[3] = {4, D * 4, D * D * 4};
@@ -487,10 +476,8 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
         rev = base;
         rev.rev = 1; rev.NCa = t.F; rev.NC = t.F - 1; rev.NSc = t.F; rev.S_in = nullptr; rev.S_out = nullptr;
         rev.z_vec_in = nullptr; rev.z_vec_out = nullptr;            // z< starts from zero as well and is not carried
-        fwd.hist_cnt = rev.hist_cnt = t.hist_cnt;
-        fwd.hist_dst = rev.hist_dst = t.Sc;
-        fwd.hist_src = rev.hist_src = t.ScR;
-        fwd.hist_F = rev.hist_F = t.F;
+        fwd.snap_add = rev.snap_add = 1;                            // both add into the forward snapshots (zeroed by Phase A)
+        rev.snap_off = 1; rev.snap_stride = t.NSc;
     };
     if (zt && zc) {
         // normalised path with the dual Phase A: the scans of both passes in one launch
@@ -506,13 +493,13 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
         }
         const int total = cs.n[0] + cs.n[1] + cs.n[2] + cs.n[3];
         le = launch_pdl(tok::gdn_tok_chain_multi<D>, dim3(total), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS,
-                        both ? tp.tmScR : tp.tmScS, zt->tmG, zt->tmN, zt->tmScS, both ? zt->tmScR : zt->tmScS, cs);
+                        tp.tmScS, zt->tmG, zt->tmN, zt->tmScS, zt->tmScS, cs);
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_tok_chain_multi");
     } else if (both) {
         TokParams fwd, rp;
         scan_pair(tp, cp, fwd, rp);
-        le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScR, fwd, rp, nchain);
+        le = launch_pdl(tok::gdn_tok_chain_bidir<D>, dim3(2 * nchain), dim3(tok::kChainThreads), smem2, st, tp.tmG, tp.tmN, tp.tmScS, tp.tmScS, fwd, rp, nchain);
         if (le != cudaSuccess) return le;
         if (prof) prof->mark(st, "gdn_tok_chain_bidir");
     } else {
@@ -557,6 +544,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
         fp.o_ts = ts(c.o_token_stride, c.d_v);
         fp.scale = c.scale;
         fp.log_alpha = (c.flags & GDN_FLAG_LOG_ALPHA) ? 1 : 0;
+        fp.zero_sc = (tp.bidir && tp.F > 1) ? tp.Sc : nullptr;
         TokParams cp{};
         cp.S_in = S_in; cp.S_out = S_out; cp.Gw = tp.Gw; cp.Nw = tp.Nw; cp.gam = tp.gam; cp.Sc = tp.Sc;
         cp.B = c.B; cp.H = c.H; cp.T = c.T; cp.NT = tp.NT; cp.NC = tp.NC; cp.NCa = tp.NC; cp.NSc = tp.NSc; cp.dr = c.d_k;
@@ -579,6 +567,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
             FrmParams zf = fp;
             zf.part = zt.part; zf.counters = zt.flags; zf.Gw = zt.Gw; zf.Nw = zt.Nw; zf.gam = zt.gam;
             zf.zpass = 1; zf.scale = 1.f;
+            zf.zero_sc = (tp.bidir && tp.F > 1) ? zt.Sc : nullptr;
             TokParams zc = cp;
             zc.Gw = zt.Gw; zc.Nw = zt.Nw; zc.gam = zt.gam; zc.Sc = zt.Sc;
             zc.S_in = nullptr; zc.S_out = nullptr;

@@ -11,8 +11,8 @@
 //                                data, no separate reduction launch.
 //   Phase B  gdn_tok_chain     : S_f = alpha_f S_{f-1} - G_f S_{f-1} + N_f  -- the same one-MMA-per-step chain
 //                                kernel as the token-wise path (Eq. 5: S_f = alpha_f (I - Gram_f) S_{f-1} + A_f)
-//   (bidirectional scan, Alg. 1 l.9-21: forward and reverse scan in ONE launch, gdn_tok_chain_bidir; the CTA of a pair that
-//    finishes last adds S<_f into the forward snapshot S>_f in place, so Phase C reads S^hist with no second output pass, L122)
+//   (bidirectional scan, Alg. 1 l.9-21: forward and reverse scan in ONE launch; both ADD their snapshots into slots that
+//    Phase A zeroes (TMA reduction), so Phase C reads S^hist = S> + S< with no second output pass, L122)
 //   Phase C  gdn_frm_readout   : O_f = scale * Q_f S_f  (every token of frame f reads the post-update state, Eq. 22)
 //                                persistent CTAs over contiguous tile ranges: TMA ring for Q, S_f reloaded only when
 //                                the frame changes, two TMEM accumulators, bf16 tiles leave by TMA store.
@@ -50,6 +50,9 @@ struct FrmParams {
     int den_mode;                // readout: 0 = plain, 1 = normalised
     float eps;
     const __nv_bfloat16* z_sc;   // [BH][NSc][D][D] bf16 snapshots of the z pass (slot f + 1 = the state frame f reads)
+    // Phase A, bidirectional path: slot f + 1 of these snapshots [BH][NSc][D][D] is zeroed (this CTA's column block): both
+    // scans add their states into it (TokParams::snap_add).  NULL = off.
+    __nv_bfloat16* zero_sc;
     // output gate (Eq. 23, the Hadamard product G (.) Y): multiplied in the readout's epilogue, before the
     // bf16 rounding of the tile.  gate [B][T][H][dr] bf16, token stride g_ts; NULL = no gate.
     const __nv_bfloat16* gate;
@@ -248,6 +251,10 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
     const bool m_ok = warp < 4 && ((D == 128) || (lane < 16));
     float a_f = p.alpha[bhf];
     if (p.log_alpha) a_f = expf(a_f);
+    if (p.zero_sc && warp < 4 && split == 0) {
+        __nv_bfloat16* zb = p.zero_sc + (((long long)bh * p.NSc + f + 1) * D) * D + j * HW;
+        for (int idx = tid; idx < D * (HW / 8); idx += 128) st_global_v4(zb + (long long)(idx / (HW / 8)) * D + (idx % (HW / 8)) * 8, 0u, 0u, 0u, 0u);
+    }
     if (p.NSPLIT == 1) {
         // no token split: G_f = alpha_f Gram_f (bf16), N_f = A_f (fp32).  The rows leave TMEM one per thread; written to global
         // memory like that, every store instruction of a warp touches 32 different lines (measured: ~6 us for 128 KB).  They
@@ -559,6 +566,10 @@ gdn_frm_summaries_dual(const __grid_constant__ CUtensorMap tmK, const __grid_con
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
             const FrmParams& q = pass ? pz : p;
+            if (q.zero_sc) {                       // (see FrmParams::zero_sc)
+                __nv_bfloat16* zb = q.zero_sc + (((long long)bh * q.NSc + f + 1) * D) * D + j * HW;
+                for (int idx = tid; idx < D * (HW / 8); idx += 128) st_global_v4(zb + (long long)(idx / (HW / 8)) * D + (idx % (HW / 8)) * 8, 0u, 0u, 0u, 0u);
+            }
             const uint32_t stgG = smem_u32(smem) + (uint32_t)pass * (D * 128 + D * 256), stgN = stgG + D * 128;
 #pragma unroll 1
             for (int cc = 0; cc < NW / 32; ++cc) {

@@ -53,13 +53,11 @@ struct TokParams {
     long long o_ts;              // out token stride (elements)
     float scale;
     int log_alpha;
-    // chain kernel, bidirectional frame path (Alg. 1 l.19-21): S^hist_f = S>_f + S<_f.  The forward and the reverse CTA of a
-    // (b, h, column tile) count themselves in hist_cnt; the one that finishes last adds the reverse snapshots hist_src
-    // [BH][hist_F][D][D] into the forward ones hist_dst [BH][hist_F + 1][D][D] (slot f + 1) for its 64 columns.  NULL = off.
-    unsigned int* hist_cnt;
-    __nv_bfloat16* hist_dst;
-    const __nv_bfloat16* hist_src;
-    int hist_F;
+    // chain kernel, bidirectional frame path (Alg. 1 l.19-21): S^hist_f = S>_f + S<_f.  snap_add = 1: both scans ADD their
+    // snapshots (slots > 0) into the forward snapshot array by TMA reduction; Phase A has zeroed the slots, 0 + a is exact, so the
+    // sum takes one bf16 rounding whichever scan lands first (deterministic), and nothing has to wait for anything.  The reverse
+    // scan's S<_e joins slot e + 1 (snap_off = 1) of an array with snap_stride slots per (b,h) (0 = NSc).
+    int snap_add, snap_off, snap_stride;
 };
 
 
@@ -908,11 +906,14 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
         // ===== TMA producer: refill a stage as soon as the step that used it has ended, and write the bf16
         //       operand tile sS (= state at the start of chunk c) to the workspace for kernel 3 with one TMA
         //       store straight from shared memory (no per-thread global stores on the chain) =====
+        const int sstride = p.snap_stride ? p.snap_stride : p.NSc;
         auto store_snapshot = [&](int c) {           // sS[c & 1] holds the state at the start of chunk c
-            tma_store_3d(tmScp, sS + (c & 1) * L::S_BYTES, n0, 0, bh * p.NSc + ent(c));
+            const int slot = ent(c) + p.snap_off;
+            if (p.snap_add && slot > 0) tma_reduce_add_3d(tmScp, sS + (c & 1) * L::S_BYTES, n0, 0, bh * sstride + slot);
+            else tma_store_3d(tmScp, sS + (c & 1) * L::S_BYTES, n0, 0, bh * sstride + slot);
             tma_store_commit();
         };
-        if (lane == 0) store_snapshot(0);
+        if (lane == 0 && !(p.snap_add && p.rev)) store_snapshot(0);      // (the reverse scan starts from zero: nothing to add)
         for (int c = 0; c < p.NC; ++c) {
             if (lane == 0) tma_store_wait_read();    // snapshot c has left sS[c & 1] before step c+1 may overwrite it
             __syncthreads();                          // end of step c: sS[(c+1) & 1] published, stage c % STAGES free
@@ -921,10 +922,7 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
                 if (c + STAGES < p.NC) issue_loads(c + STAGES);
             }
         }
-        if (lane == 0) {
-            if (p.hist_cnt) { tma_store_wait_all(); __threadfence(); }     // the snapshots are in global memory (read again below)
-            else tma_store_wait_read();              // the snapshots have left shared memory; their writes complete with the kernel
-        }
+        if (lane == 0) tma_store_wait_read();        // the snapshots have left shared memory; their writes complete with the kernel
     } else {
         // ===== state rows: S <- (gamma_c S + N_c) - G_c S =====
         uint32_t ph_mma = 0;
@@ -970,48 +968,6 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
 #pragma unroll
             for (int i = 0; i < 16; ++i)
                 if (n0 + 4 * i < p.dr) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
-        }
-    }
-    if (p.hist_cnt) {
-        // sum of the two scans' snapshots by whichever CTA of the (forward, reverse) pair finishes last: no separate launch
-        // (the element-wise kernel this replaces took 4-5 us per call, most of it launch and drain)
-        __shared__ unsigned int s_last;
-        __syncthreads();
-        if (tid == 0) {
-            const unsigned int prev = atomicAdd(p.hist_cnt + cta, 1u);
-            s_last = prev == 1u ? 1u : 0u;
-            if (prev == 1u) p.hist_cnt[cta] = 0u;    // ready for the next call (stream order)
-        }
-        __syncthreads();
-        if (s_last) {
-            __threadfence();
-            const int total = p.hist_F * D * 8;      // 16-byte pieces of this CTA's 64 columns
-            constexpr int UN = 8;                    // pieces per thread and pass: all 2 UN loads in flight before the first use
-            for (int base = tid; base < total; base += UN * kChainThreads) {
-                uint4* dst[UN];
-                uint4 a[UN], r[UN];
-#pragma unroll
-                for (int u = 0; u < UN; ++u) {
-                    const int idx = base + u * kChainThreads;
-                    const bool ok = idx < total;
-                    const int f = ok ? idx / (D * 8) : 0, row = (idx >> 3) % D, c = idx & 7;
-                    dst[u] = ok ? reinterpret_cast<uint4*>(p.hist_dst + (((long long)bh * (p.hist_F + 1) + f + 1) * D + row) * D + n0 + c * 8) : nullptr;
-                    if (ok) {
-                        r[u] = __ldcg(reinterpret_cast<const uint4*>(p.hist_src + (((long long)bh * p.hist_F + f) * D + row) * D + n0 + c * 8));
-                        a[u] = __ldcg(dst[u]);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < UN; ++u) {
-                    if (!dst[u]) continue;
-                    float x[8], y[8];
-                    unpack8(a[u], x); unpack8(r[u], y);
-                    uint4 o;
-                    o.x = pack_bf16(x[0] + y[0], x[1] + y[1]); o.y = pack_bf16(x[2] + y[2], x[3] + y[3]);
-                    o.z = pack_bf16(x[4] + y[4], x[5] + y[5]); o.w = pack_bf16(x[6] + y[6], x[7] + y[7]);
-                    *dst[u] = o;
-                }
-            }
         }
     }
     tc_fence_before();
