@@ -469,8 +469,8 @@ inline cudaError_t tc_launch_frame(TcPlan& tp, const CUtensorMap& tmK, const CUt
     if (prof && phase_a) prof->mark(st, "gdn_frm_summaries");
     const int nchain = tp.BH * (cp.col_tiles ? cp.col_tiles : D / 64);
     const bool both = tp.bidir && tp.F > 1;
-    // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero state; the CTA of
-    // a (forward, reverse) pair that finishes last forms S^hist = S> + S< in place in the forward snapshots
+    // Alg. 1 l.9-21: forward scan and, in the same launch, the reverse scan over the frames F-1 .. 1 from a zero state; both ADD
+    // their snapshots into the forward snapshot slots (zeroed by Phase A): S^hist = S> + S< with no pass of its own
     auto scan_pair = [&](TcPlan& t, const TokParams& base, TokParams& fwd, TokParams& rev) {
         fwd = base;
         rev = base;
