@@ -963,11 +963,25 @@ __device__ __forceinline__ void chain_body(const CUtensorMap* tmGp, const CUtens
         }
         if (p.zvec) {
             if (m_ok && m < p.dr && ct == 0 && p.z_vec_out) p.z_vec_out[(long long)bh * p.dr + m] = S[0];
-        } else if (m_ok && m < p.dr && p.S_out) {
-            float4* dst = reinterpret_cast<float4*>(p.S_out + ((long long)bh * p.dr + m) * p.dr + n0);
+        } else if (p.S_out) {
+            // The state rows leave through shared memory (the operand stages are idle now; 16-byte chunks XOR-ed with the row
+            // against bank conflicts) so that a warp writes whole 256-byte row segments: row-per-thread stores (32 lines per
+            // request) took 1.5 us here, and the next kernel waits for this one to complete.
+            const uint32_t stg = smem_u32(sStage);
+            if (m_ok) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i)
-                if (n0 + 4 * i < p.dr) dst[i] = make_float4(S[4 * i], S[4 * i + 1], S[4 * i + 2], S[4 * i + 3]);
+                for (int i = 0; i < 16; ++i)
+                    st_shared_v4(stg + (uint32_t)m * 256u + (uint32_t)((i ^ (m & 15)) << 4), __float_as_uint(S[4 * i]), __float_as_uint(S[4 * i + 1]),
+                                 __float_as_uint(S[4 * i + 2]), __float_as_uint(S[4 * i + 3]));
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int idx = tid; idx < D * 16; idx += 128) {
+                const int row = idx >> 4, c = idx & 15;
+                if (row < p.dr && n0 + 4 * c < p.dr) {
+                    const uint4 u = ld_shared_v4(stg + (uint32_t)row * 256u + (uint32_t)((c ^ (row & 15)) << 4));
+                    st_global_v4(p.S_out + ((long long)bh * p.dr + row) * p.dr + n0 + 4 * c, u.x, u.y, u.z, u.w);
+                }
+            }
         }
     }
     tc_fence_before();
