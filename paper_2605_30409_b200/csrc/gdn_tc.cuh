@@ -417,7 +417,9 @@ inline cudaError_t tc_launch_fused(TcPlan& tp, const TokParams& p, cudaStream_t 
     fp.epoch = ++tp.epoch;
     fp.NWC = tp.NWC; fp.HPR = tp.HPR; fp.total_tiles = tp.BH * tp.NT;
     if (prof) prof->begin(st);
-    fused::gdn_tok_fused<D><<<tp.grid, fused::kThreads, smem, st>>>(tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt, tp.tmO, fp);
+    cudaError_t le = launch_pdl(fused::gdn_tok_fused<D>, dim3(tp.grid), dim3(fused::kThreads), smem, st, tp.tmQ, tp.tmK, tp.tmV, tp.tmG, tp.tmN, tp.tmQt,
+                                tp.tmO, fp);
+    if (le != cudaSuccess) return le;
     if (prof) prof->mark(st, "gdn_tok_fused");
     return cudaGetLastError();
 }

@@ -120,6 +120,11 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    // The kernel is launched as a programmatic dependent of whatever precedes it in the stream (normally the previous call's
+    // launch of this kernel): its CTAs take the SMs as the previous grid's CTAs leave, set themselves up, and wait here,
+    // before their first global access, until that grid has completed.
+    pdl_launch_dependents();
+    pdl_wait();
     const uint32_t acc_chain = tmem;
     const int NT = p.NT;
     const int nunits = p.B * p.H * NCT;
@@ -385,6 +390,20 @@ __device__ __forceinline__ void prepass_role(uint8_t* smem, const CUtensorMap* t
         const int hr = min(fp.HPR, BH - r * fp.HPR);
         tile = il / hr; bh = r * fp.HPR + il % hr;
     };
+    // (see chain_role)  The first tile's operands are the caller's: asked into L2 while the previous grid finishes.
+    pdl_launch_dependents();
+    if (tid == 0 && w < fp.total_tiles) {
+        constexpr int NBp = D / 64;
+        int bh0, t0;
+        tile_of(w, bh0, t0);
+#pragma unroll
+        for (int nb = 0; nb < NBp; ++nb) {
+            tma_prefetch_5d(tmK, nb * 64, bh0 % p.H, t0 * 128, 0, bh0 / p.H);
+            tma_prefetch_5d(tmQ, nb * 64, bh0 % p.H, t0 * 128, 0, bh0 / p.H);
+            tma_prefetch_5d(tmV, nb * 64, bh0 % p.H, t0 * 128, 0, bh0 / p.H);
+        }
+    }
+    pdl_wait();
     for (int i = w; i < fp.total_tiles; i += nwp, ++it) {
         int bh, tile, nbh = -1, ntile = -1;
         tile_of(i, bh, tile);
