@@ -58,8 +58,10 @@ struct ChainSmem {
     static constexpr uint32_t GN_BYTES = G_BYTES + N_BYTES;
     static constexpr uint32_t Q_BYTES = 128u * D * 2;                 // NB blocks of [128][64] bf16; block 0 then stages the out tile
     static constexpr uint32_t S_BYTES = (uint32_t)D * 128;            // [D][64] bf16
-    static constexpr int GST = (D == 128) ? 2 : 3;
-    static constexpr int QST = (D == 128) ? 2 : 3;
+    // d = 64: six stages each (the chain CTA has the SM to itself: 216 KB): a step moves 48 KB through one SM's TMA path, and
+    // with three stages in flight that path ran at the latency-bound ~50 GB/s (config 2: 41.6 -> 41.15 us)
+    static constexpr int GST = (D == 128) ? 2 : 6;
+    static constexpr int QST = (D == 128) ? 2 : 6;
     static constexpr int NSB = (D == 128) ? 2 : 3;                    // bf16 state operand buffers
     static constexpr uint32_t OFF_Q = GST * GN_BYTES;
     static constexpr uint32_t OFF_S = OFF_Q + QST * Q_BYTES;
