@@ -319,6 +319,7 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
         const int ew = warp - 8;
         const int row = ew * 32 + lane;
         uint32_t gs = 0;
+        int prev_qst = -1;
         for (int u = blockIdx.x; u < nunits; u += fp.NWC) {
             const int bh = u / NCT, ct = u % NCT;
             const int b = bh / p.H, h = bh % p.H;
@@ -345,14 +346,27 @@ __device__ __forceinline__ void chain_role(uint8_t* smem, const CUtensorMap* tmG
                 fence_proxy_async();
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 if (warp == 8 && lane == 0) {
+                    // the slot goes back to the producer once the reduction has READ it: checked one step later, so that this
+                    // thread (and with it the next step's barrier) does not sit out the read of the tile it has just sent
+                    // (deep ring only: with two slots the late release starves the producer -- config 5 180 -> 270 us)
                     tma_reduce_add_5d(tmO, sQ + qst * L::Q_BYTES, ct * 64, h, c * 128, 0, b);
                     tma_store_commit();
-                    tma_store_wait_read();
-                    mbar_arrive(&q_empty[qst]);
+                    if (QST >= 4) {
+                        tma_store_wait_read_but1();
+                        if (prev_qst >= 0) mbar_arrive(&q_empty[prev_qst]);
+                        prev_qst = qst;
+                    } else {
+                        tma_store_wait_read();
+                        mbar_arrive(&q_empty[qst]);
+                    }
                 }
             }
         }
-        if (warp == 8 && lane == 0) tma_store_wait_all();
+        if (warp == 8 && lane == 0) {
+            tma_store_wait_read();
+            if (prev_qst >= 0) mbar_arrive(&q_empty[prev_qst]);
+            tma_store_wait_all();
+        }
     }
     tc_fence_before();
     __syncthreads();
