@@ -228,9 +228,15 @@ gdn_status_t gdn_forward_chunk_full(gdn_plan_t* plan, const gdn_featmap_args_t* 
 
 /*
  * gdn_forward_chunk_host: the same operator with HOST buffers (dense layouts, strides in the plan are
- *   ignored; pinned memory recommended).  Copies the inputs to plan-owned device staging buffers on
- *   `stream`, runs gdn_forward_chunk, copies out and state_out back, and returns without synchronising:
- *   the caller synchronises `stream` before reading the results.  state_in_host may be NULL.
+ *   ignored; pinned memory recommended).  Copies the inputs to plan-owned device staging buffers,
+ *   runs gdn_forward_chunk on `stream`, copies out and state_out back on `stream`, and returns without
+ *   synchronising: the caller synchronises `stream` before reading the results.  state_in_host may be NULL.
+ *   ORDERING of the input copies: q, k, v, alpha, beta must hold their data WHEN THE CALL IS MADE (they are host
+ *   memory): they are copied on internal streams that do not wait for work queued earlier on `stream`, so that
+ *   in a sequence of calls the copy-in of call i+1 overlaps the compute and copy-out of call i (two staging
+ *   sets).  state_in_host IS read in stream order (a stream of chunks hands the state on through host
+ *   memory), and so is every input that overlaps out_host / state_out_host of the plan's previous host call.
+ *   As before, no host buffer of a call may be overwritten until `stream` has reached the end of that call.
  */
 gdn_status_t gdn_forward_chunk_host(gdn_plan_t* plan,
                                     const void* q_host, const void* k_host, const void* v_host,

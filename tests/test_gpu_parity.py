@@ -744,3 +744,32 @@ def test_host_entry_point_pipelined_across_calls():
             torch.cuda.synchronize()
             assert torch.equal(o, od.cpu())
         assert torch.equal(hs, S.cpu())
+
+
+def test_host_entry_point_input_that_is_the_previous_calls_output_stays_in_stream_order():
+    """The copy-in of an unsegmented host call does not wait for the caller's stream -- EXCEPT when an input overlaps a host
+    buffer the previous call writes (gdn.h).  Call 2 takes call 1's out_host as its v_host, with no synchronisation in
+    between: the result must be what two device calls chained through that tensor give."""
+    B, H, T, d = 1, 4, 1024, 64
+    dev = torch.device("cuda:0")
+    pin = lambda t: t.contiguous().pin_memory()
+    x1 = gin.make_inputs(gin.GdnWorkload("hostchain", B, H, T, d, d, seed=90), with_state=False)
+    x2 = gin.make_inputs(gin.GdnWorkload("hostchain", B, H, T, d, d, seed=91), with_state=False)
+    h1 = tuple(map(pin, (x1.q, x1.k, x1.v, x1.alpha, x1.beta)))
+    h2 = tuple(map(pin, (x2.q, x2.k, x2.v, x2.alpha, x2.beta)))
+    o1 = torch.full((B, T, H, d), float("nan"), dtype=torch.bfloat16).pin_memory()
+    o2 = torch.full((B, T, H, d), float("nan"), dtype=torch.bfloat16).pin_memory()
+    hs = pin(torch.zeros(B, H, d, d))
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d) as p:
+        for _ in range(3):                                   # (the third round runs with both staging sets in use)
+            hs.zero_()
+            p.forward_host(h1[0], h1[1], h1[2], h1[3], h1[4], hs, o1, hs)
+            p.forward_host(h2[0], h2[1], o1, h2[3], h2[4], hs, o2, hs)       # v = the previous call's output
+            torch.cuda.synchronize()
+        S = torch.zeros(B, H, d, d, device=dev)
+        d1 = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+        d2 = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+        p.forward(x1.q.to(dev), x1.k.to(dev), x1.v.to(dev), x1.alpha.to(dev), x1.beta.to(dev), S, d1, S)
+        p.forward(x2.q.to(dev), x2.k.to(dev), d1, x2.alpha.to(dev), x2.beta.to(dev), S, d2, S)
+        torch.cuda.synchronize()
+        assert torch.equal(o1, d1.cpu()) and torch.equal(o2, d2.cpu()) and torch.equal(hs, S.cpu())
