@@ -278,7 +278,7 @@ inline gdn_status_t tc_plan_init(TcPlan& tp, const gdn_config_t& c, int sm_count
         tp.HPR = hpr;
         tp.NWC = hpr * nct;
         long long nwp = (long long)sms - tp.NWC;
-        if (nwp > (long long)BH * NT) nwp = (long long)BH * NT;
+        if (nwp > (long long)(BH * NT)) nwp = (long long)(BH * NT);
         if (nwp < 1) nwp = 1;
         tp.grid = tp.NWC + (int)nwp;
     }
