@@ -773,3 +773,31 @@ def test_host_entry_point_input_that_is_the_previous_calls_output_stays_in_strea
         p.forward(x2.q.to(dev), x2.k.to(dev), d1, x2.alpha.to(dev), x2.beta.to(dev), S, d2, S)
         torch.cuda.synchronize()
         assert torch.equal(o1, d1.cpu()) and torch.equal(o2, d2.cpu()) and torch.equal(hs, S.cpu())
+
+
+@pytest.mark.parametrize("B,H,G,F,d", [
+    (1, 20, 40, 6, 128),        # frames shorter than one 64-token tile of the dual Phase A
+    (1, 40, 65, 7, 128),        # one token over a tile, seven frames, more (b, h, f, column) units than SMs
+    (2, 10, 64, 3, 128),        # exactly one tile per frame
+    (1, 20, 129, 3, 64),        # d = 64: the two-stream path (no dual Phase A), one token over a 128-token tile
+])
+def test_normalised_bidirectional_short_and_ragged_frames(B, H, G, F, d):
+    """Alg. 1 with the normalised readout on frame lengths around the tile sizes of Phase A (64 tokens in the dual kernel,
+    128 otherwise), called twice on the same plan (the bidirectional path adds both scans into snapshot slots that Phase A
+    must have zeroed again)."""
+    import oracle
+    T = G * F
+    dev = torch.device("cuda:0")
+    wl = gin.GdnWorkload("ragged", B, H, T, d, d, group=G, seed=77)
+    inp = gin.make_normalizer_inputs(wl)
+    ex = inp.extras
+    out = torch.empty(B, T, H, d, device=dev, dtype=torch.bfloat16)
+    with gdn.GdnPlan(B=B, H=H, T=T, d_k=d, d_v=d, group=G, flags=gdn.GDN_FLAG_NORMALIZER | gdn.GDN_FLAG_BIDIR) as p:
+        for _ in range(2):
+            S, z = inp.state.to(dev), ex["z_in"].to(dev)
+            p.forward_norm(inp.q.to(dev), inp.k.to(dev), inp.v.to(dev), ex["q_raw"].to(dev), ex["k_raw"].to(dev),
+                           inp.alpha.to(dev), inp.beta.to(dev), S, z, out, S, z)
+            torch.cuda.synchronize()
+    o_ref, S_ref, z_ref = oracle.gdn_forward(inp.q, inp.k, inp.v, inp.alpha, inp.beta, inp.state, group=G, q_raw=ex["q_raw"],
+                                             k_raw=ex["k_raw"], z_in=ex["z_in"], normalizer=True, bidir=True)
+    assert rel_err(out.cpu(), o_ref) <= TOL_BF16 and rel_err(S.cpu(), S_ref) <= TOL_BF16 and rel_err(z.cpu(), z_ref) <= TOL_BF16
