@@ -444,6 +444,11 @@ def roofline(wl, info, kernels, ms_per_step, pk, pk_src, by):
         top = max(kernels, key=lambda k: k["avg_us"])
         dur_ms, name = top["avg_us"] * 1e-3, top["name"]
         kb = kernel_bytes(name, wl, by)
+        if len(kernels) == 1 and info.launches_per_call == 1:
+            # one launch per step: the kernel's average launch duration over the TIMED region is the step time itself (CUDA
+            # events around the K steps).  The per-kernel pass puts an event pair around every launch, which keeps the
+            # programmatic launches of consecutive calls from overlapping their set-up with the previous grid's tail.
+            dur_ms = ms_per_step
     achieved = kb / (dur_ms * 1e-3) / 1e9
     # what the measurements say limits the kernel: below half of the HBM roofline (and, for the token path, with the
     # tensor pipe at 10-20 % in the ncu captures) the dominant kernel is bound by the latency of its dependent steps
