@@ -303,13 +303,17 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
             if (tid == 0 && j == 0) p.gam[bhf] = a_f;
         }
     } else {
-        // partial [Gram | A] of this split -> workspace (fp32, full-width rows [D][2D]; this CTA owns its columns)
+        // partial [Gram | A] of this split -> workspace (fp32, full-width rows [D][2D]; this CTA owns its columns).  Staged in
+        // shared memory like the unsplit epilogue above (row-per-thread global stores touch 32 lines per instruction) and
+        // copied out as whole 512-byte row segments, one per warp and instruction.
         if (warp < 4) {
-            float* dst = p.part + (((long long)bhf * p.NSPLIT + split) * D + m) * (2 * D) + j * HW;
             if (ntiles > 0) {
                 mbar_wait(bar_done, 0);
                 tc_fence_after();
             }
+            constexpr uint32_t ROWB = NW * 4;           // bytes of a staged row: [Gram block | A block] fp32
+            constexpr int CH = NW / 4;                  // 16-byte chunks per row
+            const uint32_t stg = smem_u32(smem);
 #pragma unroll 1
             for (int cc = 0; cc < NW / 32; ++cc) {
                 float v[32];
@@ -319,13 +323,21 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
 #pragma unroll
                     for (int e = 0; e < 32; ++e) v[e] = 0.f;
                 }
-                float* d2 = dst + (cc / (HW / 32)) * D + (cc % (HW / 32)) * 32;
                 if (m_ok) {
 #pragma unroll
                     for (int q4 = 0; q4 < 8; ++q4)
-                        st_global_v4(d2 + q4 * 4, __float_as_uint(v[4 * q4]), __float_as_uint(v[4 * q4 + 1]),
-                                     __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
+                        st_shared_v4(stg + (uint32_t)m * ROWB + (uint32_t)(((cc * 8 + q4) ^ (m & 7)) << 4), __float_as_uint(v[4 * q4]),
+                                     __float_as_uint(v[4 * q4 + 1]), __float_as_uint(v[4 * q4 + 2]), __float_as_uint(v[4 * q4 + 3]));
                 }
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            float* pbase = p.part + ((long long)bhf * p.NSPLIT + split) * D * (2 * D) + j * HW;
+#pragma unroll 4
+            for (int idx = tid; idx < D * CH; idx += 128) {
+                const int row = idx / CH, c = idx % CH;
+                const uint4 u = ld_shared_v4(stg + (uint32_t)row * ROWB + (uint32_t)((c ^ (row & 7)) << 4));
+                const int col = c * 4;
+                st_global_v4(pbase + (long long)row * (2 * D) + (col < HW ? col : D + (col - HW)), u.x, u.y, u.z, u.w);
             }
         }
         // the last CTA of the frame to get here reduces all partials in split order
@@ -343,7 +355,8 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
             const float4* src = reinterpret_cast<const float4*>(p.part + (long long)bhf * p.NSPLIT * D * 2 * D);
             constexpr int ROW4 = 2 * D / 4;             // float4 per summary row
             constexpr int TOT4 = D * ROW4;
-            constexpr int UN = 4;                       // independent float4 columns per thread per pass (loads in flight)
+            constexpr int UN = 4;                       // independent float4 columns per thread per pass ...
+            constexpr int SG = 4;                       // ... times splits per group: UN * SG loads in flight per thread
             for (int e0 = tid; e0 < TOT4; e0 += UN * kSumThreads) {
                 float4 acc[UN];
 #pragma unroll
@@ -351,15 +364,19 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
                     const int e = e0 + u * kSumThreads;
                     acc[u] = (e < TOT4) ? __ldcg(src + e) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
-                for (int s = 1; s < p.NSPLIT; ++s) {
-                    float4 v[UN];
+                for (int s0 = 1; s0 < p.NSPLIT; s0 += SG) {             // fixed split order; an absent split adds 0
+                    float4 v[SG][UN];
 #pragma unroll
-                    for (int u = 0; u < UN; ++u) {
-                        const int e = e0 + u * kSumThreads;
-                        v[u] = (e < TOT4) ? __ldcg(src + (long long)s * TOT4 + e) : make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
+                    for (int g = 0; g < SG; ++g)
 #pragma unroll
-                    for (int u = 0; u < UN; ++u) { acc[u].x += v[u].x; acc[u].y += v[u].y; acc[u].z += v[u].z; acc[u].w += v[u].w; }
+                        for (int u = 0; u < UN; ++u) {
+                            const int e = e0 + u * kSumThreads;
+                            v[g][u] = (s0 + g < p.NSPLIT && e < TOT4) ? __ldcg(src + (long long)(s0 + g) * TOT4 + e) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        }
+#pragma unroll
+                    for (int g = 0; g < SG; ++g)
+#pragma unroll
+                        for (int u = 0; u < UN; ++u) { acc[u].x += v[g][u].x; acc[u].y += v[g][u].y; acc[u].z += v[g][u].z; acc[u].w += v[g][u].w; }
                 }
 #pragma unroll
                 for (int u = 0; u < UN; ++u) {
