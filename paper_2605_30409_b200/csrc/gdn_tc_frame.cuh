@@ -154,6 +154,7 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
             // The ring holds what fits in shared memory (three tiles); the DRAM latency of a tile (~3500 cycles measured from
             // issue to arrival with the ring alone) is taken earlier, by an L2 prefetch kPF tiles ahead of the load.
             constexpr int kPF = 3;
+            const uint64_t pol = l2_policy_evict_first();      // K and V are streamed (K is read by the sibling column CTA within a tile time)
             auto prefetch = [&](int i) {
                 const int n0 = (tile_lo + i) * 128;
                 if (j == 0) {                     // the column CTAs of a frame read the same K: one of them prefetches it
@@ -177,13 +178,13 @@ gdn_frm_summaries(const __grid_constant__ CUtensorMap tmK, const __grid_constant
                 mbar_expect_tx(&bar_full[st], zp ? L::KTILE : L::STAGE);
                 const int n0 = (tile_lo + i) * 128;
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + nb * kBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(base + nb * kBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b, pol);
                 if (zp) continue;                  // no V: the constant block stands in
                 if (NC == 1) {
 #pragma unroll
-                    for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + (NB + nb) * kBlk, &tmV, &bar_full[st], nb * 64, h, n0, f, b);
+                    for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(base + (NB + nb) * kBlk, &tmV, &bar_full[st], nb * 64, h, n0, f, b, pol);
                 } else {
-                    tma_load_5d(base + NB * kBlk, &tmV, &bar_full[st], j * 64, h, n0, f, b);
+                    tma_load_5d_hint(base + NB * kBlk, &tmV, &bar_full[st], j * 64, h, n0, f, b, pol);
                 }
             }
         }
@@ -483,6 +484,7 @@ gdn_frm_summaries_dual(const __grid_constant__ CUtensorMap tmK, const __grid_con
         // ===== TMA producer =====
         if (elect_one()) {
             constexpr int kPF = 4;                 // L2 prefetch distance (64-token tiles) ahead of the ring
+            const uint64_t pol = l2_policy_evict_first();
             auto prefetch = [&](int i) {
                 const int n0 = i * 64;
                 if (j == 0) {
@@ -500,10 +502,10 @@ gdn_frm_summaries_dual(const __grid_constant__ CUtensorMap tmK, const __grid_con
                 mbar_expect_tx(&bar_full[st], L::STAGE);
                 const int n0 = i * 64;
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + nb * kHBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b);
-                tma_load_5d(base + L::KT, &tmV, &bar_full[st], j * 64, h, n0, f, b);
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(base + nb * kHBlk, &tmK, &bar_full[st], nb * 64, h, n0, f, b, pol);
+                tma_load_5d_hint(base + L::KT, &tmV, &bar_full[st], j * 64, h, n0, f, b, pol);
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(base + L::KT + kHBlk + nb * kHBlk, &tmKr, &bar_full[st], nb * 64, h, n0, f, b);
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(base + L::KT + kHBlk + nb * kHBlk, &tmKr, &bar_full[st], nb * 64, h, n0, f, b, pol);
             }
         }
     }
@@ -703,14 +705,14 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const int st = i % qst;
                 mbar_expect_tx(&q_full[st], L::Q_BYTES);
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(smem + st * L::Q_BYTES + nb * kBlk, &tmQ, &q_full[st], nb * 64, bh % p.H, tile * 128, f, bh / p.H, l2_policy_evict_first());
             };
             auto load_qr = [&](int t) {
                 const int bhf = t / p.TPF, tile = t % p.TPF;
                 const int f = bhf % p.F, bh = bhf / p.F;
                 mbar_expect_tx(qr_full, L::Q_BYTES);
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_load_5d(sQr + nb * kBlk, &tmQr, qr_full, nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+                for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(sQr + nb * kBlk, &tmQr, qr_full, nb * 64, bh % p.H, tile * 128, f, bh / p.H, l2_policy_evict_first());
             };
             for (int i = 0; i < qst && t_lo + i < t_hi; ++i) load_q(t_lo + i, i);
             if (norm && t_lo < t_hi) load_qr(t_lo);
@@ -777,7 +779,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const int f = bhf % p.F, bh = bhf / p.F;
             mbar_expect_tx(&g_full[i & 1], L::Q_BYTES);
 #pragma unroll
-            for (int nb = 0; nb < NB; ++nb) tma_load_5d(sO + (i & 1) * L::Q_BYTES + nb * kBlk, &tmGt, &g_full[i & 1], nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+            for (int nb = 0; nb < NB; ++nb) tma_load_5d_hint(sO + (i & 1) * L::Q_BYTES + nb * kBlk, &tmGt, &g_full[i & 1], nb * 64, bh % p.H, tile * 128, f, bh / p.H, l2_policy_evict_first());
         };
         if (gated && tid == 0 && t_lo < t_hi) load_gate(t_lo, 0);
         for (int t = t_lo, i = 0; t < t_hi; ++t, ++i) {
@@ -868,7 +870,7 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (tid == 0) {
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) tma_store_5d(&tmO, sO + a * L::Q_BYTES + nb * kBlk, nb * 64, bh % p.H, tile * 128, f, bh / p.H);
+                for (int nb = 0; nb < NB; ++nb) tma_store_5d_hint(&tmO, sO + a * L::Q_BYTES + nb * kBlk, nb * 64, bh % p.H, tile * 128, f, bh / p.H, l2_policy_evict_first());
                 tma_store_commit();
             }
         }
