@@ -41,6 +41,20 @@ struct GateParams {
 
 namespace fe {
 
+// a 16-byte read of data that is used once (q, k, x): non-coherent path, and an L2 evict-first policy so that the stream does
+// not push the previous kernel's dirty lines (or the feature tensors this kernel writes for the next one) out of L2
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p, uint64_t pol) {
+    uint4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ uint64_t stream_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+
 __device__ __forceinline__ void unpack8f(const uint4& u, float (&f)[8]) {
     const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
 #pragma unroll
@@ -88,8 +102,8 @@ __device__ __forceinline__ void featmap_body(const FeatmapParams& p, int block, 
 #pragma unroll
             for (int i = 0; i < 8; ++i) { xq[j][i] = 0.f; xk[j][i] = 0.f; }
             if (on) {
-                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.q + bt * p.q_ts + (long long)h * p.D + c0)), xq[j]);
-                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.k + bt * p.k_ts + (long long)h * p.D + c0)), xk[j]);
+                unpack8f(ldg_stream(reinterpret_cast<const uint4*>(p.q + bt * p.q_ts + (long long)h * p.D + c0), stream_policy()), xq[j]);
+                unpack8f(ldg_stream(reinterpret_cast<const uint4*>(p.k + bt * p.k_ts + (long long)h * p.D + c0), stream_policy()), xk[j]);
             }
         }
 #pragma unroll
@@ -162,7 +176,7 @@ __device__ __forceinline__ void gates_body(const GateParams& p, int bhf, int s, 
 #pragma unroll
             for (int i = 0; i < 8; ++i) x[j][i] = 0.f;
             if (on && valid[j])
-                unpack8f(__ldg(reinterpret_cast<const uint4*>(p.x + ((long long)b * p.T + (long long)f * p.G + n) * p.x_ts + (long long)h * p.D + c0)), x[j]);
+                unpack8f(ldg_stream(reinterpret_cast<const uint4*>(p.x + ((long long)b * p.T + (long long)f * p.G + n) * p.x_ts + (long long)h * p.D + c0), stream_policy()), x[j]);
         }
 #pragma unroll
         for (int j = 0; j < R; ++j) {
