@@ -612,6 +612,7 @@ inline gdn_status_t tc_forward(TcPlan& tp, const gdn_config_t& c, const void* q,
                 zscan = zc;                          // the z scan rides in the matrix pass's scan launch (tc_launch_frame below)
             }
             fp.den_mode = 1; fp.eps = c.eps; fp.z_sc = zt.Sc;
+            if (na->dense_qk && c.d_k == 128) { fp.drop_q = static_cast<const __nv_bfloat16*>(q); fp.drop_qr = static_cast<const __nv_bfloat16*>(na->q_raw); }
             fp.gate = static_cast<const __nv_bfloat16*>(na->gate); fp.g_ts = na->g_ts ? na->g_ts : (long long)c.H * c.d_v; fp.dr = c.d_v;
             if (na->gate && na->gate != tp.cgate) {
                 if (!tc::make_act_tmap(&tp.tmGt, na->gate, c.B, c.T, c.H, c.d_v, c.group, fp.g_ts, 128, err)) { tp.cgate = nullptr; return GDN_ERR_CUDA; }

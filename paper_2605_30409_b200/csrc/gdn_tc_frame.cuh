@@ -58,6 +58,11 @@ struct FrmParams {
     const __nv_bfloat16* gate;
     long long g_ts;
     int dr;                      // real head dim (112 when padded to D = 128): channels >= dr are clipped by the store
+    // readout: q_rot / q_raw when they are the plan's OWN feature buffers (gdn_forward_chunk_full; dense [B][T][H][D]): a tile that
+    // has been consumed is dropped from L2 (discard.global.L2), so the dead intermediate is never written back to DRAM.
+    // NULL = the caller's memory, left alone.
+    const __nv_bfloat16* drop_q;
+    const __nv_bfloat16* drop_qr;
 };
 
 namespace frm {
@@ -838,6 +843,14 @@ gdn_frm_readout(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
             mbar_wait(&acc_full[a], (uint32_t)(i >> 1) & 1u);
             tc_fence_after();
+            if (p.drop_q && n < p.G) {                           // the MMAs have read the Q tile (and the dot product above the q_raw tile)
+                const long long roff = ((((long long)(bh / p.H) * p.T + (long long)f * p.G + n) * p.H) + bh % p.H) * D;
+#pragma unroll
+                for (int l = 0; l < D * 2 / 128; ++l) {
+                    asm volatile("discard.global.L2 [%0], 128;" ::"l"(p.drop_q + roff + l * 64) : "memory");
+                    if (p.drop_qr) asm volatile("discard.global.L2 [%0], 128;" ::"l"(p.drop_qr + roff + l * 64) : "memory");
+                }
+            }
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (gated) mbar_wait(&g_full[a], (uint32_t)(i >> 1) & 1u);
             const uint32_t stg = smem_u32(sO + a * L::Q_BYTES);
